@@ -1,0 +1,143 @@
+/*
+ * sangam.h -- C ABI of the B200-native hot path of one cached-dLLM serving iteration
+ * (arxiv/paper_2607_04206, "Sangam").  Plain pointers and sizes; no torch types.
+ *
+ * The two operations follow the paper's statement of the problem:
+ *   - sangam_kv_write:  store freshly computed K/V rows into the paged KV cache
+ *       (PagedAttention, page size 16: PAPER.md:258; the cache is recomputed at
+ *        every block boundary and the current block's K/V change every step: PAPER.md:77).
+ *   - sangam_block_attn: batched, varlen, NON-CAUSAL attention of each request's query rows over
+ *       that request's paged context ("the causal mask is dropped so tokens attend
+ *       bidirectionally over the full prompt-and-response"; a decode "contributes an
+ *       entire response block while attending over the prompt and response context", PAPER.md:33;
+ *       a prefill is one indivisible pass over prompt+response; a hybrid iteration
+ *       mixes decodes and whole prefills in one microbatch, Alg. 1).
+ *
+ * Layouts (all device memory unless a function says "host"; every pointer 16-byte aligned):
+ *   q, out        bf16 [total_q][num_q_heads][head_dim], contiguous, rows of request r are
+ *                 cu_q_lens[r] .. cu_q_lens[r+1]-1
+ *   k, v          bf16 [num_tokens][num_kv_heads][head_dim], contiguous (token-major)
+ *   k_pages,      bf16 [num_pages][num_kv_heads][16][head_dim]  (head-major pages: one
+ *   v_pages         (page, kv head) is one contiguous 16*head_dim*2-byte block)
+ *   block_table   int32 [batch][max_pages_per_req] row-major; entry i of row r is the page holding
+ *                 context positions 16*i .. 16*i+15 of request r.  Entries at or past
+ *                 ceil(ctx_lens[r]/16) are never read and may hold anything.
+ *   cu_q_lens     int32 [batch+1], prefix sums of query rows, cu_q_lens[0] = 0
+ *   ctx_lens      int32 [batch], context length c_r of each request
+ *   slot_mapping  int32 [num_tokens]; slot = page*16 + offset; slot < 0 skips the row
+ * q head h reads kv head h / (num_q_heads / num_kv_heads).  Slots past ctx_lens[r] inside the last
+ * page, and pages no request lists, may hold any bits (NaN included); results never depend on them.
+ *
+ * Ownership: the caller owns every tensor and the stream.  The library owns only the workspace
+ * allocated in sangam_create.  Both calls only enqueue work on `stream`: no host sync, no
+ * allocation, no host read of a device array.  All lengths are read on the device, so a captured
+ * CUDA graph replays correctly after the caller rewrites q/k/v/metadata in the same buffers;
+ * host-side arguments (batch, num_tokens, pointers, scale) are baked into the capture.
+ * Padding (q_r = 0, slot = -1) lets a larger capture serve a smaller batch.
+ *
+ * Errors: every call returns 0 on success or a negative sangam_status; nothing throws or aborts.
+ * sangam_last_error gives a message for the last failing call on that ctx.  Conditions only the
+ * device can see (a context needing more than max_pages_per_req pages, a page id >= num_pages,
+ * a slot >= num_pages*16) never fault: the offending request/row is skipped and a sticky flag is
+ * raised, readable with sangam_device_status after a stream sync.
+ * One ctx per stream; calls on one ctx are not re-entrant.
+ */
+#ifndef SANGAM_H_
+#define SANGAM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sangam_ctx sangam_ctx;
+
+typedef enum {
+    SANGAM_OK = 0,
+    SANGAM_ERR_INVALID_ARG = -1,      /* null pointer, misalignment, count out of range */
+    SANGAM_ERR_UNSUPPORTED = -2,      /* geometry the kernels are not compiled for */
+    SANGAM_ERR_WORKSPACE = -3,        /* batch / total_q above what sangam_create sized */
+    SANGAM_ERR_CUDA = -4              /* CUDA runtime / driver error; see sangam_last_error */
+} sangam_status;
+
+/* sticky device-side flags (sangam_device_status) */
+#define SANGAM_DEV_BAD_SLOT   1u      /* kv_write: slot >= num_pages*16, row skipped */
+#define SANGAM_DEV_BAD_PAGE   2u      /* block_attn: page id out of [0,num_pages), request skipped */
+#define SANGAM_DEV_CTX_TOO_LONG 4u    /* block_attn: ctx_len needs more than max_pages_per_req pages */
+#define SANGAM_DEV_TIMEOUT    8u      /* an in-kernel barrier wait gave up (internal error) */
+
+typedef struct {
+    int32_t num_q_heads;        /* Hq */
+    int32_t num_kv_heads;       /* Hkv, Hq % Hkv == 0 */
+    int32_t head_dim;           /* 64 or 128 */
+    int32_t page_size;          /* must be 16 */
+    int32_t num_pages;          /* P: capacity of each of the K and V pools */
+    int32_t max_batch;          /* largest `batch` of any call */
+    int32_t max_total_q;        /* largest total number of query rows of any call */
+    int32_t max_pages_per_req;  /* W: row width of block_table */
+    int32_t device;             /* CUDA device ordinal */
+} sangam_config;
+
+/* Allocates the workspace once (split-KV partials, host staging for the *_host call). */
+int sangam_create(const sangam_config* cfg, sangam_ctx** out);
+int sangam_destroy(sangam_ctx* ctx);
+
+/*
+ * KV write (step a2): for every i < num_tokens with s = slot_mapping[i] >= 0 and every kv head h,
+ *   k_pages[s/16][h][s%16][:] = k[i][h][:]   and the same for v.   Bit copies, no arithmetic.
+ * Non-negative slots must be unique within one call.  num_tokens = 0 is a no-op.
+ */
+int sangam_kv_write(sangam_ctx* ctx, const void* k, const void* v, const int32_t* slot_mapping,
+                    int32_t num_tokens, void* k_pages, void* v_pages, void* stream);
+
+/*
+ * Block attention (steps a3-a9): for request r < batch, row t in [cu_q_lens[r], cu_q_lens[r+1]),
+ * q head h, kv head g = h / G, context length c = ctx_lens[r]:
+ *   s_j = scale * <q[t][h], K_r[j][g]>, j < c;   out[t][h] = sum_j softmax_j(s) V_r[j][g]
+ * with K_r[j] = k_pages[block_table[r][j/16]][g][j%16].  No mask among j < c.  c = 0 writes zeros.
+ * bf16 inputs, fp32 accumulation, P rounded to bf16 before PV, out = bf16(O / l).
+ * Long contexts are split over CTAs and merged by a combine kernel; results are bitwise
+ * reproducible for fixed inputs.  `total_q` is the host-known number of rows of q/out
+ * (an upper bound is fine: rows past cu_q_lens[batch] are not touched).
+ */
+int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_pages, const void* v_pages,
+                      const int32_t* block_table, const int32_t* cu_q_lens, const int32_t* ctx_lens,
+                      int32_t batch, int32_t total_q, float scale, void* out, void* stream);
+
+/*
+ * Same contract as sangam_block_attn, computed by a plain CUDA-core (no tensor core) kernel with
+ * fp32 arithmetic.  A cross-check for the tcgen05 path on workloads too large for the CPU oracle;
+ * never dispatched by sangam_block_attn.
+ */
+int sangam_block_attn_simt(sangam_ctx* ctx, const void* q, const void* k_pages, const void* v_pages,
+                           const int32_t* block_table, const int32_t* cu_q_lens, const int32_t* ctx_lens,
+                           int32_t batch, int32_t total_q, float scale, void* out, void* stream);
+
+/*
+ * One whole iteration from HOST buffers (the end-to-end entry point): copies q, k, v and the
+ * metadata host->device into ctx-owned staging, runs sangam_kv_write then sangam_block_attn on
+ * `stream`, copies `out` device->host and synchronises the stream.  *_host pointers are host
+ * memory (pinned for full copy speed); k_pages / v_pages are the device pools.
+ */
+int sangam_iteration_host(sangam_ctx* ctx, const void* q_host, const void* k_host, const void* v_host,
+                          const int32_t* slot_mapping_host, int32_t num_tokens,
+                          void* k_pages, void* v_pages,
+                          const int32_t* block_table_host, const int32_t* cu_q_lens_host,
+                          const int32_t* ctx_lens_host, int32_t batch, int32_t total_q,
+                          float scale, void* out_host, void* stream);
+
+/* Reads and clears nothing: returns the sticky device flag word (synchronises the ctx's device). */
+int sangam_device_status(sangam_ctx* ctx, uint32_t* flags);
+int sangam_clear_device_status(sangam_ctx* ctx);
+
+/* Number of kernels this ctx has launched since creation (bench.py's gpu_launches). */
+int64_t sangam_launch_count(const sangam_ctx* ctx);
+
+const char* sangam_last_error(const sangam_ctx* ctx);
+const char* sangam_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SANGAM_H_ */

@@ -1,0 +1,7 @@
+"""sangam-b200: B200-native paged non-causal block attention + KV page write (arxiv/paper_2607_04206).
+
+Thin Python binding over the C ABI in include/sangam.h.  Argument marshalling only: every step
+of the path runs in the CUDA kernels of csrc/.  There is no CPU fallback -- if libsangam.so is
+missing or a CUDA device is absent the calls raise.
+"""
+from .binding import (SangamError, Sangam, load_library, exported_symbols, DECLARED_SYMBOLS)  # noqa: F401

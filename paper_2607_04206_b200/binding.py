@@ -1,0 +1,133 @@
+"""ctypes binding with the same names as include/sangam.h.  torch tensors are used only as
+device memory: the binding passes `tensor.data_ptr()` and the current CUDA stream handle."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libsangam.so")
+
+DECLARED_SYMBOLS = [
+    "sangam_create", "sangam_destroy", "sangam_kv_write", "sangam_block_attn", "sangam_block_attn_simt",
+    "sangam_iteration_host", "sangam_device_status", "sangam_clear_device_status", "sangam_launch_count",
+    "sangam_last_error", "sangam_version",
+]
+
+
+class SangamError(RuntimeError):
+    pass
+
+
+class _Config(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in (
+        "num_q_heads", "num_kv_heads", "head_dim", "page_size", "num_pages", "max_batch", "max_total_q",
+        "max_pages_per_req", "device")]
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = False):
+    """dlopen libsangam.so; fails loudly when it is missing (no fallback path exists)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        if build_if_missing:
+            from .build import build
+            build()
+        else:
+            raise SangamError(f"{LIB_PATH} not built: run `python -m paper_2607_04206_b200.build`")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32, f32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_float
+    lib.sangam_create.argtypes = [ctypes.POINTER(_Config), ctypes.POINTER(vp)]
+    lib.sangam_destroy.argtypes = [vp]
+    lib.sangam_kv_write.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp]
+    lib.sangam_block_attn.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
+    lib.sangam_block_attn_simt.argtypes = lib.sangam_block_attn.argtypes
+    lib.sangam_iteration_host.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
+    lib.sangam_device_status.argtypes = [vp, ctypes.POINTER(ctypes.c_uint32)]
+    lib.sangam_clear_device_status.argtypes = [vp]
+    lib.sangam_launch_count.argtypes = [vp]
+    lib.sangam_launch_count.restype = ctypes.c_int64
+    lib.sangam_last_error.argtypes = [vp]
+    lib.sangam_last_error.restype = ctypes.c_char_p
+    lib.sangam_version.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def exported_symbols():
+    lib = load_library()
+    return [s for s in DECLARED_SYMBOLS if hasattr(lib, s)]
+
+
+def _ptr(t):
+    return ctypes.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _stream(stream):
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+class Sangam:
+    """One sangam_ctx (geometry + library workspace).  Methods mirror the C entry points."""
+
+    def __init__(self, *, num_q_heads, num_kv_heads, head_dim, num_pages, max_batch, max_total_q,
+                 max_pages_per_req, page_size=16, device=0):
+        import torch
+        if not torch.cuda.is_available():
+            raise SangamError("no CUDA device: the sangam kernels have no CPU fallback")
+        self.lib = load_library()
+        self.cfg = _Config(num_q_heads, num_kv_heads, head_dim, page_size, num_pages, max_batch, max_total_q,
+                           max_pages_per_req, device)
+        self.ctx = ctypes.c_void_p()
+        rc = self.lib.sangam_create(ctypes.byref(self.cfg), ctypes.byref(self.ctx))
+        if rc != 0:
+            raise SangamError(f"sangam_create failed: {rc}")
+
+    def _check(self, rc):
+        if rc != 0:
+            raise SangamError(f"sangam error {rc}: {self.lib.sangam_last_error(self.ctx).decode()}")
+
+    def close(self):
+        if self.ctx:
+            self.lib.sangam_destroy(self.ctx)
+            self.ctx = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def kv_write(self, k, v, slot_mapping, k_pages, v_pages, stream=None):
+        self._check(self.lib.sangam_kv_write(self.ctx, _ptr(k), _ptr(v), _ptr(slot_mapping), int(slot_mapping.numel()),
+                                             _ptr(k_pages), _ptr(v_pages), _stream(stream)))
+
+    def block_attn(self, q, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, scale, out, stream=None, simt=False):
+        fn = self.lib.sangam_block_attn_simt if simt else self.lib.sangam_block_attn
+        self._check(fn(self.ctx, _ptr(q), _ptr(k_pages), _ptr(v_pages), _ptr(block_table), _ptr(cu_q_lens),
+                       _ptr(ctx_lens), int(ctx_lens.numel()), int(q.shape[0]), float(scale), _ptr(out), _stream(stream)))
+
+    def iteration_host(self, q, k, v, slot_mapping, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, scale, out,
+                       stream=None):
+        """q, k, v, slot_mapping, block_table, cu_q_lens, ctx_lens, out: HOST (pinned) tensors; pools on device."""
+        self._check(self.lib.sangam_iteration_host(
+            self.ctx, _ptr(q), _ptr(k), _ptr(v), _ptr(slot_mapping), int(slot_mapping.numel()), _ptr(k_pages),
+            _ptr(v_pages), _ptr(block_table), _ptr(cu_q_lens), _ptr(ctx_lens), int(ctx_lens.numel()), int(q.shape[0]),
+            float(scale), _ptr(out), _stream(stream)))
+
+    def device_status(self) -> int:
+        f = ctypes.c_uint32(0)
+        self._check(self.lib.sangam_device_status(self.ctx, ctypes.byref(f)))
+        return int(f.value)
+
+    def clear_device_status(self):
+        self._check(self.lib.sangam_clear_device_status(self.ctx))
+
+    def launch_count(self) -> int:
+        return int(self.lib.sangam_launch_count(self.ctx))
