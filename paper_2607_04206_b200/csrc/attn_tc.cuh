@@ -277,4 +277,426 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, SlotMeta* met
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// warp 1: MMA issuer (a5, a7).  TMEM columns: S0 = [0,128), S1 = [128,256), O = [256,256+D).
+// P_b (bf16, two per column) overwrites the first 64 columns of S_b.
+// Issue order per item: QK0, [QK1], PV0, [QK2], PV1, ...  -- the next tile's logits are computed
+// while the softmax warpgroup works on the current one.
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, uint32_t tmem, const Item* items,
+                                         volatile uint32_t* abort_flag, int lane) {
+    using L = Smem<D>;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    const uint32_t q_addr = sbase + L::OFF_Q;
+    uint32_t kvi = 0, icount = 0, tcount = 0;
+    while (true) {
+        if (*abort_flag) break;
+        const uint32_t islot = icount & 1u;
+        ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
+        const Item it = items[islot];
+        if (!it.valid) break;
+        const int n = it.kv1 - it.kv0;
+        ptx::mbar_wait(bar(L::B_Q_FULL), icount & 1u, abort_flag);
+        ptx::tc_fence_after();
+        auto issue_qk = [&](int j, uint32_t sb) {
+            const uint32_t stage = kvi % NSTAGE;
+            ptx::mbar_wait(bar(L::B_KV_FULL + stage), (kvi / NSTAGE) & 1u, abort_flag);
+            ptx::tc_fence_after();
+            int nv = it.c - (it.kv0 + j) * BN;
+            nv = nv > BN ? BN : nv;
+            const uint32_t ncols = (uint32_t)((nv + 15) & ~15);
+            if (lane == 0) {
+                const uint32_t k_addr = sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES);
+                const uint32_t idesc = ptx::idesc_bf16(BM, ncols, 0, 0);
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    const uint32_t off = (uint32_t)((ks >> 2) * SLAB + (ks & 3) * 32);
+                    ptx::mma_ss(tmem + sb * 128u, ptx::smem_desc_sw128(q_addr + off, 16, 1024),
+                                ptx::smem_desc_sw128(k_addr + off, 16, 1024), idesc, ks > 0);
+                }
+                ptx::mma_commit(bar(L::B_KV_EMPTY + stage));
+                ptx::mma_commit(bar(L::B_S_FULL + sb));
+            }
+            __syncwarp();
+            ++kvi;
+        };
+        if (n > 0) {
+            issue_qk(0, tcount & 1u);
+            for (int j = 0; j < n; ++j) {
+                if (*abort_flag) break;
+                const uint32_t sb = tcount & 1u;
+                if (j + 1 < n) issue_qk(j + 1, sb ^ 1u);
+                const uint32_t stage = kvi % NSTAGE;
+                ptx::mbar_wait(bar(L::B_KV_FULL + stage), (kvi / NSTAGE) & 1u, abort_flag);
+                int nv = it.c - (it.kv0 + j) * BN;
+                nv = nv > BN ? BN : nv;
+                const int ncols = (nv + 15) & ~15;
+                const uint32_t v_addr = sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES);
+                if (nv < ncols) {
+                    // stale rows of the last page: zero them so that P = 0 meets V = 0, never NaN (reading S12)
+                    const int nrows = ncols - nv;
+                    for (int e = lane; e < nrows * 8 * (D / 64); e += 32) {
+                        const int chunk = e & 7, rr = (e >> 3) % nrows, slab = (e >> 3) / nrows;
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(
+                                         v_addr + (uint32_t)(slab * SLAB + (nv + rr) * 128 + chunk * 16)),
+                                     "r"(0)
+                                     : "memory");
+                    }
+                    ptx::fence_proxy_async_smem();
+                    __syncwarp();
+                }
+                ptx::mbar_wait(bar(L::B_P_FULL + sb), (tcount >> 1) & 1u, abort_flag);
+                ptx::tc_fence_after();
+                if (lane == 0) {
+                    const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
+                    const int nk = ncols / 16;
+                    for (int ks = 0; ks < nk; ++ks)
+                        ptx::mma_ts(tmem + 256u, tmem + sb * 128u + (uint32_t)(ks * 8),
+                                    ptx::smem_desc_sw128(v_addr + (uint32_t)(ks * 2048), SLAB, 1024), idesc,
+                                    (j > 0 || ks > 0) ? 1u : 0u);
+                    ptx::mma_commit(bar(L::B_KV_EMPTY + stage));
+                    ptx::mma_commit(bar(L::B_PV_DONE));
+                }
+                __syncwarp();
+                ++kvi;
+                ++tcount;
+            }
+        }
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
+        ++icount;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// warps 4-7: softmax warpgroup (a6) + epilogue (a8).  Thread `row` owns TMEM lane `row`.
+// ------------------------------------------------------------------------------------------------
+template <bool MASK>
+__device__ __forceinline__ void softmax_row(uint32_t s_taddr, int nv, float scale_log2, float& m, float& l,
+                                            float& alpha, uint32_t (&pk)[64]) {
+    uint32_t r[4][32];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) ptx::tmem_ld32(s_taddr + (uint32_t)(c * 32), r[c]);
+    ptx::tmem_wait_ld();
+    float mx = -INFINITY;
+    if (scale_log2 >= 0.f) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+                if (!MASK || c * 32 + i < nv) mx = fmaxf(mx, __uint_as_float(r[c][i]));
+    } else {
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+                if (!MASK || c * 32 + i < nv) mx = fmaxf(mx, -__uint_as_float(r[c][i]));
+        mx = -mx;
+    }
+    const float m_new = fmaxf(m, mx * scale_log2);
+    alpha = ptx::ex2(m - m_new);
+    const float neg = -m_new;
+    float sum0 = 0.f, sum1 = 0.f;
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            float p0 = ptx::ex2(fmaf(__uint_as_float(r[c][2 * i]), scale_log2, neg));
+            float p1 = ptx::ex2(fmaf(__uint_as_float(r[c][2 * i + 1]), scale_log2, neg));
+            if (MASK) {
+                if (c * 32 + 2 * i >= nv) p0 = 0.f;
+                if (c * 32 + 2 * i + 1 >= nv) p1 = 0.f;
+            }
+            sum0 += p0;
+            sum1 += p1;
+            pk[c * 16 + i] = ptx::pack_bf16(p0, p1);
+        }
+    l = l * alpha + (sum0 + sum1);
+    m = m_new;
+}
+
+template <int D>
+__device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, uint32_t sbase, uint32_t tmem,
+                                           const Item* items, volatile uint32_t* abort_flag, int wg_warp, int lane) {
+    using L = Smem<D>;
+    const unsigned FULL = 0xffffffffu;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    const int row = wg_warp * 32 + lane;
+    const int wtid = wg_warp * 32 + lane;   // 0..127
+    const uint32_t lane_base = (uint32_t)(wg_warp * 32) << 16;
+    const uint32_t o_taddr = tmem + lane_base + 256u;
+    uint32_t icount = 0, tcount = 0;
+    while (true) {
+        if (*abort_flag) break;
+        const uint32_t islot = icount & 1u;
+        ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
+        const Item it = items[islot];
+        if (!it.valid) break;
+        // ---- Q tile -> smem, 128B swizzle, zero rows past rows_valid
+        {
+            constexpr int CPR = D / 8;                 // 16-byte chunks per row
+            constexpr int RPP = 128 / CPR;             // rows per pass
+            const int chunk = wtid % CPR, rsub = wtid / CPR;
+#pragma unroll 4
+            for (int i = 0; i < BM / RPP; ++i) {
+                const int rr = i * RPP + rsub;
+                uint4 v = make_uint4(0, 0, 0, 0);
+                if (rr < it.rows_valid) {
+                    const int rg = it.row0 + rr;
+                    const int tl = rg / p.G, hh = rg - tl * p.G;
+                    v = __ldg(reinterpret_cast<const uint4*>(p.q + ((int64_t)(it.q_start + tl) * p.Hq + it.g * p.G + hh) * D) + chunk);
+                }
+                const int slab = chunk >> 3, c16 = chunk & 7;
+                *reinterpret_cast<uint4*>(smem + L::OFF_Q + slab * SLAB + rr * 128 + ((c16 ^ (rr & 7)) << 4)) = v;
+            }
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_Q_FULL));
+        }
+        const bool warp_active = wg_warp * 32 < it.rows_valid;
+        const int n = it.kv1 - it.kv0;
+        float m = -INFINITY, l = 0.f;
+        for (int j = 0; j < n; ++j) {
+            if (*abort_flag) break;
+            const uint32_t sb = tcount & 1u;
+            ptx::mbar_wait(bar(L::B_S_FULL + sb), (tcount >> 1) & 1u, abort_flag);
+            ptx::tc_fence_after();
+            int nv = it.c - (it.kv0 + j) * BN;
+            nv = nv > BN ? BN : nv;
+            float alpha = 1.f;
+            const uint32_t s_taddr = tmem + lane_base + sb * 128u;
+            if (warp_active) {
+                uint32_t pk[64];
+                if (nv == BN) softmax_row<false>(s_taddr, nv, p.scale_log2, m, l, alpha, pk);
+                else softmax_row<true>(s_taddr, nv, p.scale_log2, m, l, alpha, pk);
+                ptx::tmem_st32(s_taddr, *reinterpret_cast<const uint32_t(*)[32]>(&pk[0]));
+                ptx::tmem_st32(s_taddr + 32u, *reinterpret_cast<const uint32_t(*)[32]>(&pk[32]));
+            }
+            if (j > 0) {
+                ptx::mbar_wait(bar(L::B_PV_DONE), (tcount - 1u) & 1u, abort_flag);
+                ptx::tc_fence_after();
+                if (warp_active && __any_sync(FULL, alpha != 1.f)) {
+#pragma unroll
+                    for (int c = 0; c < D / 32; ++c) {
+                        uint32_t o[32];
+                        ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
+                        ptx::tmem_wait_ld();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                        ptx::tmem_st32(o_taddr + (uint32_t)(c * 32), o);
+                    }
+                }
+            }
+            ptx::tmem_wait_st();
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL + sb));
+            ++tcount;
+        }
+        if (n > 0) {
+            ptx::mbar_wait(bar(L::B_PV_DONE), (tcount - 1u) & 1u, abort_flag);
+            ptx::tc_fence_after();
+        }
+        // ---- epilogue (TMEM loads are warp-collective: predicate only the global stores)
+        if (warp_active) {
+            const bool row_ok = row < it.rows_valid;
+            if (it.part_slot < 0) {
+                const float inv = (n > 0 && l > 0.f) ? 1.f / l : 0.f;
+                const int rg = it.row0 + row;
+                const int tl = rg / p.G, hh = rg - tl * p.G;
+                uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)(it.q_start + tl) * p.Hq + it.g * p.G + hh) * D);
+#pragma unroll
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t o[32];
+                    if (n > 0) {
+                        ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
+                        ptx::tmem_wait_ld();
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) o[i] = 0u;
+                    }
+                    if (row_ok) {
+#pragma unroll
+                        for (int v = 0; v < 4; ++v) {
+                            uint4 w;
+                            w.x = ptx::pack_bf16(__uint_as_float(o[v * 8 + 0]) * inv, __uint_as_float(o[v * 8 + 1]) * inv);
+                            w.y = ptx::pack_bf16(__uint_as_float(o[v * 8 + 2]) * inv, __uint_as_float(o[v * 8 + 3]) * inv);
+                            w.z = ptx::pack_bf16(__uint_as_float(o[v * 8 + 4]) * inv, __uint_as_float(o[v * 8 + 5]) * inv);
+                            w.w = ptx::pack_bf16(__uint_as_float(o[v * 8 + 6]) * inv, __uint_as_float(o[v * 8 + 7]) * inv);
+                            dst[c * 4 + v] = w;
+                        }
+                    }
+                }
+            } else {
+                float* po = p.part_o + ((int64_t)it.part_slot * BM + row) * D;
+#pragma unroll
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t o[32];
+                    ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
+                    ptx::tmem_wait_ld();
+                    if (row_ok) {
+#pragma unroll
+                        for (int v = 0; v < 8; ++v)
+                            reinterpret_cast<uint4*>(po)[c * 8 + v] = make_uint4(o[v * 4], o[v * 4 + 1], o[v * 4 + 2], o[v * 4 + 3]);
+                    }
+                }
+                if (row_ok) reinterpret_cast<float2*>(p.part_ml)[(int64_t)it.part_slot * BM + row] = make_float2(m, l);
+            }
+        }
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
+        ++icount;
+    }
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// kernel entry
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(NTHREADS, 1)
+attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV, const AttnParams p) {
+    using L = Smem<D>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    const uint32_t sbase = ptx::smem_u32(smem);
+    Item* items = reinterpret_cast<Item*>(smem + L::OFF_ITEMS);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::OFF_MISC);
+    volatile uint32_t* abort_flag = reinterpret_cast<volatile uint32_t*>(smem + L::OFF_MISC + 4);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+        for (int s = 0; s < NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 1); }
+        for (int s = 0; s < 2; ++s) {
+            ptx::mbar_init(bar(L::B_ITEM_FULL + s), 1);
+            ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 5);   // MMA lane + 4 softmax warps
+            ptx::mbar_init(bar(L::B_S_FULL + s), 1);
+            ptx::mbar_init(bar(L::B_P_FULL + s), 4);
+        }
+        ptx::mbar_init(bar(L::B_Q_FULL), 4);
+        ptx::mbar_init(bar(L::B_PV_DONE), 1);
+        *abort_flag = 0u;
+        ptx::fence_mbar_init();
+        ptx::prefetch_tensormap(&mapK);
+        ptx::prefetch_tensormap(&mapV);
+    }
+    if (warp == 2) {
+        ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == 0) {
+        producer_warp<D>(p, reinterpret_cast<SlotMeta*>(p.slot_meta), &mapK, &mapV, sbase, items, abort_flag, lane);
+    } else if (warp == 1) {
+        mma_warp<D>(p, sbase, tmem, items, abort_flag, lane);
+    } else if (warp >= 4) {
+        softmax_wg<D>(p, smem, sbase, tmem, items, abort_flag, warp - 4, lane);
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (tid == 0 && *abort_flag) raise_flag(p.flags, DEV_TIMEOUT);
+    if (warp == 2) ptx::tmem_dealloc(tmem, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+// combine (a9): merge the split-KV partials of one unit.  Block b owns the unit whose head piece
+// is in slot 2b+1; continuation pieces are slots 2b' of CTAs b' in (b, b_last].  Fixed order, no
+// atomics: bitwise reproducible.  m is in log2 units:
+//   m* = max m_i;  l* = sum l_i 2^(m_i-m*);  O* = sum O_i 2^(m_i-m*);  out = bf16(O*/l*)
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(256)
+combine_kernel(const AttnParams p) {
+    const SlotMeta* meta = reinterpret_cast<const SlotMeta*>(p.slot_meta);
+    const int b = blockIdx.x;
+    const SlotMeta h = meta[2 * b + 1];
+    if (!h.valid) return;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int EPL = D / 32;
+    const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
+    for (int row = warp; row < h.rows_valid; row += 8) {
+        float ms = ml[(int64_t)(2 * b + 1) * BM + row].x;
+        for (int bb = b + 1; bb <= h.b_last; ++bb)
+            if (meta[2 * bb].valid) ms = fmaxf(ms, ml[(int64_t)(2 * bb) * BM + row].x);
+        float acc[EPL];
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
+        float ls = 0.f;
+        for (int bb = b; bb <= h.b_last; ++bb) {
+            const int slot = bb == b ? 2 * b + 1 : 2 * bb;
+            if (bb != b && !meta[slot].valid) continue;
+            const float2 x = ml[(int64_t)slot * BM + row];
+            const float w = ptx::ex2(x.x - ms);
+            ls += x.y * w;
+            const float* po = p.part_o + ((int64_t)slot * BM + row) * D + lane * EPL;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e) acc[e] += po[e] * w;
+        }
+        const float inv = ls > 0.f ? 1.f / ls : 0.f;
+        const int rg = h.row0 + row;
+        const int tl = rg / p.G, hh = rg - tl * p.G;
+        __nv_bfloat16* dst = p.out + ((int64_t)(h.q_start + tl) * p.Hq + h.g * p.G + hh) * D + lane * EPL;
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) dst[e] = __float2bfloat16(acc[e] * inv);
+    }
+}
+
 }  // namespace tc
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+static inline cudaError_t tc_configure(int head_dim) {
+    if (head_dim == 128)
+        return cudaFuncSetAttribute(tc::attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Smem<128>::ALLOC);
+    return cudaFuncSetAttribute(tc::attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Smem<64>::ALLOC);
+}
+
+typedef CUresult (*sangam_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// Pool viewed as a 2-D tensor [P*Hkv*16 rows][D] bf16; one box = 16 rows (a page of one head) x 64 columns,
+// 128-byte swizzled: exactly one UMMA swizzle slab of a page.
+static inline int tc_encode_maps(TcMaps* maps, const void* k_pages, const void* v_pages, int num_pages, int Hkv, int D) {
+    static sangam_encode_fn enc = nullptr;
+    if (!enc) {
+        cudaDriverEntryPointQueryResult q;
+        void* fn = nullptr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return -1;
+        enc = reinterpret_cast<sangam_encode_fn>(fn);
+    }
+    const cuuint64_t gdim[2] = {(cuuint64_t)D, (cuuint64_t)num_pages * Hkv * SANGAM_PAGE};
+    const cuuint64_t gstr[1] = {(cuuint64_t)D * 2};
+    const cuuint32_t box[2] = {64, SANGAM_PAGE}, estr[2] = {1, 1};
+    const void* ptrs[2] = {k_pages, v_pages};
+    CUtensorMap* out[2] = {&maps->k, &maps->v};
+    for (int i = 0; i < 2; ++i) {
+        CUresult r = enc(out[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptrs[i]), gdim, gstr, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return -1;
+    }
+    return 0;
+}
+
+static inline cudaError_t tc_launch(const AttnParams& p, const TcMaps& maps, int head_dim, int sm_count,
+                                    cudaStream_t stream, int* launched) {
+    *launched = 0;
+    if (head_dim == 128) {
+        tc::attn_kernel<128><<<sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream>>>(maps.k, maps.v, p);
+        tc::combine_kernel<128><<<sm_count, 256, 0, stream>>>(p);
+    } else {
+        tc::attn_kernel<64><<<sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream>>>(maps.k, maps.v, p);
+        tc::combine_kernel<64><<<sm_count, 256, 0, stream>>>(p);
+    }
+    *launched = 2;
+    return cudaGetLastError();
+}
