@@ -1,0 +1,456 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Sangam hot path (kv_write -> block_attn) on B200.
+
+One "step" = one pass of the whole hot path over one synthetic batch: sangam_kv_write of the
+iteration's fresh K/V rows followed by sangam_block_attn (device-side plan, tcgen05 attention,
+split-KV combine), captured once as a CUDA graph and replayed.
+Headline workload (N = 1): BASELINE.json configs[1], the LLaDA-8B-like block decode.  Steps
+rotate over several independent per-layer pool sets so that consecutive replays never find
+their K/V in L2 (cold-L2 rule).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5] [--all-configs]
+  python bench.py --impl reference ...      # times the fp64 CPU oracle on a bounded sample
+
+Multi-GPU: the path does not shard ("replicas only"): under torchrun every rank runs
+the same workload on its own GPU, time = max over ranks, value = sum of work / that time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import sangam_inputs as si  # noqa: E402
+
+METRIC = "block_attn_tflops"
+UNIT = "TFLOP/s"
+WORKLOAD_NAMES = {1: "config1_tiny", 2: "config2_llada_block_decode", 3: "config3_dream_gqa_block_decode",
+                  4: "config4_kv_refresh_prefill", 5: "config5_hybrid_mixed"}
+NSETS = {1: 8, 2: 10, 3: 6, 4: 1, 5: 1}        # independent pool sets rotated per step (>= 8x L2 of distinct data)
+BOUND = {1: "hbm", 2: "hbm", 3: "hbm", 4: "tensor", 5: "tensor"}
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]),
+                "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+def load_traffic():
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f)
+    return {}
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks: sampled DURING the timed region
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20,
+           "sw_power_cap": 0x4, "hw_power_brake": 0x80}
+
+    def __init__(self, index=0, period=0.01):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.period, self.stop_evt, self.thread, self.h = period, threading.Event(), None, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        while not self.stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for name, bit in self.BAD.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self.stop_evt.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self.thread = threading.Thread(target=self._loop, daemon=True)
+            self.thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop_evt.set()
+        if self.thread:
+            self.thread.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": int(statistics.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------
+# device state
+# ------------------------------------------------------------------------------------------------
+def _bf16(bits, device):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).to(device).view(torch.bfloat16)
+
+
+def _i32(a, device):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.int32)).to(device)
+
+
+class Workload:
+    """A Batch resident in HBM: `nsets` independent (pools, q, k_new, v_new, out) sets + shared metadata."""
+
+    def __init__(self, b: si.Batch, nsets: int, device="cuda"):
+        import torch
+        import paper_2607_04206_b200 as sg
+        self.b, self.nsets, self.device = b, nsets, device
+        self.eng = sg.Sangam(num_q_heads=b.num_q_heads, num_kv_heads=b.num_kv_heads, head_dim=b.head_dim,
+                             num_pages=b.num_pages, max_batch=b.batch, max_total_q=max(b.total_q, len(b.slot_new), 1),
+                             max_pages_per_req=b.max_pages_per_req)
+        self.block_table, self.cu_q_lens, self.ctx_lens = _i32(b.block_table, device), _i32(b.cu_q_lens, device), _i32(b.ctx_lens, device)
+        self.slot_new = _i32(b.slot_new, device)
+        k_cache, v_cache, slot_cache = _bf16(b.k_cache, device), _bf16(b.v_cache, device), _i32(b.slot_cache, device)
+        q0, kn0, vn0 = _bf16(b.q, device), _bf16(b.k_new, device), _bf16(b.v_new, device)
+        self.sets = []
+        shape = (b.num_pages, b.num_kv_heads, si.PAGE, b.head_dim)
+        for _ in range(nsets):
+            kp = torch.zeros(shape, dtype=torch.bfloat16, device=device)
+            vp = torch.zeros(shape, dtype=torch.bfloat16, device=device)
+            self.eng.kv_write(k_cache, v_cache, slot_cache, kp, vp)          # cache content (setup, untimed)
+            self.sets.append({"kp": kp, "vp": vp, "q": q0.clone(), "kn": kn0.clone(), "vn": vn0.clone(),
+                              "out": torch.zeros_like(q0)})
+        torch.cuda.synchronize()
+        del k_cache, v_cache, slot_cache
+        self.stream = torch.cuda.Stream()
+        self.iter_graphs, self.attn_graphs, self.write_graphs = [], [], []
+
+    def run_iteration(self, s, stream):
+        self.eng.kv_write(s["kn"], s["vn"], self.slot_new, s["kp"], s["vp"], stream=stream)
+        self.run_attn(s, stream)
+
+    def run_attn(self, s, stream):
+        self.eng.block_attn(s["q"], s["kp"], s["vp"], self.block_table, self.cu_q_lens, self.ctx_lens,
+                            float(self.b.scale), s["out"], stream=stream)
+
+    def capture(self):
+        import torch
+        with torch.cuda.stream(self.stream):
+            for s in self.sets:                       # warm-up outside capture (first-launch work)
+                self.run_iteration(s, self.stream)
+            self.stream.synchronize()
+            for s in self.sets:
+                for lst, fn in ((self.iter_graphs, self.run_iteration), (self.attn_graphs, self.run_attn),
+                                (self.write_graphs, lambda ss, st: self.eng.kv_write(ss["kn"], ss["vn"], self.slot_new, ss["kp"], ss["vp"], stream=st))):
+                    g = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(g, stream=self.stream):
+                        fn(s, self.stream)
+                    lst.append(g)
+        torch.cuda.synchronize()
+
+    def time_graphs(self, graphs, steps, warmup):
+        """K replays between two CUDA events on the launching stream; returns total ms."""
+        import torch
+        n = len(graphs)
+        with torch.cuda.stream(self.stream):
+            for i in range(warmup):
+                graphs[i % n].replay()
+            self.stream.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(self.stream)
+            for i in range(steps):
+                graphs[i % n].replay()
+            e1.record(self.stream)
+            e1.synchronize()
+        return e0.elapsed_time(e1)
+
+
+def roofline_time_us(b: si.Batch, peaks, which="attn"):
+    f = b.flops() / (peaks["bf16_tflops"] * 1e12) * 1e6
+    by = (b.attn_bytes() if which == "attn" else b.attn_bytes() + b.write_bytes()) / (peaks["hbm_gbs"] * 1e9) * 1e6
+    return max(f, by), f, by
+
+
+def measure_config(cfg: int, steps: int, warmup: int, peaks, reps: int = 3):
+    """All figures of one config: iteration / attention / kv_write time, TFLOP/s, GB/s, roofline fraction."""
+    b = si.CONFIGS[cfg]()
+    w = Workload(b, NSETS[cfg])
+    w.capture()
+    res = {"workload": WORKLOAD_NAMES[cfg], "pool_sets": w.nsets}
+    for key, graphs in (("iteration", w.iter_graphs), ("attn", w.attn_graphs), ("kv_write", w.write_graphs)):
+        per = [w.time_graphs(graphs, steps, warmup) / steps * 1e3 for _ in range(reps)]   # us per step
+        res[key + "_us"] = round(statistics.median(per), 3)
+        res[key + "_us_min"] = round(min(per), 3)
+    t_roof, t_f, t_b = roofline_time_us(b, peaks)
+    a = res["attn_us"]
+    res.update({"flops": b.flops(), "attn_bytes": b.attn_bytes(), "write_bytes": b.write_bytes(),
+                "attn_tflops": round(b.flops() / a / 1e6, 2), "attn_gbs": round(b.attn_bytes() / a / 1e3, 1),
+                "kv_write_gbs": round(b.write_bytes() / max(res["kv_write_us"], 1e-9) / 1e3, 1),
+                "bound": BOUND[cfg], "t_roof_us": round(t_roof, 2), "roofline_frac": round(t_roof / a, 4)})
+    return res, w
+
+
+# ------------------------------------------------------------------------------------------------
+# end to end through the C ABI with HOST buffers (sangam_iteration_host)
+# ------------------------------------------------------------------------------------------------
+def measure_e2e(w: Workload, steps: int, warmup: int):
+    import torch
+    b = w.b
+
+    def pin(a, view_bf16=False):
+        t = torch.from_numpy(np.ascontiguousarray(a).view(np.int16) if view_bf16 else np.ascontiguousarray(a)).pin_memory()
+        return t.view(torch.bfloat16) if view_bf16 else t
+
+    q, kn, vn = pin(b.q, True), pin(b.k_new, True), pin(b.v_new, True)
+    slot, bt, cu, cl = pin(b.slot_new.astype(np.int32)), pin(b.block_table.astype(np.int32)), pin(b.cu_q_lens.astype(np.int32)), pin(b.ctx_lens.astype(np.int32))
+    out = torch.empty_like(q).pin_memory()
+    h2d = sum(int(t.numel()) * t.element_size() for t in (q, kn, vn, slot, bt, cu, cl))
+    d2h = int(out.numel()) * out.element_size()
+    n = len(w.sets)
+
+    def step(i):
+        s = w.sets[i % n]
+        w.eng.iteration_host(q, kn, vn, slot, s["kp"], s["vp"], bt, cu, cl, float(b.scale), out, stream=w.stream)
+
+    for i in range(warmup):
+        step(i)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(steps):
+        step(i)                         # each call ends with a stream synchronize (D2H of `out` complete)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    return dt / steps, h2d, d2h
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/)
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(b: si.Batch, rows_per_request: int):
+    """Pools as the oracle builds them + the sampled global q rows."""
+    import oracle
+    kp, vp = si.empty_pools(b, poison=False)
+    oracle.kv_write(b.k_cache, b.v_cache, b.slot_cache, kp, vp)
+    rows = si.sample_rows(b, per_request=rows_per_request)
+    return oracle, kp, vp, rows
+
+
+def oracle_step(oracle, b, kp, vp, rows):
+    oracle.kv_write(b.k_new, b.v_new, b.slot_new, kp, vp)
+    oracle.block_attn(b.q, kp, vp, b.block_table, b.cu_q_lens, b.ctx_lens, b.scale, rows=rows)
+
+
+def sample_flops(b: si.Batch, rows) -> float:
+    r_of = np.searchsorted(b.cu_q_lens, rows, side="right") - 1
+    return 4.0 * b.num_q_heads * b.head_dim * float(np.sum(b.ctx_lens[r_of].astype(np.int64)))
+
+
+def cpu_baseline(b: si.Batch, target_s: float = 15.0):
+    oracle, kp, vp, rows1 = oracle_sample(b, 1)
+    t0 = time.perf_counter()
+    oracle_step(oracle, b, kp, vp, rows1)
+    t1 = time.perf_counter() - t0
+    per = max(1, int(target_s / max(t1, 1e-3)))
+    qmax = int(b.q_lens.max())
+    per = min(per, qmax)
+    rows = si.sample_rows(b, per_request=per)
+    t0 = time.perf_counter()
+    oracle_step(oracle, b, kp, vp, rows)
+    dt = time.perf_counter() - t0
+    f = sample_flops(b, rows)
+    return {"value": round(f / dt / 1e12, 6), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{len(rows)} of {b.total_q} query rows (<= {per} per request, all heads, full contexts) + the kv_write, "
+                      f"{dt:.2f} s, fp64 C -O2 -fopenmp",
+            "seconds": round(dt, 3), "sample_flops": f}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = args.workload
+    b = si.CONFIGS[cfg]()
+    oracle, kp, vp, rows = oracle_sample(b, 2)
+    for _ in range(min(args.warmup, 3)):
+        oracle_step(oracle, b, kp, vp, rows)
+    steps = min(args.steps, 200)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(oracle, b, kp, vp, rows)
+    dt = (time.perf_counter() - t0) / steps
+    f = sample_flops(b, rows)
+    val = round(f / dt / 1e12, 6)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": min(args.warmup, 3), "ms_per_step": round(dt * 1e3, 4), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[cfg], "sample": f"{len(rows)} of {b.total_q} query rows per step"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "kind": "oracle", "cores": oracle.num_threads(),
+                             "sample": f"{len(rows)} of {b.total_q} query rows (2 per request, all heads) + kv_write per step"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# multi-process plumbing: replicas only, max time over ranks
+# ------------------------------------------------------------------------------------------------
+def dist_setup():
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world <= 1:
+        return 0, 1, None
+    import torch
+    import torch.distributed as dist
+    rank, local = int(os.environ["RANK"]), int(os.environ.get("LOCAL_RANK", "0"))
+    backend = "nccl" if torch.cuda.is_available() else "gloo"
+    if backend == "nccl":
+        torch.cuda.set_device(local)
+    dist.init_process_group(backend=backend)
+    return rank, world, dist
+
+
+def max_over_ranks(value: float, dist, device=None) -> float:
+    if dist is None:
+        return value
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device or ("cuda" if dist.get_backend() == "nccl" else "cpu"))
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def barrier(dist):
+    if dist is not None:
+        dist.barrier()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20000)
+    ap.add_argument("--warmup", type=int, default=200)
+    ap.add_argument("--workload", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="sangam", choices=["sangam", "reference"])
+    ap.add_argument("--all-configs", dest="all_configs", action="store_true", default=None)
+    ap.add_argument("--no-all-configs", dest="all_configs", action="store_false")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    rank, world, dist = dist_setup()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the sangam kernels have no CPU fallback)")
+    peaks = load_peaks()
+    cfg = args.workload
+    steps, warmup = max(1, args.steps), max(3, args.warmup)
+    b = si.CONFIGS[cfg]()
+    w = Workload(b, NSETS[cfg])
+    w.capture()
+    launches0 = w.eng.launch_count()
+
+    # ---- timed region: K steps of the whole hot path, barrier + synchronize on both sides
+    barrier(dist)
+    torch.cuda.synchronize()
+    with ClockSampler(index=torch.cuda.current_device()) as cs:
+        ms_total = w.time_graphs(w.iter_graphs, steps, warmup)
+    torch.cuda.synchronize()
+    barrier(dist)
+    ms_total = max_over_ranks(ms_total, dist)
+    ms_step = ms_total / steps
+    value = world * b.flops() / (ms_step * 1e-3) / 1e12
+    kernels_per_step = 3                      # kv_write, attention, combine (captured; replayed K times)
+    gpu_launches = steps * kernels_per_step
+
+    # ---- dominant kernel (attention + its combine), timed alone, L2-cold
+    attn_ms = w.time_graphs(w.attn_graphs, steps, warmup) / steps
+    attn_ms = max_over_ranks(attn_ms, dist)
+    write_ms = w.time_graphs(w.write_graphs, steps, warmup) / steps
+    traffic = load_traffic().get(WORLD_KEY(cfg))
+    if BOUND[cfg] == "hbm":
+        ach = b.attn_bytes() / (attn_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": round(ach, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": round(ach / peaks["hbm_gbs"], 4)}
+    else:
+        ach = b.flops() / (attn_ms * 1e-3) / 1e12
+        roof = {"bound": "tensor", "achieved": round(ach, 1), "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                "frac": round(ach / peaks["bf16_tflops"], 4)}
+    roof.update({"traffic": traffic, "kernel": "tc::attn_kernel (+ combine_kernel), timed alone over the same rotation",
+                 "kernel_us": round(attn_ms * 1e3, 3), "peak_source": peaks["source"] + " (burst)",
+                 "algorithmic_bytes": b.attn_bytes(), "algorithmic_flops": b.flops()})
+
+    # ---- end to end from host buffers
+    e2e_steps = max(10, min(steps, 300))
+    e2e_s, h2d, d2h = measure_e2e(w, e2e_steps, 5)
+    e2e_s = max_over_ranks(e2e_s, dist)
+    e2e = {"value": round(world * b.flops() / e2e_s / 1e12, 4), "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "ms_per_step": round(e2e_s * 1e3, 4), "steps": e2e_steps,
+           "api": "sangam_iteration_host (pinned host buffers, H2D + kv_write + block_attn + D2H per step)"}
+
+    line = {"metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": round(ms_step, 6), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[cfg], "batch": b.batch, "total_q": b.total_q,
+                       "sum_ctx": int(b.ctx_lens.sum()), "heads": f"{b.num_q_heads}/{b.num_kv_heads}",
+                       "head_dim": b.head_dim, "page": si.PAGE, "parallelism": f"replicas x{world}",
+                       "l2": f"cold: steps rotate over {w.nsets} independent pool sets "
+                             f"({w.nsets * b.attn_bytes() / 1e6:.0f} MB distinct per rotation)",
+                       "step": "CUDA-graph replay of kv_write + block_attn (plan + tcgen05 attention + combine)"},
+            "us_per_iteration": round(ms_step * 1e3, 3), "attn_us": round(attn_ms * 1e3, 3),
+            "kv_write_us": round(write_ms * 1e3, 3),
+            "clocks": cs.summary(), "e2e": e2e, "gpu_launches": gpu_launches,
+            "launch_count_check": w.eng.launch_count() - launches0, "roofline": roof}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(b)
+    run_all = args.all_configs if args.all_configs is not None else (world == 1)
+    if run_all and rank == 0:
+        del w
+        torch.cuda.empty_cache()
+        allc = []
+        for c in (1, 2, 3, 4, 5):
+            st = {1: 2000, 2: 2000, 3: 1000, 4: 20, 5: 40}[c]
+            r, ww = measure_config(c, st, max(3, st // 10), peaks)
+            allc.append(r)
+            del ww
+            torch.cuda.empty_cache()
+        line["all_configs"] = allc
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def WORLD_KEY(cfg):
+    return WORKLOAD_NAMES[cfg]
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,51 @@
+"""-m gpu parity at BASELINE.json's full sizes, in the launch configuration bench.py times (CUDA-graph replay
+of kv_write + block_attn over bench.Workload): KV pools bit-exact against the oracle, attention checked on a
+stratified row sample the oracle computes one by one (tile-edge rows + seeded random rows, all heads), and on
+every element against the CUDA-core cross-check kernel."""
+import numpy as np
+import pytest
+
+import sangam_inputs as si
+from gpu_harness import MAX_ABS, MEAN_ABS, bits_of, compare
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("cfg,per_req", [(2, 32), (3, 32), (4, 24), (5, 16)])
+def test_full_size_config(oracle, cfg, per_req):
+    import torch
+    import bench
+    b = si.CONFIGS[cfg]()
+    w = bench.Workload(b, 1)
+    w.capture()
+    s = w.sets[0]
+    s["out"].fill_(float("nan"))
+    w.iter_graphs[0].replay()
+    torch.cuda.synchronize()
+    # pages: bit-exact, whole pools (bench pools start zero-filled, so the oracle's do too)
+    rows = si.sample_rows(b, per_request=per_req)
+    ref, kp, vp = oracle.iteration(b, rows=rows, poison=False)
+    assert np.array_equal(bits_of(s["kp"]), kp), "K pool differs"
+    assert np.array_equal(bits_of(s["vp"]), vp), "V pool differs"
+    del kp, vp
+    mx, mean = compare(s["out"], ref, rows=rows)
+    print(f"config{cfg} full size, {len(rows)} sampled rows x {b.num_q_heads} heads: max-abs {mx:.3e} mean-abs {mean:.3e}")
+    assert mx <= MAX_ABS and mean <= MEAN_ABS
+    # every element against the CUDA-core kernel (itself oracle-checked on the sample above)
+    out_tc = si.bf16_bits_to_f64(bits_of(s["out"]))
+    simt = torch.full_like(s["out"], float("nan"))
+    w.eng.block_attn(s["q"], s["kp"], s["vp"], w.block_table, w.cu_q_lens, w.ctx_lens, float(b.scale), simt, simt=True)
+    torch.cuda.synchronize()
+    mx_s, mean_s = compare(simt, ref, rows=rows)
+    assert mx_s <= MAX_ABS and mean_s <= MEAN_ABS
+    out_simt = si.bf16_bits_to_f64(bits_of(simt))
+    assert np.all(np.isfinite(out_tc))
+    d = np.abs(out_tc - out_simt)
+    print(f"config{cfg} tcgen05 vs simt over all {d.size} elements: max {d.max():.3e} mean {d.mean():.3e}")
+    assert d.max() <= MAX_ABS and d.mean() <= MEAN_ABS
+    # identical replays are bit-identical
+    first = bits_of(s["out"]).copy()
+    w.iter_graphs[0].replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(first, bits_of(s["out"]))
+    assert w.eng.device_status() == 0
