@@ -3,7 +3,7 @@
 
 One "step" = one pass of the whole hot path over one synthetic batch: sangam_kv_write of the
 iteration's fresh K/V rows followed by sangam_block_attn (device-side plan, tcgen05 attention,
-split-KV combine), captured once as a CUDA graph and replayed.
+fused split-KV merge), captured once as a CUDA graph and replayed.
 Headline workload (N = 1): BASELINE.json configs[1], the LLaDA-8B-like block decode.  Steps
 rotate over several independent per-layer pool sets so that consecutive replays never find
 their K/V in L2 (cold-L2 rule).
@@ -385,10 +385,10 @@ def main():
     ms_total = max_over_ranks(ms_total, dist)
     ms_step = ms_total / steps
     value = world * b.flops() / (ms_step * 1e-3) / 1e12
-    kernels_per_step = 3                      # kv_write, attention, combine (captured; replayed K times)
+    kernels_per_step = 2                      # kv_write, attention (plan + split-KV merge fused in; captured, replayed K times)
     gpu_launches = steps * kernels_per_step
 
-    # ---- dominant kernel (attention + its combine), timed alone, L2-cold
+    # ---- dominant kernel (attention), timed alone, L2-cold
     attn_ms = w.time_graphs(w.attn_graphs, steps, warmup) / steps
     attn_ms = max_over_ranks(attn_ms, dist)
     write_ms = w.time_graphs(w.write_graphs, steps, warmup) / steps
@@ -401,7 +401,7 @@ def main():
         ach = b.flops() / (attn_ms * 1e-3) / 1e12
         roof = {"bound": "tensor", "achieved": round(ach, 1), "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                 "frac": round(ach / peaks["bf16_tflops"], 4)}
-    roof.update({"traffic": traffic, "kernel": "tc::attn_kernel (+ combine_kernel), timed alone over the same rotation",
+    roof.update({"traffic": traffic, "kernel": "tc::attn_kernel (plan and split-KV merge fused in), timed alone over the same rotation",
                  "kernel_us": round(attn_ms * 1e3, 3), "peak_source": peaks["source"] + " (burst)",
                  "algorithmic_bytes": b.attn_bytes(), "algorithmic_flops": b.flops()})
 
@@ -421,7 +421,7 @@ def main():
                        "head_dim": b.head_dim, "page": si.PAGE, "parallelism": f"replicas x{world}",
                        "l2": f"cold: steps rotate over {w.nsets} independent pool sets "
                              f"({w.nsets * b.attn_bytes() / 1e6:.0f} MB distinct per rotation)",
-                       "step": "CUDA-graph replay of kv_write + block_attn (plan + tcgen05 attention + combine)"},
+                       "step": "CUDA-graph replay of kv_write + block_attn (plan + tcgen05 attention + fused split-KV merge)"},
             "us_per_iteration": round(ms_step * 1e3, 3), "attn_us": round(attn_ms * 1e3, 3),
             "kv_write_us": round(write_ms * 1e3, 3),
             "clocks": cs.summary(), "e2e": e2e, "gpu_launches": gpu_launches,

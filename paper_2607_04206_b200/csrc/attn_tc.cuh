@@ -1,18 +1,26 @@
-// attn_tc.cuh -- steps a3..a8: paged, varlen, non-causal block attention on tcgen05 (sm_100a).
+// attn_tc.cuh -- steps a3..a9: paged, varlen, non-causal block attention on tcgen05 (sm_100a).
 //
-// One persistent CTA per SM, 8 warps, warp-specialised:
-//   warp 0      scheduler + TMA producer: plans the work on the device (a3), gathers K/V pages of
+// One persistent CTA per SM, 12 warps, warp-specialised, TWO softmax streams per CTA:
+//   warp 0      scheduler + TMA producer: plans the work on the device (a3) and gathers K/V pages of
 //               the current (request, kv head) through the block table with TMA into a ring of
 //               128-row, 128B-swizzled shared-memory tiles (a4)
-//   warp 1      MMA issuer: S = Q K^T (tcgen05.mma, operands in smem, S in TMEM; a5) and
-//               O += P V (P read from TMEM, V from smem, O in TMEM; a7)
-//   warp 2      TMEM allocator
-//   warps 4-7   softmax warpgroup: thread i owns row i of the tile (TMEM lane i): online softmax
-//               in fp32 (a6), P written back to TMEM as bf16, O rescale, epilogue (a8)
-// Work unit = (request r, kv head g, 128-row tile of the packed (query row, q head in group) rows):
-// the G q heads of a GQA group share every K/V tile.  A unit's kv range may be split across CTAs
-// (static stream-K partition for decode-sized batches); partials go to the workspace and are merged
-// by combine_kernel (a9).  With many units (prefill / hybrid) whole units are handed out dynamically.
+//   warp 1      MMA issuer: S_s = Q_s K^T (tcgen05.mma, operands in smem, S in TMEM; a5) and
+//               O_s += P_s V (P read from TMEM, V from smem, O in TMEM; a7) for streams s = 0, 1
+//   warps 2-3   Q loader: packed (query row, q head of the group) rows -> swizzled smem, 2-slot ring
+//               (warp 2 also owns the TMEM allocation)
+//   warps 4-7   softmax warpgroup of stream 0;  warps 8-11: stream 1.  Thread i owns row i of the
+//               stream's tile (TMEM lane i): online softmax in fp32 with a lazily updated reference
+//               maximum (a6), P written back over S as bf16, epilogue (a8), fused split-KV merge (a9)
+// Work unit = (request r, kv head g, PAIR of 128-row tiles of the packed rows).  Two modes per unit:
+//   SHARED  (more than 128 rows in the pair): stream s owns q tile s, both streams consume the same
+//           K/V tile -- the G q heads of a GQA group and the two q tiles share every K/V byte.
+//   SPLIT   (at most 128 rows): both streams work on the one q tile, stream s takes the kv tiles
+//           kv0 + 2i + s; the two partial results are merged in the epilogue (in-CTA split-KV).
+// While one stream's warpgroup runs its softmax the tensor pipe works for the other stream.
+// A unit's kv range may also be split across CTAs (static stream-K partition for decode-sized
+// batches): pieces go to the workspace as (O fp32, m, l) and the CTA that finishes a unit's last
+// piece merges them in fixed slot order (bitwise reproducible).  With many units (prefill / hybrid)
+// whole units are handed out dynamically.
 // The attention definition is PAPER.md:67 (no causal mask) over the context of PAPER.md:33.
 #pragma once
 #include <cuda.h>
@@ -28,49 +36,53 @@ namespace tc {
 
 constexpr int BM = 128;          // rows per q tile  (UMMA M)
 constexpr int BN = 128;          // kv positions per tile (8 pages)
-constexpr int NSTAGE = 6;        // K/V tile ring depth
-constexpr int NTHREADS = 256;
+constexpr int PAIR = 2 * BM;     // packed rows per work unit
+constexpr int NSTAGE = 5;        // K/V tile ring depth
+constexpr int NTHREADS = 384;
 constexpr int SLAB = 128 * 128;  // bytes of one 64-wide swizzled slab of a 128-row tile
 constexpr int DYN_UNITS_PER_CTA = 4;   // >= this many units per CTA: whole units, dynamic hand-out
+constexpr float LAZY_T = 8.f;    // the reference maximum moves only when a tile exceeds it by 2^8
+#ifndef SANGAM_POLY_EXP
+#define SANGAM_POLY_EXP 0        // of every 8 exponentials, this many run on the FMA pipe instead of MUFU
+#endif
 
-struct Item {          // one piece of work, published through shared memory
+struct Item {          // one piece of work, published through shared memory (64 bytes)
     int valid;         // 0 = no more work
     int r, g;
-    int row0;          // first packed row of the tile inside the (r, g) unit group
-    int rows_valid;    // rows of this tile that exist (<= 128)
+    int row0;          // first packed row of the pair inside the (r, g) group
+    int rows0, rows1;  // rows of q tile 0 / 1 that exist; rows1 > 0 <=> SHARED mode
     int q_start;       // cu_q_lens[r]
     int c;             // context length
     int kv0, kv1;      // kv tile range [kv0, kv1)
     int part_slot;     // -1: write `out`; else partial slot in the workspace
-    int pad0, pad1;
-};
-
-struct SlotMeta {      // global, one per partial slot, rewritten by its CTA every launch
-    int valid;
-    int b_last;        // head slots: last CTA holding a piece of this unit
-    int g, row0, rows_valid, q_start;
-    int pad0, pad1;
+    int b_head;        // split units: CTA holding the piece that starts at kv tile 0
+    int npieces;       // split units: number of CTAs holding a piece
+    int pad0, pad1, pad2;
 };
 
 template <int D>
 struct Smem {
     static constexpr int Q_BYTES = BM * D * 2;
     static constexpr int KV_BYTES = BN * D * 2;
-    static constexpr int OFF_Q = 0;
-    static constexpr int OFF_KV = Q_BYTES;
+    static constexpr int OFF_Q = 0;                       // 2 q-tile slots
+    static constexpr int OFF_KV = 2 * Q_BYTES;
     static constexpr int OFF_BAR = OFF_KV + NSTAGE * KV_BYTES;
     // barrier indices
-    static constexpr int B_KV_FULL = 0, B_KV_EMPTY = NSTAGE, B_ITEM_FULL = 2 * NSTAGE, B_ITEM_EMPTY = 2 * NSTAGE + 2,
-                         B_Q_FULL = 2 * NSTAGE + 4, B_S_FULL = 2 * NSTAGE + 5, B_P_FULL = 2 * NSTAGE + 7,
-                         B_PV_DONE = 2 * NSTAGE + 9, NBAR = 2 * NSTAGE + 10;
+    static constexpr int B_KV_FULL = 0, B_KV_EMPTY = NSTAGE, B_ITEM_FULL = 2 * NSTAGE, B_ITEM_EMPTY = B_ITEM_FULL + 2,
+                         B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 2, B_S_FULL = B_Q_EMPTY + 2,
+                         B_P_FULL = B_S_FULL + 2, B_PV_DONE = B_P_FULL + 2, B_EPI_A = B_PV_DONE + 2,
+                         B_EPI_B = B_EPI_A + 1, B_EPI_C = B_EPI_B + 1, B_EPI_D = B_EPI_C + 1, NBAR = B_EPI_D + 1;
     static constexpr int OFF_ITEMS = OFF_BAR + ((NBAR * 8 + 15) / 16) * 16;
-    static constexpr int OFF_MISC = OFF_ITEMS + 2 * (int)sizeof(Item);
+    static constexpr int OFF_ML = OFF_ITEMS + 2 * (int)sizeof(Item);    // (m, l) of stream 1, 128 rows
+    static constexpr int OFF_MISC = OFF_ML + BM * 8;
     static constexpr int TOTAL = OFF_MISC + 16;
     static constexpr int ALLOC = TOTAL + 1024;   // slack to align the base to 1024 B (128B swizzle atoms)
 };
+static_assert(sizeof(Item) == 64, "Item is 64 bytes");
+static_assert(Smem<128>::ALLOC <= 232448, "shared memory budget (227 KB)");
 
 struct ReqInfo {
-    int q0, c, nm, tiles_u, units, rows;
+    int q0, c, np, tiles_u, units, rows;
 };
 
 __device__ __forceinline__ ReqInfo req_info(const AttnParams& p, int r) {
@@ -83,21 +95,57 @@ __device__ __forceinline__ ReqInfo req_info(const AttnParams& p, int r) {
     if ((c + SANGAM_PAGE - 1) / SANGAM_PAGE > p.W) { raise_flag(p.flags, DEV_CTX_TOO_LONG); c = 0; }
     x.c = c;
     x.rows = qn * p.G;
-    x.nm = (x.rows + BM - 1) / BM;
+    x.np = (x.rows + PAIR - 1) / PAIR;
     const int nkv = (c + BN - 1) / BN;
     x.tiles_u = nkv > 0 ? nkv : 1;
-    x.units = p.Hkv * x.nm;
+    x.units = p.Hkv * x.np;
     return x;
 }
 
+// The order in which the MMA warp consumes K/V tiles of one item; the producer loads in the same
+// order.  Op k = 0, 1: QK of stream k, tile index 0.  Then rounds j = 0, 1, ...:
+//   PV(0, j), QK(0, j+1), PV(1, j), QK(1, j+1).
+// SHARED: stream 0 acquires a ring stage, stream 1 reuses and releases it.  SPLIT: every op has its own.
+struct Op {
+    int is_pv, s, i, tile, acquire, release;
+};
+struct OpWalk {
+    int shared, kv0, n0, n1, nops, k;
+    __device__ __forceinline__ OpWalk(const Item& it) {
+        const int n = it.kv1 - it.kv0;
+        shared = it.rows1 > 0;
+        kv0 = it.kv0;
+        n0 = shared ? n : (n + 1) / 2;
+        n1 = shared ? n : n / 2;
+        nops = n > 0 ? 2 + 4 * n0 : 0;
+        k = 0;
+    }
+    __device__ __forceinline__ bool next(Op& op) {
+        while (k < nops) {
+            const int kk = k++;
+            if (kk < 2) { op.is_pv = 0; op.s = kk; op.i = 0; }
+            else {
+                const int j = (kk - 2) >> 2, ph = (kk - 2) & 3;
+                op.is_pv = (ph & 1) ^ 1;
+                op.s = ph >> 1;
+                op.i = op.is_pv ? j : j + 1;
+            }
+            if (op.i >= (op.s ? n1 : n0)) continue;
+            op.tile = shared ? kv0 + op.i : kv0 + 2 * op.i + op.s;
+            op.acquire = shared ? (op.s == 0) : 1;
+            op.release = shared ? (op.s == 1) : 1;
+            return true;
+        }
+        return false;
+    }
+};
 
 // ------------------------------------------------------------------------------------------------
 // warp 0: device-side plan (a3) + TMA page gather (a4)
 // ------------------------------------------------------------------------------------------------
 template <int D>
-__device__ __forceinline__ void producer_warp(const AttnParams& p, SlotMeta* meta, const CUtensorMap* mapK,
-                                              const CUtensorMap* mapV, uint32_t sbase, Item* items,
-                                              volatile uint32_t* abort_flag, int lane) {
+__device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtensorMap* mapK, const CUtensorMap* mapV,
+                                              uint32_t sbase, Item* items, volatile uint32_t* abort_flag, int lane) {
     using L = Smem<D>;
     const unsigned FULL = 0xffffffffu;
     const int G_ctas = gridDim.x, b = blockIdx.x, R = p.batch;
@@ -116,13 +164,11 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, SlotMeta* met
         T += __shfl_xor_sync(FULL, T, o);
     }
     const bool dynamic = U >= DYN_UNITS_PER_CTA * G_ctas;
-    if (lane < 2) meta[2 * b + lane].valid = 0;
-    __syncwarp();
 
     // walking state
     int r_cur = 0, ubase = 0, u_in_r = 0, kvoff = 0, remaining = 0, tile_base = 0, Geff = 1;
     ReqInfo cur;
-    cur.units = 0; cur.tiles_u = 1; cur.nm = 1; cur.c = 0; cur.q0 = 0; cur.rows = 0;
+    cur.units = 0; cur.tiles_u = 1; cur.np = 1; cur.c = 0; cur.q0 = 0; cur.rows = 0;
     if (R > 0) cur = req_info(p, 0);
     if (!dynamic && T > 0) {
         Geff = G_ctas < T ? G_ctas : T;
@@ -166,8 +212,8 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, SlotMeta* met
     while (true) {
         if (*abort_flag) break;
         Item it;
-        it.valid = 0; it.r = 0; it.g = 0; it.row0 = 0; it.rows_valid = 0; it.q_start = 0; it.c = 0;
-        it.kv0 = 0; it.kv1 = 0; it.part_slot = -1; it.pad0 = 0; it.pad1 = 0;
+        it.valid = 0; it.r = 0; it.g = 0; it.row0 = 0; it.rows0 = 0; it.rows1 = 0; it.q_start = 0; it.c = 0;
+        it.kv0 = 0; it.kv1 = 0; it.part_slot = -1; it.b_head = 0; it.npieces = 1; it.pad0 = 0; it.pad1 = 0; it.pad2 = 0;
         if (dynamic) {
             int u = 0;
             if (lane == 0) u = atomicAdd(p.sched, 1);
@@ -180,29 +226,25 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, SlotMeta* met
                 }
                 if (r_cur < R) {
                     const int ul = u - ubase;
-                    it.valid = 1; it.r = r_cur; it.g = ul / cur.nm;
-                    it.row0 = (ul - it.g * cur.nm) * BM;
+                    it.valid = 1; it.r = r_cur; it.g = ul / cur.np;
+                    it.row0 = (ul - it.g * cur.np) * PAIR;
                     it.kv0 = 0; it.kv1 = cur.tiles_u;
                 }
             }
         } else if (remaining > 0 && r_cur < R) {
             const int take = remaining < cur.tiles_u - kvoff ? remaining : cur.tiles_u - kvoff;
-            it.valid = 1; it.r = r_cur; it.g = u_in_r / cur.nm;
-            it.row0 = (u_in_r - it.g * cur.nm) * BM;
+            it.valid = 1; it.r = r_cur; it.g = u_in_r / cur.np;
+            it.row0 = (u_in_r - it.g * cur.np) * PAIR;
             it.kv0 = kvoff; it.kv1 = kvoff + take;
             if (!(it.kv0 == 0 && it.kv1 == cur.tiles_u)) {
-                const bool head = it.kv0 == 0;
-                it.part_slot = 2 * b + (head ? 1 : 0);
-                if (lane == 0) {
-                    SlotMeta mm;
-                    mm.valid = 1; mm.g = it.g; mm.row0 = it.row0;
-                    mm.rows_valid = cur.rows - it.row0 < BM ? cur.rows - it.row0 : BM;
-                    mm.q_start = cur.q0; mm.pad0 = it.r; mm.pad1 = 0;
-                    const int64_t ut1 = (int64_t)tile_base + (int64_t)(u_in_r + 1) * cur.tiles_u;
-                    int bl = (int)((ut1 * Geff + T - 1) / T) - 1;
-                    mm.b_last = bl > Geff - 1 ? Geff - 1 : bl;
-                    meta[it.part_slot] = mm;
-                }
+                // a piece of a unit split across CTAs: CTA x holds flattened tiles [floor(xT/Geff), floor((x+1)T/Geff))
+                it.part_slot = 2 * b + (it.kv0 == 0 ? 1 : 0);
+                const int64_t ut0 = (int64_t)tile_base + (int64_t)u_in_r * cur.tiles_u, ut1 = ut0 + cur.tiles_u;
+                const int bh = (int)(((ut0 + 1) * Geff + T - 1) / T) - 1;
+                int bl = (int)((ut1 * Geff + T - 1) / T) - 1;
+                bl = bl > Geff - 1 ? Geff - 1 : bl;
+                it.b_head = bh;
+                it.npieces = bl - bh + 1;
             }
             remaining -= take;
             kvoff += take;
@@ -218,10 +260,12 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, SlotMeta* met
                 }
             }
         }
-        ReqInfo ri = cur;
         if (it.valid) {
+            ReqInfo ri = cur;
             if (it.r != r_cur) ri = req_info(p, it.r);   // static walk may already have advanced
-            it.rows_valid = ri.rows - it.row0 < BM ? ri.rows - it.row0 : BM;
+            const int left = ri.rows - it.row0;
+            it.rows0 = left < BM ? left : BM;
+            it.rows1 = left > BM ? (left - BM < BM ? left - BM : BM) : 0;
             it.q_start = ri.q0;
             it.c = ri.c;
             if (ri.c == 0) { it.kv0 = 0; it.kv1 = 0; }
@@ -237,35 +281,30 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, SlotMeta* met
         ++icount;
         if (!it.valid) break;
 
-        // K/V tile loads in the order the MMA warp consumes them: K0, [K1], V0, [K2], V1, ...
-        const int n = it.kv1 - it.kv0;
+        // K/V tile loads in the order the MMA warp consumes them (OpWalk)
         const int pages_total = (it.c + SANGAM_PAGE - 1) / SANGAM_PAGE;
         const int32_t* bt = p.block_table + (int64_t)it.r * p.W;
-        auto load_tile = [&](int tile, bool is_v) {
+        OpWalk walk(it);
+        Op op;
+        while (walk.next(op)) {
+            if (!op.acquire) continue;
+            if (*abort_flag) break;
             const uint32_t stage = kvi % NSTAGE;
             ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), ((kvi / NSTAGE) & 1u) ^ 1u, abort_flag);
-            int np = pages_total - tile * 8;
+            int np = pages_total - op.tile * 8;
             np = np > 8 ? 8 : np;
             constexpr int BOX_PER_PAGE = D / 64;
             if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_KV_FULL + stage), (uint32_t)(np * SANGAM_PAGE * D * 2));
             __syncwarp();
             if (lane < np * BOX_PER_PAGE) {
                 const int pg = lane / BOX_PER_PAGE, slab = lane % BOX_PER_PAGE;
-                const int page = __ldg(bt + tile * 8 + pg);
+                const int page = __ldg(bt + op.tile * 8 + pg);
                 if ((unsigned)page >= (unsigned)p.P) raise_flag(p.flags, DEV_BAD_PAGE);   // TMA zero-fills out of range
                 ptx::tma_load_2d(sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES + slab * SLAB + pg * 2048),
-                                 is_v ? mapV : mapK, bar(L::B_KV_FULL + stage), slab * 64,
+                                 op.is_pv ? mapV : mapK, bar(L::B_KV_FULL + stage), slab * 64,
                                  (page * p.Hkv + it.g) * SANGAM_PAGE);
             }
             ++kvi;
-        };
-        if (n > 0) {
-            load_tile(it.kv0, false);
-            for (int j = 0; j < n; ++j) {
-                if (*abort_flag) break;
-                if (j + 1 < n) load_tile(it.kv0 + j + 1, false);
-                load_tile(it.kv0 + j, true);
-            }
         }
     }
     if (dynamic && lane == 0) {
@@ -277,92 +316,56 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, SlotMeta* met
     }
 }
 
-
 // ------------------------------------------------------------------------------------------------
-// warp 1: MMA issuer (a5, a7).  TMEM columns: S0 = [0,128), S1 = [128,256), O = [256,256+D).
-// P_b (bf16, two per column) overwrites the first 64 columns of S_b.
-// Issue order per item: QK0, [QK1], PV0, [QK2], PV1, ...  -- the next tile's logits are computed
-// while the softmax warpgroup works on the current one.
+// warps 2-3: Q loader.  Packed row rg of the (r, g) group = (token rg / G, q head g*G + rg % G).
+// Rows go to a 2-slot ring of 128-row tiles in the K-major 128B-swizzled UMMA layout.
 // ------------------------------------------------------------------------------------------------
 template <int D>
-__device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, uint32_t tmem, const Item* items,
-                                         volatile uint32_t* abort_flag, int lane) {
+__device__ __forceinline__ void qload_warps(const AttnParams& p, uint8_t* smem, uint32_t sbase, const Item* items,
+                                            volatile uint32_t* abort_flag, int tid64, int lane) {
     using L = Smem<D>;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
-    const uint32_t q_addr = sbase + L::OFF_Q;
-    uint32_t kvi = 0, icount = 0, tcount = 0;
+    constexpr int CPR = D / 8;                 // 16-byte chunks per row
+    constexpr int RPP = 64 / CPR;              // rows per pass of the 64 loader threads
+    const int chunk = tid64 % CPR, rsub = tid64 / CPR;
+    const int slab = chunk >> 3, c16 = chunk & 7;
+    uint32_t icount = 0, qcount = 0;
     while (true) {
         if (*abort_flag) break;
         const uint32_t islot = icount & 1u;
         ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
         const Item it = items[islot];
         if (!it.valid) break;
-        const int n = it.kv1 - it.kv0;
-        ptx::mbar_wait(bar(L::B_Q_FULL), icount & 1u, abort_flag);
-        ptx::tc_fence_after();
-        auto issue_qk = [&](int j, uint32_t sb) {
-            const uint32_t stage = kvi % NSTAGE;
-            ptx::mbar_wait(bar(L::B_KV_FULL + stage), (kvi / NSTAGE) & 1u, abort_flag);
-            ptx::tc_fence_after();
-            int nv = it.c - (it.kv0 + j) * BN;
-            nv = nv > BN ? BN : nv;
-            const uint32_t ncols = (uint32_t)((nv + 15) & ~15);
-            if (lane == 0) {
-                const uint32_t k_addr = sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES);
-                const uint32_t idesc = ptx::idesc_bf16(BM, ncols, 0, 0);
+        const int nq = it.kv1 > it.kv0 ? (it.rows1 > 0 ? 2 : 1) : 0;   // c = 0: no MMA, no q tile
+        for (int t = 0; t < nq; ++t) {
+            const uint32_t qs = qcount & 1u;
+            ptx::mbar_wait(bar(L::B_Q_EMPTY + qs), ((qcount >> 1) & 1u) ^ 1u, abort_flag);
+            const int rows = t ? it.rows1 : it.rows0;
+            const int rows_pad = (rows + 31) & ~31;      // partially valid warps see zeros, not stale bits
+            uint8_t* dst = smem + L::OFF_Q + qs * L::Q_BYTES + slab * SLAB;
+            constexpr int UN = 8;
+            for (int i0 = 0; i0 < rows_pad; i0 += RPP * UN) {
+                uint4 v[UN];
 #pragma unroll
-                for (int ks = 0; ks < D / 16; ++ks) {
-                    const uint32_t off = (uint32_t)((ks >> 2) * SLAB + (ks & 3) * 32);
-                    ptx::mma_ss(tmem + sb * 128u, ptx::smem_desc_sw128(q_addr + off, 16, 1024),
-                                ptx::smem_desc_sw128(k_addr + off, 16, 1024), idesc, ks > 0);
-                }
-                ptx::mma_commit(bar(L::B_KV_EMPTY + stage));
-                ptx::mma_commit(bar(L::B_S_FULL + sb));
-            }
-            __syncwarp();
-            ++kvi;
-        };
-        if (n > 0) {
-            issue_qk(0, tcount & 1u);
-            for (int j = 0; j < n; ++j) {
-                if (*abort_flag) break;
-                const uint32_t sb = tcount & 1u;
-                if (j + 1 < n) issue_qk(j + 1, sb ^ 1u);
-                const uint32_t stage = kvi % NSTAGE;
-                ptx::mbar_wait(bar(L::B_KV_FULL + stage), (kvi / NSTAGE) & 1u, abort_flag);
-                int nv = it.c - (it.kv0 + j) * BN;
-                nv = nv > BN ? BN : nv;
-                const int ncols = (nv + 15) & ~15;
-                const uint32_t v_addr = sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES);
-                if (nv < ncols) {
-                    // stale rows of the last page: zero them so that P = 0 meets V = 0, never NaN (reading S12)
-                    const int nrows = ncols - nv;
-                    for (int e = lane; e < nrows * 8 * (D / 64); e += 32) {
-                        const int chunk = e & 7, rr = (e >> 3) % nrows, slab = (e >> 3) / nrows;
-                        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(
-                                         v_addr + (uint32_t)(slab * SLAB + (nv + rr) * 128 + chunk * 16)),
-                                     "r"(0)
-                                     : "memory");
+                for (int u = 0; u < UN; ++u) {
+                    const int rr = i0 + u * RPP + rsub;
+                    v[u] = make_uint4(0, 0, 0, 0);
+                    if (rr < rows) {
+                        const int rg = it.row0 + t * BM + rr;
+                        const int tl = rg / p.G, hh = rg - tl * p.G;
+                        v[u] = __ldg(reinterpret_cast<const uint4*>(p.q + ((int64_t)(it.q_start + tl) * p.Hq + it.g * p.G + hh) * D) + chunk);
                     }
-                    ptx::fence_proxy_async_smem();
-                    __syncwarp();
                 }
-                ptx::mbar_wait(bar(L::B_P_FULL + sb), (tcount >> 1) & 1u, abort_flag);
-                ptx::tc_fence_after();
-                if (lane == 0) {
-                    const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
-                    const int nk = ncols / 16;
-                    for (int ks = 0; ks < nk; ++ks)
-                        ptx::mma_ts(tmem + 256u, tmem + sb * 128u + (uint32_t)(ks * 8),
-                                    ptx::smem_desc_sw128(v_addr + (uint32_t)(ks * 2048), SLAB, 1024), idesc,
-                                    (j > 0 || ks > 0) ? 1u : 0u);
-                    ptx::mma_commit(bar(L::B_KV_EMPTY + stage));
-                    ptx::mma_commit(bar(L::B_PV_DONE));
+#pragma unroll
+                for (int u = 0; u < UN; ++u) {
+                    const int rr = i0 + u * RPP + rsub;
+                    if (rr < rows_pad) *reinterpret_cast<uint4*>(dst + rr * 128 + ((c16 ^ (rr & 7)) << 4)) = v[u];
                 }
-                __syncwarp();
-                ++kvi;
-                ++tcount;
             }
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_Q_FULL + qs));
+            ++qcount;
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
@@ -371,178 +374,413 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
 }
 
 // ------------------------------------------------------------------------------------------------
-// warps 4-7: softmax warpgroup (a6) + epilogue (a8).  Thread `row` owns TMEM lane `row`.
+// warp 1: MMA issuer (a5, a7).  TMEM columns: S_s = [128 s, 128 s + 128), O_s = [256 + 128 s, .. + D).
+// P_s (bf16, two per column) overwrites the first 64 columns of S_s.
 // ------------------------------------------------------------------------------------------------
-template <bool MASK>
-__device__ __forceinline__ void softmax_row(uint32_t s_taddr, int nv, float scale_log2, float& m, float& l,
-                                            float& alpha, uint32_t (&pk)[64]) {
-    uint32_t r[4][32];
-#pragma unroll
-    for (int c = 0; c < 4; ++c) ptx::tmem_ld32(s_taddr + (uint32_t)(c * 32), r[c]);
-    ptx::tmem_wait_ld();
-    float mx = -INFINITY;
-    if (scale_log2 >= 0.f) {
-#pragma unroll
-        for (int c = 0; c < 4; ++c)
-#pragma unroll
-            for (int i = 0; i < 32; ++i)
-                if (!MASK || c * 32 + i < nv) mx = fmaxf(mx, __uint_as_float(r[c][i]));
-    } else {
-#pragma unroll
-        for (int c = 0; c < 4; ++c)
-#pragma unroll
-            for (int i = 0; i < 32; ++i)
-                if (!MASK || c * 32 + i < nv) mx = fmaxf(mx, -__uint_as_float(r[c][i]));
-        mx = -mx;
-    }
-    const float m_new = fmaxf(m, mx * scale_log2);
-    alpha = ptx::ex2(m - m_new);
-    const float neg = -m_new;
-    float sum0 = 0.f, sum1 = 0.f;
-#pragma unroll
-    for (int c = 0; c < 4; ++c)
-#pragma unroll
-        for (int i = 0; i < 16; ++i) {
-            float p0 = ptx::ex2(fmaf(__uint_as_float(r[c][2 * i]), scale_log2, neg));
-            float p1 = ptx::ex2(fmaf(__uint_as_float(r[c][2 * i + 1]), scale_log2, neg));
-            if (MASK) {
-                if (c * 32 + 2 * i >= nv) p0 = 0.f;
-                if (c * 32 + 2 * i + 1 >= nv) p1 = 0.f;
-            }
-            sum0 += p0;
-            sum1 += p1;
-            pk[c * 16 + i] = ptx::pack_bf16(p0, p1);
-        }
-    l = l * alpha + (sum0 + sum1);
-    m = m_new;
-}
-
 template <int D>
-__device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, uint32_t sbase, uint32_t tmem,
-                                           const Item* items, volatile uint32_t* abort_flag, int wg_warp, int lane) {
+__device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, uint32_t tmem, const Item* items,
+                                         volatile uint32_t* abort_flag, int lane) {
     using L = Smem<D>;
-    const unsigned FULL = 0xffffffffu;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
-    const int row = wg_warp * 32 + lane;
-    const int wtid = wg_warp * 32 + lane;   // 0..127
-    const uint32_t lane_base = (uint32_t)(wg_warp * 32) << 16;
-    const uint32_t o_taddr = tmem + lane_base + 256u;
-    uint32_t icount = 0, tcount = 0;
+    uint32_t kvi = 0, icount = 0, qcount = 0;
+    uint32_t pv_cnt0 = 0u, pv_cnt1 = 0u;
     while (true) {
         if (*abort_flag) break;
         const uint32_t islot = icount & 1u;
         ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
         const Item it = items[islot];
         if (!it.valid) break;
-        // ---- Q tile -> smem, 128B swizzle, zero rows past rows_valid
-        {
-            constexpr int CPR = D / 8;                 // 16-byte chunks per row
-            constexpr int RPP = 128 / CPR;             // rows per pass
-            const int chunk = wtid % CPR, rsub = wtid / CPR;
-#pragma unroll 4
-            for (int i = 0; i < BM / RPP; ++i) {
-                const int rr = i * RPP + rsub;
-                uint4 v = make_uint4(0, 0, 0, 0);
-                if (rr < it.rows_valid) {
-                    const int rg = it.row0 + rr;
-                    const int tl = rg / p.G, hh = rg - tl * p.G;
-                    v = __ldg(reinterpret_cast<const uint4*>(p.q + ((int64_t)(it.q_start + tl) * p.Hq + it.g * p.G + hh) * D) + chunk);
-                }
-                const int slab = chunk >> 3, c16 = chunk & 7;
-                *reinterpret_cast<uint4*>(smem + L::OFF_Q + slab * SLAB + rr * 128 + ((c16 ^ (rr & 7)) << 4)) = v;
-            }
-            ptx::fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(bar(L::B_Q_FULL));
-        }
-        const bool warp_active = wg_warp * 32 < it.rows_valid;
         const int n = it.kv1 - it.kv0;
-        float m = -INFINITY, l = 0.f;
-        for (int j = 0; j < n; ++j) {
-            if (*abort_flag) break;
-            const uint32_t sb = tcount & 1u;
-            ptx::mbar_wait(bar(L::B_S_FULL + sb), (tcount >> 1) & 1u, abort_flag);
+        const int shared = it.rows1 > 0;
+        const int nq = shared ? 2 : 1;
+        if (n > 0) {
+            // q tiles of this item: ring slots (qcount + t) & 1
+            for (int t = 0; t < nq; ++t)
+                ptx::mbar_wait(bar(L::B_Q_FULL + ((qcount + t) & 1u)), ((qcount + t) >> 1) & 1u, abort_flag);
             ptx::tc_fence_after();
-            int nv = it.c - (it.kv0 + j) * BN;
-            nv = nv > BN ? BN : nv;
-            float alpha = 1.f;
-            const uint32_t s_taddr = tmem + lane_base + sb * 128u;
-            if (warp_active) {
-                uint32_t pk[64];
-                if (nv == BN) softmax_row<false>(s_taddr, nv, p.scale_log2, m, l, alpha, pk);
-                else softmax_row<true>(s_taddr, nv, p.scale_log2, m, l, alpha, pk);
-                ptx::tmem_st32(s_taddr, *reinterpret_cast<const uint32_t(*)[32]>(&pk[0]));
-                ptx::tmem_st32(s_taddr + 32u, *reinterpret_cast<const uint32_t(*)[32]>(&pk[32]));
+            OpWalk walk(it);
+            const int n0 = walk.n0, n1 = walk.n1;
+            Op op;
+            uint32_t stage_k = 0, stage_v = 0;
+            while (walk.next(op)) {
+                if (*abort_flag) break;
+                int nv = it.c - op.tile * BN;
+                nv = nv > BN ? BN : nv;
+                const int ncols = (nv + 15) & ~15;
+                if (!op.is_pv) {
+                    if (op.acquire) {
+                        stage_k = kvi % NSTAGE;
+                        ptx::mbar_wait(bar(L::B_KV_FULL + stage_k), (kvi / NSTAGE) & 1u, abort_flag);
+                        ptx::tc_fence_after();
+                        ++kvi;
+                    }
+                    const uint32_t qs = (qcount + (shared ? (uint32_t)op.s : 0u)) & 1u;
+                    const bool last_qk = shared ? (op.i == n0 - 1)
+                                                : ((op.s == 0 && op.i == n0 - 1 && n0 > n1) || (op.s == 1 && op.i == n1 - 1 && n1 == n0));
+                    if (lane == 0) {
+                        const uint32_t q_addr = sbase + (uint32_t)(L::OFF_Q + qs * L::Q_BYTES);
+                        const uint32_t k_addr = sbase + (uint32_t)(L::OFF_KV + stage_k * L::KV_BYTES);
+                        const uint32_t idesc = ptx::idesc_bf16(BM, (uint32_t)ncols, 0, 0);
+#pragma unroll
+                        for (int ks = 0; ks < D / 16; ++ks) {
+                            const uint32_t off = (uint32_t)((ks >> 2) * SLAB + (ks & 3) * 32);
+                            ptx::mma_ss(tmem + (uint32_t)op.s * 128u, ptx::smem_desc_sw128(q_addr + off, 16, 1024),
+                                        ptx::smem_desc_sw128(k_addr + off, 16, 1024), idesc, ks > 0);
+                        }
+                        if (op.release) ptx::mma_commit(bar(L::B_KV_EMPTY + stage_k));
+                        ptx::mma_commit(bar(L::B_S_FULL + op.s));
+                        if (last_qk) ptx::mma_commit(bar(L::B_Q_EMPTY + qs));
+                    }
+                    __syncwarp();
+                } else {
+                    if (op.acquire) {
+                        stage_v = kvi % NSTAGE;
+                        ptx::mbar_wait(bar(L::B_KV_FULL + stage_v), (kvi / NSTAGE) & 1u, abort_flag);
+                        ++kvi;
+                        if (nv < ncols) {
+                            // stale rows of the last page: zero them so that P = 0 meets V = 0, never NaN (reading S12)
+                            const uint32_t v_addr = sbase + (uint32_t)(L::OFF_KV + stage_v * L::KV_BYTES);
+                            const int nrows = ncols - nv;
+                            for (int e = lane; e < nrows * 8 * (D / 64); e += 32) {
+                                const int chunk = e & 7, rr = (e >> 3) % nrows, slab = (e >> 3) / nrows;
+                                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(
+                                                 v_addr + (uint32_t)(slab * SLAB + (nv + rr) * 128 + chunk * 16)),
+                                             "r"(0)
+                                             : "memory");
+                            }
+                            ptx::fence_proxy_async_smem();
+                            __syncwarp();
+                        }
+                    }
+                    ptx::mbar_wait(bar(L::B_P_FULL + op.s), (op.s ? pv_cnt1 : pv_cnt0) & 1u, abort_flag);
+                    ptx::tc_fence_after();
+                    if (lane == 0) {
+                        const uint32_t v_addr = sbase + (uint32_t)(L::OFF_KV + stage_v * L::KV_BYTES);
+                        const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
+                        const int nk = ncols / 16;
+                        for (int ks = 0; ks < nk; ++ks)
+                            ptx::mma_ts(tmem + 256u + (uint32_t)op.s * 128u, tmem + (uint32_t)op.s * 128u + (uint32_t)(ks * 8),
+                                        ptx::smem_desc_sw128(v_addr + (uint32_t)(ks * 2048), SLAB, 1024), idesc,
+                                        (op.i > 0 || ks > 0) ? 1u : 0u);
+                        if (op.release) ptx::mma_commit(bar(L::B_KV_EMPTY + stage_v));
+                        ptx::mma_commit(bar(L::B_PV_DONE + op.s));
+                    }
+                    __syncwarp();
+                    if (op.s) ++pv_cnt1; else ++pv_cnt0;
+                }
             }
-            if (j > 0) {
-                ptx::mbar_wait(bar(L::B_PV_DONE), (tcount - 1u) & 1u, abort_flag);
-                ptx::tc_fence_after();
-                if (warp_active && __any_sync(FULL, alpha != 1.f)) {
+            qcount += nq;
+        }
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
+        ++icount;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// warps 4-11: softmax warpgroups (a6) + epilogue (a8) + fused split-KV merge (a9).
+// Thread `row` of stream s owns TMEM lane `row` of S_s / O_s.
+// ------------------------------------------------------------------------------------------------
+// 2^x on the FMA pipe (Cody-Waite split + degree-3 minimax on [-0.5, 0.5], rel. error 7.6e-5 --
+// far below the bf16 rounding of P); relieves the 16/clk/SM MUFU unit, the co-critical pipe of prefill.
+__device__ __forceinline__ float ex2_poly(float x) {
+    x = fmaxf(x, -125.f);
+    const float t = x + 12582912.f;            // 1.5 * 2^23: round(x) sits in the low mantissa bits
+    const float f = x - (t - 12582912.f);
+    float y = fmaf(f, 0.05520550534129143f, 0.24261397123336792f);
+    y = fmaf(y, f, 0.6932547688484192f);
+    y = fmaf(y, f, 0.9999276995658875f);
+    return __int_as_float(__float_as_int(y) + (__float_as_int(t) << 23));
+}
+
+// One 128-column tile of one row: returns alpha (the factor by which O and l shrink; 1 if the
+// reference maximum m_ref stays).  m_ref is in log2 units and is only raised when the tile maximum
+// exceeds it by more than LAZY_T, so p = 2^(x - m_ref) <= 2^LAZY_T: exact in range for bf16 / fp32.
+template <bool MASK, bool NEG>
+__device__ __forceinline__ float softmax_tile(uint32_t s_taddr, int nv, float scale_log2, float& m_ref, float& l) {
+    uint32_t r[4][32];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) ptx::tmem_ld32(s_taddr + (uint32_t)(c * 32), r[c]);
+    ptx::tmem_wait_ld();
+    float mx4[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        float a = -INFINITY;
+#pragma unroll
+        for (int i = 0; i < 32; i += 2) {
+            float v0 = __uint_as_float(r[c][i]), v1 = __uint_as_float(r[c][i + 1]);
+            if (NEG) { v0 = -v0; v1 = -v1; }
+            if (MASK) {
+                if (c * 32 + i >= nv) v0 = -INFINITY;
+                if (c * 32 + i + 1 >= nv) v1 = -INFINITY;
+            }
+            a = fmaxf(a, fmaxf(v0, v1));
+        }
+        mx4[c] = a;
+    }
+    const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * fabsf(scale_log2);
+    const bool grow = mx > m_ref + LAZY_T;
+    const float m_new = grow ? mx : m_ref;
+    const float alpha = grow ? ptx::ex2(m_ref - m_new) : 1.f;
+    const float neg = -m_new;
+    float sum0 = 0.f, sum1 = 0.f;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        uint32_t pk[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const float x0 = fmaf(__uint_as_float(r[c][2 * i]), scale_log2, neg);
+            const float x1 = fmaf(__uint_as_float(r[c][2 * i + 1]), scale_log2, neg);
+            float p0 = ((2 * i) & 7) < SANGAM_POLY_EXP ? ex2_poly(x0) : ptx::ex2(x0);
+            float p1 = ((2 * i + 1) & 7) < SANGAM_POLY_EXP ? ex2_poly(x1) : ptx::ex2(x1);
+            if (MASK) {
+                if (c * 32 + 2 * i >= nv) p0 = 0.f;
+                if (c * 32 + 2 * i + 1 >= nv) p1 = 0.f;
+            }
+            sum0 += p0;
+            sum1 += p1;
+            pk[i] = ptx::pack_bf16(p0, p1);
+        }
+        ptx::tmem_st16(s_taddr + (uint32_t)(c * 16), pk);
+    }
+    l = l * alpha + (sum0 + sum1);
+    m_ref = m_new;
+    return alpha;
+}
+
+// out row (bf16) <- (w0 * O0 [+ w1 * O1]) scaled;  TMEM loads are warp-collective, stores predicated
+template <int D, bool TWO>
+__device__ __forceinline__ void store_final_row(uint32_t o0_taddr, uint32_t o1_taddr, float w0, float w1, bool row_ok, uint4* dst) {
+#pragma unroll
+    for (int c = 0; c < D / 32; ++c) {
+        uint32_t o[32], o1[32];
+        ptx::tmem_ld32(o0_taddr + (uint32_t)(c * 32), o);
+        if (TWO) ptx::tmem_ld32(o1_taddr + (uint32_t)(c * 32), o1);
+        ptx::tmem_wait_ld();
+        if (row_ok) {
+#pragma unroll
+            for (int v = 0; v < 4; ++v) {
+                float f[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    f[e] = __uint_as_float(o[v * 8 + e]) * w0;
+                    if (TWO) f[e] = fmaf(__uint_as_float(o1[v * 8 + e]), w1, f[e]);
+                }
+                uint4 w;
+                w.x = ptx::pack_bf16(f[0], f[1]); w.y = ptx::pack_bf16(f[2], f[3]);
+                w.z = ptx::pack_bf16(f[4], f[5]); w.w = ptx::pack_bf16(f[6], f[7]);
+                dst[c * 4 + v] = w;
+            }
+        }
+    }
+}
+// partial row (fp32, unnormalised) <- w0 * O0 [+ w1 * O1]
+template <int D, bool TWO>
+__device__ __forceinline__ void store_partial_row(uint32_t o0_taddr, uint32_t o1_taddr, float w0, float w1, bool row_ok, float* po) {
+#pragma unroll
+    for (int c = 0; c < D / 32; ++c) {
+        uint32_t o[32], o1[32];
+        ptx::tmem_ld32(o0_taddr + (uint32_t)(c * 32), o);
+        if (TWO) ptx::tmem_ld32(o1_taddr + (uint32_t)(c * 32), o1);
+        ptx::tmem_wait_ld();
+        if (row_ok) {
+#pragma unroll
+            for (int v = 0; v < 8; ++v) {
+                float f[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    f[e] = __uint_as_float(o[v * 4 + e]) * w0;
+                    if (TWO) f[e] = fmaf(__uint_as_float(o1[v * 4 + e]), w1, f[e]);
+                }
+                reinterpret_cast<float4*>(po)[c * 8 + v] = make_float4(f[0], f[1], f[2], f[3]);
+            }
+        }
+    }
+}
+
+template <int D>
+__device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, uint32_t sbase, uint32_t tmem,
+                                           const Item* items, volatile uint32_t* abort_flag, int s, int wg_warp, int lane) {
+    using L = Smem<D>;
+    const unsigned FULL = 0xffffffffu;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    const int row = wg_warp * 32 + lane;
+    const uint32_t lane_base = (uint32_t)(wg_warp * 32) << 16;
+    const uint32_t s_taddr = tmem + lane_base + (uint32_t)s * 128u;
+    const uint32_t o_taddr = tmem + lane_base + 256u + (uint32_t)s * 128u;     // own accumulator
+    const uint32_t o_other = tmem + lane_base + 256u + (uint32_t)(s ^ 1) * 128u;
+    float2* ml_x = reinterpret_cast<float2*>(smem + L::OFF_ML);
+    volatile int* last_flag = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 8);
+    uint32_t icount = 0, tcount = 0, ecount = 0, ccount = 0;
+    while (true) {
+        if (*abort_flag) break;
+        const uint32_t islot = icount & 1u;
+        ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
+        const Item it = items[islot];
+        if (!it.valid) break;
+        const bool shared = it.rows1 > 0;
+        const int n = it.kv1 - it.kv0;
+        const int ns = shared ? n : (s == 0 ? (n + 1) / 2 : n / 2);
+        const int rows_valid = (shared && s == 1) ? it.rows1 : it.rows0;
+        const bool warp_active = wg_warp * 32 < rows_valid;
+        float m = -INFINITY, l = 0.f;
+        for (int i = 0; i < ns; ++i) {
+            if (*abort_flag) break;
+            ptx::mbar_wait(bar(L::B_S_FULL + s), tcount & 1u, abort_flag);
+            ptx::tc_fence_after();
+            const int tile = shared ? it.kv0 + i : it.kv0 + 2 * i + s;
+            int nv = it.c - tile * BN;
+            nv = nv > BN ? BN : nv;
+            if (warp_active) {
+                float alpha;
+                if (p.scale_log2 >= 0.f) {
+                    if (nv == BN) alpha = softmax_tile<false, false>(s_taddr, nv, p.scale_log2, m, l);
+                    else alpha = softmax_tile<true, false>(s_taddr, nv, p.scale_log2, m, l);
+                } else {
+                    if (nv == BN) alpha = softmax_tile<false, true>(s_taddr, nv, p.scale_log2, m, l);
+                    else alpha = softmax_tile<true, true>(s_taddr, nv, p.scale_log2, m, l);
+                }
+                // S_FULL(i) was committed after PV(i-1) of this stream: O is quiescent here
+                if (i > 0 && __any_sync(FULL, alpha != 1.f)) {
 #pragma unroll
                     for (int c = 0; c < D / 32; ++c) {
                         uint32_t o[32];
                         ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
                         ptx::tmem_wait_ld();
 #pragma unroll
-                        for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                        for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
                         ptx::tmem_st32(o_taddr + (uint32_t)(c * 32), o);
                     }
                 }
+                ptx::tmem_wait_st();
             }
-            ptx::tmem_wait_st();
             ptx::tc_fence_before();
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL + sb));
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL + s));
             ++tcount;
         }
-        if (n > 0) {
-            ptx::mbar_wait(bar(L::B_PV_DONE), (tcount - 1u) & 1u, abort_flag);
+        if (ns > 0) {
+            ptx::mbar_wait(bar(L::B_PV_DONE + s), (tcount - 1u) & 1u, abort_flag);
             ptx::tc_fence_after();
         }
-        // ---- epilogue (TMEM loads are warp-collective: predicate only the global stores)
-        if (warp_active) {
-            const bool row_ok = row < it.rows_valid;
-            if (it.part_slot < 0) {
-                const float inv = (n > 0 && l > 0.f) ? 1.f / l : 0.f;
-                const int rg = it.row0 + row;
-                const int tl = rg / p.G, hh = rg - tl * p.G;
-                uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)(it.q_start + tl) * p.Hq + it.g * p.G + hh) * D);
+        // ---------------- epilogue
+        const bool row_ok = row < rows_valid;
+        const int rg = it.row0 + ((shared && s == 1) ? BM : 0) + row;
+        const int tl = rg / p.G, hh = rg - tl * p.G;
+        uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)(it.q_start + tl) * p.Hq + it.g * p.G + hh) * D);
+        const int prow = ((shared && s == 1) ? BM : 0) + row;                 // row inside the partial slot
+        float* po = p.part_o + ((int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * PAIR + prow) * D;
+        float2* pml = reinterpret_cast<float2*>(p.part_ml) + (int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * PAIR + prow;
+        if (n == 0) {
+            // empty context: zeros (reading S13); never split
+            if (row_ok && (shared || s == 0)) {
 #pragma unroll
-                for (int c = 0; c < D / 32; ++c) {
-                    uint32_t o[32];
-                    if (n > 0) {
-                        ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
-                        ptx::tmem_wait_ld();
+                for (int c = 0; c < D / 8; ++c) dst[c] = make_uint4(0, 0, 0, 0);
+            }
+        } else if (shared) {
+            if (warp_active) {
+                if (it.part_slot < 0) {
+                    store_final_row<D, false>(o_taddr, o_taddr, l > 0.f ? 1.f / l : 0.f, 0.f, row_ok, dst);
+                } else {
+                    store_partial_row<D, false>(o_taddr, o_taddr, 1.f, 0.f, row_ok, po);
+                    if (row_ok) *pml = make_float2(m, l);
+                }
+            }
+        } else {
+            // SPLIT: stream 1 hands (m, l) to stream 0, which merges O_0 and O_1
+            if (s == 1) {
+                ml_x[row] = make_float2(m, l);
+                ptx::mbar_arrive(bar(L::B_EPI_A));
+                ptx::mbar_wait(bar(L::B_EPI_B), ecount & 1u, abort_flag);       // stream 0 is done reading O_1
+            } else {
+                ptx::mbar_wait(bar(L::B_EPI_A), ecount & 1u, abort_flag);
+                const float2 x = ml_x[row];
+                const float ms = fmaxf(m, x.x);
+                const bool two = n > 1;                                    // stream 1 had tiles
+                const float w0 = ptx::ex2(m - ms), w1 = two ? ptx::ex2(x.x - ms) : 0.f;
+                const float ls = l * w0 + x.y * w1;
+                if (warp_active) {
+                    if (it.part_slot < 0) {
+                        const float inv = ls > 0.f ? 1.f / ls : 0.f;
+                        if (two) store_final_row<D, true>(o_taddr, o_other, w0 * inv, w1 * inv, row_ok, dst);
+                        else store_final_row<D, false>(o_taddr, o_taddr, w0 * inv, 0.f, row_ok, dst);
                     } else {
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) o[i] = 0u;
+                        if (two) store_partial_row<D, true>(o_taddr, o_other, w0, w1, row_ok, po);
+                        else store_partial_row<D, false>(o_taddr, o_taddr, w0, 0.f, row_ok, po);
+                        if (row_ok) *pml = make_float2(ms, ls);
                     }
-                    if (row_ok) {
+                }
+                ptx::tc_fence_before();
+                ptx::mbar_arrive(bar(L::B_EPI_B));
+            }
+            ++ecount;
+        }
+        // ---------------- fused split-KV merge across CTAs (a9): the CTA finishing a unit's last piece merges
+        if (it.part_slot >= 0) {
+            __threadfence();
+            ptx::mbar_arrive(bar(L::B_EPI_C));
+            ptx::mbar_wait(bar(L::B_EPI_C), ccount & 1u, abort_flag);
+            if (s == 0 && row == 0) {
+                __threadfence();
+                const int old = atomicAdd(p.unit_count + it.b_head, 1);
+                __threadfence();
+                const int last = old == it.npieces - 1;
+                if (last) { p.unit_count[it.b_head] = 0; __threadfence(); }     // re-armed for the next launch
+                *last_flag = last;
+                ptx::mbar_arrive(bar(L::B_EPI_D));
+            }
+            ptx::mbar_wait(bar(L::B_EPI_D), ccount & 1u, abort_flag);
+            const int last = *last_flag;
+            ++ccount;
+            if (last) {
+                // pieces in fixed order: head slot 2*b_head+1, then slots 2*b' of CTAs b' = b_head+1 ..; m in log2 units:
+                //   m* = max m_i;  l* = sum l_i 2^(m_i-m*);  O* = sum O_i 2^(m_i-m*);  out = bf16(O*/l*)
+                const int w8 = s * 4 + wg_warp, rows_u = it.rows0 + it.rows1, np = it.npieces;
+                const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
+                constexpr int EPL = D / 32;
+                for (int rr = w8; rr < rows_u; rr += 8) {
+                    float ms = -INFINITY;
+                    for (int base = 0; base < np; base += 32) {
+                        const int pi = base + lane;
+                        float mm = -INFINITY;
+                        if (pi < np) mm = __ldcg(&ml[(int64_t)(pi == 0 ? 2 * it.b_head + 1 : 2 * (it.b_head + pi)) * PAIR + rr].x);
 #pragma unroll
-                        for (int v = 0; v < 4; ++v) {
-                            uint4 w;
-                            w.x = ptx::pack_bf16(__uint_as_float(o[v * 8 + 0]) * inv, __uint_as_float(o[v * 8 + 1]) * inv);
-                            w.y = ptx::pack_bf16(__uint_as_float(o[v * 8 + 2]) * inv, __uint_as_float(o[v * 8 + 3]) * inv);
-                            w.z = ptx::pack_bf16(__uint_as_float(o[v * 8 + 4]) * inv, __uint_as_float(o[v * 8 + 5]) * inv);
-                            w.w = ptx::pack_bf16(__uint_as_float(o[v * 8 + 6]) * inv, __uint_as_float(o[v * 8 + 7]) * inv);
-                            dst[c * 4 + v] = w;
+                        for (int o = 16; o > 0; o >>= 1) mm = fmaxf(mm, __shfl_xor_sync(FULL, mm, o));
+                        ms = fmaxf(ms, mm);
+                    }
+                    float acc[EPL];
+#pragma unroll
+                    for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
+                    float ls = 0.f;
+#pragma unroll 4
+                    for (int pi = 0; pi < np; ++pi) {
+                        const int64_t slot = pi == 0 ? 2 * it.b_head + 1 : 2 * (it.b_head + pi);
+                        const float2 x = __ldcg(&ml[slot * PAIR + rr]);
+                        const float w = ptx::ex2(x.x - ms);
+                        ls = fmaf(x.y, w, ls);
+                        const float* src = p.part_o + (slot * PAIR + rr) * D + lane * EPL;
+                        if (EPL == 4) {
+                            const float4 o = __ldcg(reinterpret_cast<const float4*>(src));
+                            acc[0] = fmaf(o.x, w, acc[0]); acc[1] = fmaf(o.y, w, acc[1]);
+                            acc[2] = fmaf(o.z, w, acc[2]); acc[EPL - 1] = fmaf(o.w, w, acc[EPL - 1]);
+                        } else {
+                            const float2 o = __ldcg(reinterpret_cast<const float2*>(src));
+                            acc[0] = fmaf(o.x, w, acc[0]); acc[1] = fmaf(o.y, w, acc[1]);
                         }
                     }
-                }
-            } else {
-                float* po = p.part_o + ((int64_t)it.part_slot * BM + row) * D;
-#pragma unroll
-                for (int c = 0; c < D / 32; ++c) {
-                    uint32_t o[32];
-                    ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
-                    ptx::tmem_wait_ld();
-                    if (row_ok) {
-#pragma unroll
-                        for (int v = 0; v < 8; ++v)
-                            reinterpret_cast<uint4*>(po)[c * 8 + v] = make_uint4(o[v * 4], o[v * 4 + 1], o[v * 4 + 2], o[v * 4 + 3]);
+                    const float inv = ls > 0.f ? 1.f / ls : 0.f;
+                    const int rg2 = it.row0 + rr;
+                    const int tl2 = rg2 / p.G, hh2 = rg2 - tl2 * p.G;
+                    __nv_bfloat16* d2 = p.out + ((int64_t)(it.q_start + tl2) * p.Hq + it.g * p.G + hh2) * D + lane * EPL;
+                    if (EPL == 4) {
+                        uint2 w2;
+                        w2.x = ptx::pack_bf16(acc[0] * inv, acc[1] * inv);
+                        w2.y = ptx::pack_bf16(acc[2] * inv, acc[EPL - 1] * inv);
+                        *reinterpret_cast<uint2*>(d2) = w2;
+                    } else {
+                        *reinterpret_cast<uint32_t*>(d2) = ptx::pack_bf16(acc[0] * inv, acc[1] * inv);
                     }
                 }
-                if (row_ok) reinterpret_cast<float2*>(p.part_ml)[(int64_t)it.part_slot * BM + row] = make_float2(m, l);
             }
         }
         ptx::tc_fence_before();
@@ -551,7 +789,6 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         ++icount;
     }
 }
-
 
 // ------------------------------------------------------------------------------------------------
 // kernel entry
@@ -572,12 +809,17 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
         for (int s = 0; s < NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 1); }
         for (int s = 0; s < 2; ++s) {
             ptx::mbar_init(bar(L::B_ITEM_FULL + s), 1);
-            ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 5);   // MMA lane + 4 softmax warps
+            ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 11);  // MMA lane + 2 loader warps + 8 softmax warps
+            ptx::mbar_init(bar(L::B_Q_FULL + s), 2);       // the two loader warps
+            ptx::mbar_init(bar(L::B_Q_EMPTY + s), 1);
             ptx::mbar_init(bar(L::B_S_FULL + s), 1);
             ptx::mbar_init(bar(L::B_P_FULL + s), 4);
+            ptx::mbar_init(bar(L::B_PV_DONE + s), 1);
         }
-        ptx::mbar_init(bar(L::B_Q_FULL), 4);
-        ptx::mbar_init(bar(L::B_PV_DONE), 1);
+        ptx::mbar_init(bar(L::B_EPI_A), 128);
+        ptx::mbar_init(bar(L::B_EPI_B), 128);
+        ptx::mbar_init(bar(L::B_EPI_C), 256);
+        ptx::mbar_init(bar(L::B_EPI_D), 1);
         *abort_flag = 0u;
         ptx::fence_mbar_init();
         ptx::prefetch_tensormap(&mapK);
@@ -593,59 +835,18 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
     const uint32_t tmem = *tmem_slot;
 
     if (warp == 0) {
-        producer_warp<D>(p, reinterpret_cast<SlotMeta*>(p.slot_meta), &mapK, &mapV, sbase, items, abort_flag, lane);
+        producer_warp<D>(p, &mapK, &mapV, sbase, items, abort_flag, lane);
     } else if (warp == 1) {
         mma_warp<D>(p, sbase, tmem, items, abort_flag, lane);
-    } else if (warp >= 4) {
-        softmax_wg<D>(p, smem, sbase, tmem, items, abort_flag, warp - 4, lane);
+    } else if (warp < 4) {
+        qload_warps<D>(p, smem, sbase, items, abort_flag, tid - 64, lane);
+    } else {
+        softmax_wg<D>(p, smem, sbase, tmem, items, abort_flag, (warp - 4) >> 2, (warp - 4) & 3, lane);
     }
     ptx::tc_fence_before();
     __syncthreads();
     if (tid == 0 && *abort_flag) raise_flag(p.flags, DEV_TIMEOUT);
     if (warp == 2) ptx::tmem_dealloc(tmem, 512);
-}
-
-// ------------------------------------------------------------------------------------------------
-// combine (a9): merge the split-KV partials of one unit.  Block b owns the unit whose head piece
-// is in slot 2b+1; continuation pieces are slots 2b' of CTAs b' in (b, b_last].  Fixed order, no
-// atomics: bitwise reproducible.  m is in log2 units:
-//   m* = max m_i;  l* = sum l_i 2^(m_i-m*);  O* = sum O_i 2^(m_i-m*);  out = bf16(O*/l*)
-// ------------------------------------------------------------------------------------------------
-template <int D>
-__global__ void __launch_bounds__(256)
-combine_kernel(const AttnParams p) {
-    const SlotMeta* meta = reinterpret_cast<const SlotMeta*>(p.slot_meta);
-    const int b = blockIdx.x;
-    const SlotMeta h = meta[2 * b + 1];
-    if (!h.valid) return;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    constexpr int EPL = D / 32;
-    const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
-    for (int row = warp; row < h.rows_valid; row += 8) {
-        float ms = ml[(int64_t)(2 * b + 1) * BM + row].x;
-        for (int bb = b + 1; bb <= h.b_last; ++bb)
-            if (meta[2 * bb].valid) ms = fmaxf(ms, ml[(int64_t)(2 * bb) * BM + row].x);
-        float acc[EPL];
-#pragma unroll
-        for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
-        float ls = 0.f;
-        for (int bb = b; bb <= h.b_last; ++bb) {
-            const int slot = bb == b ? 2 * b + 1 : 2 * bb;
-            if (bb != b && !meta[slot].valid) continue;
-            const float2 x = ml[(int64_t)slot * BM + row];
-            const float w = ptx::ex2(x.x - ms);
-            ls += x.y * w;
-            const float* po = p.part_o + ((int64_t)slot * BM + row) * D + lane * EPL;
-#pragma unroll
-            for (int e = 0; e < EPL; ++e) acc[e] += po[e] * w;
-        }
-        const float inv = ls > 0.f ? 1.f / ls : 0.f;
-        const int rg = h.row0 + row;
-        const int tl = rg / p.G, hh = rg - tl * p.G;
-        __nv_bfloat16* dst = p.out + ((int64_t)(h.q_start + tl) * p.Hq + h.g * p.G + hh) * D + lane * EPL;
-#pragma unroll
-        for (int e = 0; e < EPL; ++e) dst[e] = __float2bfloat16(acc[e] * inv);
-    }
 }
 
 }  // namespace tc
@@ -689,14 +890,8 @@ static inline int tc_encode_maps(TcMaps* maps, const void* k_pages, const void* 
 
 static inline cudaError_t tc_launch(const AttnParams& p, const TcMaps& maps, int head_dim, int sm_count,
                                     cudaStream_t stream, int* launched) {
-    *launched = 0;
-    if (head_dim == 128) {
-        tc::attn_kernel<128><<<sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream>>>(maps.k, maps.v, p);
-        tc::combine_kernel<128><<<sm_count, 256, 0, stream>>>(p);
-    } else {
-        tc::attn_kernel<64><<<sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream>>>(maps.k, maps.v, p);
-        tc::combine_kernel<64><<<sm_count, 256, 0, stream>>>(p);
-    }
-    *launched = 2;
+    if (head_dim == 128) tc::attn_kernel<128><<<sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream>>>(maps.k, maps.v, p);
+    else tc::attn_kernel<64><<<sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream>>>(maps.k, maps.v, p);
+    *launched = 1;
     return cudaGetLastError();
 }

@@ -26,10 +26,10 @@ struct AttnParams {
     float scale;                   // natural-base logit scale
     float scale_log2;              // scale * log2(e)
     // split-KV workspace (library owned)
-    float* part_o;                 // [num_slots][128][D]  unnormalised partial sums
-    float* part_ml;                // [num_slots][128][2]  (m in log2 units, l)
+    float* part_o;                 // [num_slots][256][D]  unnormalised partial sums
+    float* part_ml;                // [num_slots][256][2]  (m in log2 units, l)
     int32_t num_slots;
-    void* slot_meta;               // [num_slots] tc::SlotMeta, rewritten every launch
+    int32_t* unit_count;           // [num_ctas] pieces of a split unit finished so far (self-resetting)
     uint32_t* flags;               // sticky device flags
     int32_t* sched;                // [0] dynamic work counter (self-resetting), [1] finished-CTA count
 };
