@@ -1,14 +1,14 @@
 // attn_tc.cuh -- steps a3..a9: paged, varlen, non-causal block attention on tcgen05 (sm_100a).
 //
 // One persistent CTA per SM, 12 warps, warp-specialised, TWO softmax streams per CTA:
-//   warp 0      scheduler + TMA producer: plans the work on the device (a3) and gathers K/V pages of
+//   warp 10     scheduler + TMA producer: plans the work on the device (a3) and gathers K/V pages of
 //               the current (request, kv head) through the block table with TMA into a ring of
 //               128-row, 128B-swizzled shared-memory tiles (a4)
-//   warp 1      MMA issuer: S_s = Q_s K^T (tcgen05.mma, operands in smem, S in TMEM; a5) and
+//   warp 11     MMA issuer: S_s = Q_s K^T (tcgen05.mma, operands in smem, S in TMEM; a5) and
 //               O_s += P_s V (P read from TMEM, V from smem, O in TMEM; a7) for streams s = 0, 1
-//   warps 2-3   Q loader: packed (query row, q head of the group) rows -> swizzled smem, 2-slot ring
-//               (warp 2 also owns the TMEM allocation)
-//   warps 4-7   softmax warpgroup of stream 0;  warps 8-11: stream 1.  Thread i owns row i of the
+//   warps 8-9   Q loader: packed (query row, q head of the group) rows -> swizzled smem, 2-slot ring
+//               (warp 8 also owns the TMEM allocation)
+//   warps 0-3   softmax warpgroup of stream 0;  warps 4-7: stream 1.  Thread i owns row i of the
 //               stream's tile (TMEM lane i): online softmax in fp32 with a lazily updated reference
 //               maximum (a6), P written back over S as bf16, epilogue (a8), fused split-KV merge (a9)
 // Work unit = (request r, kv head g, PAIR of 128-row tiles of the packed rows).  Two modes per unit:
@@ -141,7 +141,7 @@ struct OpWalk {
 };
 
 // ------------------------------------------------------------------------------------------------
-// warp 0: device-side plan (a3) + TMA page gather (a4)
+// warp 10: device-side plan (a3) + TMA page gather (a4)
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtensorMap* mapK, const CUtensorMap* mapV,
@@ -317,7 +317,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
 }
 
 // ------------------------------------------------------------------------------------------------
-// warps 2-3: Q loader.  Packed row rg of the (r, g) group = (token rg / G, q head g*G + rg % G).
+// warps 8-9: Q loader.  Packed row rg of the (r, g) group = (token rg / G, q head g*G + rg % G).
 // Rows go to a 2-slot ring of 128-row tiles in the K-major 128B-swizzled UMMA layout.
 // ------------------------------------------------------------------------------------------------
 template <int D>
@@ -374,7 +374,7 @@ __device__ __forceinline__ void qload_warps(const AttnParams& p, uint8_t* smem, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// warp 1: MMA issuer (a5, a7).  TMEM columns: S_s = [128 s, 128 s + 128), O_s = [256 + 128 s, .. + D).
+// warp 11: MMA issuer (a5, a7).  TMEM columns: S_s = [128 s, 128 s + 128), O_s = [256 + 128 s, .. + D).
 // P_s (bf16, two per column) overwrites the first 64 columns of S_s.
 // ------------------------------------------------------------------------------------------------
 template <int D>
@@ -382,6 +382,9 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
                                          volatile uint32_t* abort_flag, int lane) {
     using L = Smem<D>;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    const uint64_t q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);        // K-major operands (Q, K)
+    const uint64_t kv_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, 1024);
+    const uint64_t v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, SLAB, 1024);     // MN-major operand (V)
     uint32_t kvi = 0, icount = 0, qcount = 0;
     uint32_t pv_cnt0 = 0u, pv_cnt1 = 0u;
     while (true) {
@@ -417,16 +420,14 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
                     const uint32_t qs = (qcount + (shared ? (uint32_t)op.s : 0u)) & 1u;
                     const bool last_qk = shared ? (op.i == n0 - 1)
                                                 : ((op.s == 0 && op.i == n0 - 1 && n0 > n1) || (op.s == 1 && op.i == n1 - 1 && n1 == n0));
-                    if (lane == 0) {
-                        const uint32_t q_addr = sbase + (uint32_t)(L::OFF_Q + qs * L::Q_BYTES);
-                        const uint32_t k_addr = sbase + (uint32_t)(L::OFF_KV + stage_k * L::KV_BYTES);
+                    if (ptx::elect_one()) {
+                        const uint64_t a_desc = q_desc0 + (uint64_t)(qs * (L::Q_BYTES >> 4));
+                        const uint64_t b_desc = kv_desc0 + (uint64_t)(stage_k * (L::KV_BYTES >> 4));
                         const uint32_t idesc = ptx::idesc_bf16(BM, (uint32_t)ncols, 0, 0);
-#pragma unroll
-                        for (int ks = 0; ks < D / 16; ++ks) {
-                            const uint32_t off = (uint32_t)((ks >> 2) * SLAB + (ks & 3) * 32);
-                            ptx::mma_ss(tmem + (uint32_t)op.s * 128u, ptx::smem_desc_sw128(q_addr + off, 16, 1024),
-                                        ptx::smem_desc_sw128(k_addr + off, 16, 1024), idesc, ks > 0);
-                        }
+                        const uint32_t d_tmem = tmem + (uint32_t)op.s * 128u;
+                        // K-steps of 16 elements = 32 bytes inside a 64-wide slab; second slab SLAB bytes further
+                        ptx::mma_ss_x4(d_tmem, a_desc, b_desc, idesc, 0u, 2u);
+                        if (D == 128) ptx::mma_ss_x4(d_tmem, a_desc + (SLAB >> 4), b_desc + (SLAB >> 4), idesc, 1u, 2u);
                         if (op.release) ptx::mma_commit(bar(L::B_KV_EMPTY + stage_k));
                         ptx::mma_commit(bar(L::B_S_FULL + op.s));
                         if (last_qk) ptx::mma_commit(bar(L::B_Q_EMPTY + qs));
@@ -454,13 +455,17 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
                     }
                     ptx::mbar_wait(bar(L::B_P_FULL + op.s), (op.s ? pv_cnt1 : pv_cnt0) & 1u, abort_flag);
                     ptx::tc_fence_after();
-                    if (lane == 0) {
-                        const uint32_t v_addr = sbase + (uint32_t)(L::OFF_KV + stage_v * L::KV_BYTES);
+                    if (ptx::elect_one()) {
+                        const uint64_t b_desc = v_desc0 + (uint64_t)(stage_v * (L::KV_BYTES >> 4));
                         const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
-                        const int nk = ncols / 16;
-                        for (int ks = 0; ks < nk; ++ks)
-                            ptx::mma_ts(tmem + 256u + (uint32_t)op.s * 128u, tmem + (uint32_t)op.s * 128u + (uint32_t)(ks * 8),
-                                        ptx::smem_desc_sw128(v_addr + (uint32_t)(ks * 2048), SLAB, 1024), idesc,
+                        const uint32_t d_tmem = tmem + 256u + (uint32_t)op.s * 128u, a_tmem = tmem + (uint32_t)op.s * 128u;
+                        const int nk = ncols / 16;                       // K-steps of 16 kv rows = 2048 bytes of V
+                        int ks = 0;
+                        for (; ks + 4 <= nk; ks += 4)
+                            ptx::mma_ts_x4(d_tmem, a_tmem + (uint32_t)(ks * 8), b_desc + (uint64_t)(ks * 128), idesc,
+                                           (op.i > 0 || ks > 0) ? 1u : 0u, 128u);
+                        for (; ks < nk; ++ks)
+                            ptx::mma_ts(d_tmem, a_tmem + (uint32_t)(ks * 8), b_desc + (uint64_t)(ks * 128), idesc,
                                         (op.i > 0 || ks > 0) ? 1u : 0u);
                         if (op.release) ptx::mma_commit(bar(L::B_KV_EMPTY + stage_v));
                         ptx::mma_commit(bar(L::B_PV_DONE + op.s));
@@ -478,7 +483,7 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
 }
 
 // ------------------------------------------------------------------------------------------------
-// warps 4-11: softmax warpgroups (a6) + epilogue (a8) + fused split-KV merge (a9).
+// warps 0-7: softmax warpgroups (a6) + epilogue (a8) + fused split-KV merge (a9).
 // Thread `row` of stream s owns TMEM lane `row` of S_s / O_s.
 // ------------------------------------------------------------------------------------------------
 // 2^x on the FMA pipe (Cody-Waite split + degree-3 minimax on [-0.5, 0.5], rel. error 7.6e-5 --
@@ -825,7 +830,7 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
         ptx::prefetch_tensormap(&mapK);
         ptx::prefetch_tensormap(&mapV);
     }
-    if (warp == 2) {
+    if (warp == 8) {
         ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
         ptx::tmem_relinquish();
     }
@@ -834,19 +839,22 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
 
-    if (warp == 0) {
-        producer_warp<D>(p, &mapK, &mapV, sbase, items, abort_flag, lane);
-    } else if (warp == 1) {
-        mma_warp<D>(p, sbase, tmem, items, abort_flag, lane);
-    } else if (warp < 4) {
-        qload_warps<D>(p, smem, sbase, items, abort_flag, tid - 64, lane);
+    // Warpgroups 0 and 1 are the softmax streams (TMEM lane quarter = warp % 4); warpgroup 2 holds the
+    // service warps.  The MMA issuer is the highest warp id: the SM sub-partition arbiter favours it over
+    // the softmax warps it shares a scheduler with, so a tile's MMAs are issued the moment P is ready.
+    if (warp < 8) {
+        ptx::setmaxnreg_inc<208>();   // 8*32*208 + 4*32*80 <= 384*168: the pool is what the CTA got at launch
+        softmax_wg<D>(p, smem, sbase, tmem, items, abort_flag, warp >> 2, warp & 3, lane);
     } else {
-        softmax_wg<D>(p, smem, sbase, tmem, items, abort_flag, (warp - 4) >> 2, (warp - 4) & 3, lane);
+        ptx::setmaxnreg_dec<80>();
+        if (warp == 10) producer_warp<D>(p, &mapK, &mapV, sbase, items, abort_flag, lane);
+        else if (warp == 11) mma_warp<D>(p, sbase, tmem, items, abort_flag, lane);
+        else qload_warps<D>(p, smem, sbase, items, abort_flag, tid - 256, lane);
     }
     ptx::tc_fence_before();
     __syncthreads();
     if (tid == 0 && *abort_flag) raise_flag(p.flags, DEV_TIMEOUT);
-    if (warp == 2) ptx::tmem_dealloc(tmem, 512);
+    if (warp == 8) ptx::tmem_dealloc(tmem, 512);
 }
 
 }  // namespace tc
