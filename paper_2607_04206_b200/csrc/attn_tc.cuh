@@ -375,106 +375,152 @@ __device__ __forceinline__ void qload_warps(const AttnParams& p, uint8_t* smem, 
 
 // ------------------------------------------------------------------------------------------------
 // warp 11: MMA issuer (a5, a7).  TMEM columns: S_s = [128 s, 128 s + 128), O_s = [256 + 128 s, .. + D).
-// P_s (bf16, two per column) overwrites the first 64 columns of S_s.
+// P_s (bf16, two per column) overwrites the first 64 columns of S_s.  Issue order per item (OpWalk):
+//   QK(0,0) QK(1,0) | PV(0,j) QK(0,j+1) PV(1,j) QK(1,j+1) | ...
+// This warp is the pacemaker of the CTA: the per-op path is kept to a few dozen instructions.
 // ------------------------------------------------------------------------------------------------
+template <int D>
+struct MmaState {
+    uint32_t sbase, tmem;
+    uint64_t q_desc0, k_desc0, v_desc0;
+    uint32_t stage, phase;            // next ring stage to acquire and its parity
+    uint32_t stage_k, stage_v;        // stages currently held
+    uint32_t pv_par0, pv_par1;        // parity of the next P_FULL wait per stream
+    volatile uint32_t* abort_flag;
+};
+
+template <int D>
+__device__ __forceinline__ uint32_t mma_acquire(MmaState<D>& st) {
+    using L = Smem<D>;
+    const uint32_t stage = st.stage;
+    ptx::mbar_wait(st.sbase + (uint32_t)(L::OFF_BAR + (L::B_KV_FULL + stage) * 8), st.phase, st.abort_flag);
+    if (++st.stage == NSTAGE) { st.stage = 0; st.phase ^= 1u; }
+    return stage;
+}
+
+// S_s = Q K^T for kv tile `tile`
+template <int D>
+__device__ __forceinline__ void mma_qk(MmaState<D>& st, int s, int c, int tile, uint32_t qs, bool acquire, bool release, bool last_qk) {
+    using L = Smem<D>;
+    if (acquire) st.stage_k = mma_acquire<D>(st);
+    ptx::tc_fence_after();
+    int nv = c - tile * BN;
+    nv = nv > BN ? BN : nv;
+    const uint32_t ncols = (uint32_t)((nv + 15) & ~15);
+    if (ptx::elect_one()) {
+        const uint32_t bar0 = st.sbase + (uint32_t)L::OFF_BAR;
+        const uint64_t a_desc = st.q_desc0 + (uint64_t)(qs * (L::Q_BYTES >> 4));
+        const uint64_t b_desc = st.k_desc0 + (uint64_t)(st.stage_k * (L::KV_BYTES >> 4));
+        const uint32_t idesc = ptx::idesc_bf16(BM, ncols, 0, 0);
+        const uint32_t d_tmem = st.tmem + (uint32_t)s * 128u;
+        // K-steps of 16 elements = 32 bytes inside a 64-wide slab; the second slab is SLAB bytes further
+        ptx::mma_ss_x4(d_tmem, a_desc, b_desc, idesc, 0u, 2u);
+        if (D == 128) ptx::mma_ss_x4(d_tmem, a_desc + (SLAB >> 4), b_desc + (SLAB >> 4), idesc, 1u, 2u);
+        if (release) ptx::mma_commit(bar0 + (uint32_t)((L::B_KV_EMPTY + st.stage_k) * 8));
+        ptx::mma_commit(bar0 + (uint32_t)((L::B_S_FULL + s) * 8));
+        if (last_qk) ptx::mma_commit(bar0 + (uint32_t)((L::B_Q_EMPTY + qs) * 8));
+    }
+    __syncwarp();
+}
+
+// O_s (+)= P_s V for kv tile `tile`; `first` overwrites the accumulator
+template <int D>
+__device__ __forceinline__ void mma_pv(MmaState<D>& st, int s, int c, int tile, bool first, bool acquire, bool release, int lane) {
+    using L = Smem<D>;
+    int nv = c - tile * BN;
+    nv = nv > BN ? BN : nv;
+    const int ncols = (nv + 15) & ~15;
+    if (acquire) {
+        st.stage_v = mma_acquire<D>(st);
+        if (nv < ncols) {
+            // stale rows of the last page: zero them so that P = 0 meets V = 0, never NaN (reading S12)
+            const uint32_t v_addr = st.sbase + (uint32_t)(L::OFF_KV + st.stage_v * L::KV_BYTES);
+            const int nrows = ncols - nv;
+            for (int e = lane; e < nrows * 8 * (D / 64); e += 32) {
+                const int chunk = e & 7, rr = (e >> 3) % nrows, slab = (e >> 3) / nrows;
+                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(
+                                 v_addr + (uint32_t)(slab * SLAB + (nv + rr) * 128 + chunk * 16)),
+                             "r"(0)
+                             : "memory");
+            }
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+        }
+    }
+    uint32_t& par = s ? st.pv_par1 : st.pv_par0;
+    ptx::mbar_wait(st.sbase + (uint32_t)(L::OFF_BAR + (L::B_P_FULL + s) * 8), par, st.abort_flag);
+    par ^= 1u;
+    ptx::tc_fence_after();
+    if (ptx::elect_one()) {
+        const uint32_t bar0 = st.sbase + (uint32_t)L::OFF_BAR;
+        const uint64_t b_desc = st.v_desc0 + (uint64_t)(st.stage_v * (L::KV_BYTES >> 4));
+        const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
+        const uint32_t d_tmem = st.tmem + 256u + (uint32_t)s * 128u, a_tmem = st.tmem + (uint32_t)s * 128u;
+        if (ncols == BN) {                                    // K-steps of 16 kv rows = 2048 bytes of V
+            ptx::mma_ts_x4(d_tmem, a_tmem, b_desc, idesc, first ? 0u : 1u, 128u);
+            ptx::mma_ts_x4(d_tmem, a_tmem + 32u, b_desc + 512u, idesc, 1u, 128u);
+        } else {
+            for (int ks = 0; ks < ncols / 16; ++ks)
+                ptx::mma_ts(d_tmem, a_tmem + (uint32_t)(ks * 8), b_desc + (uint64_t)(ks * 128), idesc, (!first || ks > 0) ? 1u : 0u);
+        }
+        if (release) ptx::mma_commit(bar0 + (uint32_t)((L::B_KV_EMPTY + st.stage_v) * 8));
+        ptx::mma_commit(bar0 + (uint32_t)((L::B_PV_DONE + s) * 8));
+    }
+    __syncwarp();
+}
+
 template <int D>
 __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, uint32_t tmem, const Item* items,
                                          volatile uint32_t* abort_flag, int lane) {
     using L = Smem<D>;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
-    const uint64_t q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);        // K-major operands (Q, K)
-    const uint64_t kv_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, 1024);
-    const uint64_t v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, SLAB, 1024);     // MN-major operand (V)
-    uint32_t kvi = 0, icount = 0, qcount = 0;
-    uint32_t pv_cnt0 = 0u, pv_cnt1 = 0u;
+    MmaState<D> st;
+    st.sbase = sbase; st.tmem = tmem; st.abort_flag = abort_flag;
+    st.q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);        // K-major operands (Q, K)
+    st.k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, 1024);
+    st.v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, SLAB, 1024);     // MN-major operand (V)
+    st.stage = 0; st.phase = 0; st.stage_k = 0; st.stage_v = 0; st.pv_par0 = 0; st.pv_par1 = 0;
+    uint32_t icount = 0, qcount = 0;
     while (true) {
         if (*abort_flag) break;
         const uint32_t islot = icount & 1u;
         ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
         const Item it = items[islot];
         if (!it.valid) break;
-        const int n = it.kv1 - it.kv0;
-        const int shared = it.rows1 > 0;
-        const int nq = shared ? 2 : 1;
+        const int n = it.kv1 - it.kv0, c = it.c, kv0 = it.kv0;
         if (n > 0) {
-            // q tiles of this item: ring slots (qcount + t) & 1
-            for (int t = 0; t < nq; ++t)
-                ptx::mbar_wait(bar(L::B_Q_FULL + ((qcount + t) & 1u)), ((qcount + t) >> 1) & 1u, abort_flag);
-            ptx::tc_fence_after();
-            OpWalk walk(it);
-            const int n0 = walk.n0, n1 = walk.n1;
-            Op op;
-            uint32_t stage_k = 0, stage_v = 0;
-            while (walk.next(op)) {
-                if (*abort_flag) break;
-                int nv = it.c - op.tile * BN;
-                nv = nv > BN ? BN : nv;
-                const int ncols = (nv + 15) & ~15;
-                if (!op.is_pv) {
-                    if (op.acquire) {
-                        stage_k = kvi % NSTAGE;
-                        ptx::mbar_wait(bar(L::B_KV_FULL + stage_k), (kvi / NSTAGE) & 1u, abort_flag);
-                        ptx::tc_fence_after();
-                        ++kvi;
-                    }
-                    const uint32_t qs = (qcount + (shared ? (uint32_t)op.s : 0u)) & 1u;
-                    const bool last_qk = shared ? (op.i == n0 - 1)
-                                                : ((op.s == 0 && op.i == n0 - 1 && n0 > n1) || (op.s == 1 && op.i == n1 - 1 && n1 == n0));
-                    if (ptx::elect_one()) {
-                        const uint64_t a_desc = q_desc0 + (uint64_t)(qs * (L::Q_BYTES >> 4));
-                        const uint64_t b_desc = kv_desc0 + (uint64_t)(stage_k * (L::KV_BYTES >> 4));
-                        const uint32_t idesc = ptx::idesc_bf16(BM, (uint32_t)ncols, 0, 0);
-                        const uint32_t d_tmem = tmem + (uint32_t)op.s * 128u;
-                        // K-steps of 16 elements = 32 bytes inside a 64-wide slab; second slab SLAB bytes further
-                        ptx::mma_ss_x4(d_tmem, a_desc, b_desc, idesc, 0u, 2u);
-                        if (D == 128) ptx::mma_ss_x4(d_tmem, a_desc + (SLAB >> 4), b_desc + (SLAB >> 4), idesc, 1u, 2u);
-                        if (op.release) ptx::mma_commit(bar(L::B_KV_EMPTY + stage_k));
-                        ptx::mma_commit(bar(L::B_S_FULL + op.s));
-                        if (last_qk) ptx::mma_commit(bar(L::B_Q_EMPTY + qs));
-                    }
-                    __syncwarp();
-                } else {
-                    if (op.acquire) {
-                        stage_v = kvi % NSTAGE;
-                        ptx::mbar_wait(bar(L::B_KV_FULL + stage_v), (kvi / NSTAGE) & 1u, abort_flag);
-                        ++kvi;
-                        if (nv < ncols) {
-                            // stale rows of the last page: zero them so that P = 0 meets V = 0, never NaN (reading S12)
-                            const uint32_t v_addr = sbase + (uint32_t)(L::OFF_KV + stage_v * L::KV_BYTES);
-                            const int nrows = ncols - nv;
-                            for (int e = lane; e < nrows * 8 * (D / 64); e += 32) {
-                                const int chunk = e & 7, rr = (e >> 3) % nrows, slab = (e >> 3) / nrows;
-                                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(
-                                                 v_addr + (uint32_t)(slab * SLAB + (nv + rr) * 128 + chunk * 16)),
-                                             "r"(0)
-                                             : "memory");
-                            }
-                            ptx::fence_proxy_async_smem();
-                            __syncwarp();
-                        }
-                    }
-                    ptx::mbar_wait(bar(L::B_P_FULL + op.s), (op.s ? pv_cnt1 : pv_cnt0) & 1u, abort_flag);
-                    ptx::tc_fence_after();
-                    if (ptx::elect_one()) {
-                        const uint64_t b_desc = v_desc0 + (uint64_t)(stage_v * (L::KV_BYTES >> 4));
-                        const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
-                        const uint32_t d_tmem = tmem + 256u + (uint32_t)op.s * 128u, a_tmem = tmem + (uint32_t)op.s * 128u;
-                        const int nk = ncols / 16;                       // K-steps of 16 kv rows = 2048 bytes of V
-                        int ks = 0;
-                        for (; ks + 4 <= nk; ks += 4)
-                            ptx::mma_ts_x4(d_tmem, a_tmem + (uint32_t)(ks * 8), b_desc + (uint64_t)(ks * 128), idesc,
-                                           (op.i > 0 || ks > 0) ? 1u : 0u, 128u);
-                        for (; ks < nk; ++ks)
-                            ptx::mma_ts(d_tmem, a_tmem + (uint32_t)(ks * 8), b_desc + (uint64_t)(ks * 128), idesc,
-                                        (op.i > 0 || ks > 0) ? 1u : 0u);
-                        if (op.release) ptx::mma_commit(bar(L::B_KV_EMPTY + stage_v));
-                        ptx::mma_commit(bar(L::B_PV_DONE + op.s));
-                    }
-                    __syncwarp();
-                    if (op.s) ++pv_cnt1; else ++pv_cnt0;
+            if (it.rows1 > 0) {
+                // SHARED: stream s = q tile s; both streams read the same K/V stage (stream 0 acquires, stream 1 releases)
+                const uint32_t qs0 = qcount & 1u, qs1 = qs0 ^ 1u;
+                ptx::mbar_wait(bar(L::B_Q_FULL + qs0), (qcount >> 1) & 1u, abort_flag);
+                mma_qk<D>(st, 0, c, kv0, qs0, true, false, n == 1);
+                ptx::mbar_wait(bar(L::B_Q_FULL + qs1), ((qcount + 1) >> 1) & 1u, abort_flag);
+                mma_qk<D>(st, 1, c, kv0, qs1, false, true, n == 1);
+                for (int j = 0; j < n; ++j) {
+                    const bool more = j + 1 < n, lastq = j + 2 == n;
+                    mma_pv<D>(st, 0, c, kv0 + j, j == 0, true, false, lane);
+                    if (more) mma_qk<D>(st, 0, c, kv0 + j + 1, qs0, true, false, lastq);
+                    mma_pv<D>(st, 1, c, kv0 + j, j == 0, false, true, lane);
+                    if (more) mma_qk<D>(st, 1, c, kv0 + j + 1, qs1, false, true, lastq);
                 }
+                qcount += 2;
+            } else {
+                // SPLIT: one q tile; stream s takes kv tiles kv0 + 2i + s, every op has its own stage
+                const uint32_t qs = qcount & 1u;
+                const int n0 = (n + 1) >> 1, n1 = n >> 1;
+                ptx::mbar_wait(bar(L::B_Q_FULL + qs), (qcount >> 1) & 1u, abort_flag);
+                mma_qk<D>(st, 0, c, kv0, qs, true, true, n == 1);
+                if (n1 > 0) mma_qk<D>(st, 1, c, kv0 + 1, qs, true, true, n == 2);
+                for (int i = 0; i < n0; ++i) {
+                    mma_pv<D>(st, 0, c, kv0 + 2 * i, i == 0, true, true, lane);
+                    if (i + 1 < n0) mma_qk<D>(st, 0, c, kv0 + 2 * i + 2, qs, true, true, 2 * i + 3 == n);
+                    if (i < n1) {
+                        mma_pv<D>(st, 1, c, kv0 + 2 * i + 1, i == 0, true, true, lane);
+                        if (i + 1 < n1) mma_qk<D>(st, 1, c, kv0 + 2 * i + 3, qs, true, true, 2 * i + 4 == n);
+                    }
+                }
+                qcount += 1;
             }
-            qcount += nq;
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));

@@ -68,8 +68,8 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
 #ifndef SANGAM_WAIT_TIMEOUT_NS
 #define SANGAM_WAIT_TIMEOUT_NS 2000000000ull
 #endif
-__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile uint32_t* abort_flag) {
-    if (mbar_try_wait(bar, parity)) return true;
+__device__ __forceinline__ bool mbar_wait_slow(uint32_t bar, uint32_t parity, volatile uint32_t* abort_flag) {
+    if (*abort_flag) return false;
     uint64_t t0 = 0;
     uint32_t spins = 0;
     while (true) {
@@ -81,6 +81,11 @@ __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatil
             else if (now - t0 > SANGAM_WAIT_TIMEOUT_NS) { *abort_flag = 1u; return false; }
         }
     }
+}
+// hot path: one try_wait; everything else (suspending wait, abort flag, timeout) is out of line
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile uint32_t* abort_flag) {
+    if (mbar_try_wait(bar, parity)) return true;
+    return mbar_wait_slow(bar, parity, abort_flag);
 }
 
 __device__ __forceinline__ void fence_proxy_async_smem() {
