@@ -1,13 +1,12 @@
 // attn_tc.cuh -- steps a3..a9: paged, varlen, non-causal block attention on tcgen05 (sm_100a).
 //
 // One persistent CTA per SM, 12 warps, warp-specialised, TWO softmax streams per CTA:
-//   warp 10     scheduler + TMA producer: plans the work on the device (a3) and gathers K/V pages of
+//   warp 8      scheduler + TMA producer: plans the work on the device (a3) and gathers K/V pages of
 //               the current (request, kv head) through the block table with TMA into a ring of
-//               128-row, 128B-swizzled shared-memory tiles (a4)
-//   warp 11     MMA issuer: S_s = Q_s K^T (tcgen05.mma, operands in smem, S in TMEM; a5) and
-//               O_s += P_s V (P read from TMEM, V from smem, O in TMEM; a7) for streams s = 0, 1
-//   warps 8-9   Q loader: packed (query row, q head of the group) rows -> swizzled smem, 2-slot ring
-//               (warp 8 also owns the TMEM allocation)
+//               128-row, 128B-swizzled shared-memory tiles (a4); also owns the TMEM allocation
+//   warp 9      Q loader: packed (query row, q head of the group) rows -> swizzled smem, 2-slot ring
+//   warps 10,11 MMA issuers, one per stream s: S_s = Q_s K^T (tcgen05.mma, operands in smem, S in
+//               TMEM; a5) and O_s += P_s V (P read from TMEM, V from smem, O in TMEM; a7)
 //   warps 0-3   softmax warpgroup of stream 0;  warps 4-7: stream 1.  Thread i owns row i of the
 //               stream's tile (TMEM lane i): online softmax in fp32 with a lazily updated reference
 //               maximum (a6), P written back over S as bf16, epilogue (a8), fused split-KV merge (a9)
@@ -29,7 +28,7 @@
 #include "ptx.cuh"
 
 struct TcMaps {
-    CUtensorMap k, v;
+    CUtensorMap k, v, q;
 };
 
 namespace tc {
@@ -49,8 +48,8 @@ constexpr float LAZY_T = 8.f;    // the reference maximum moves only when a tile
 struct Item {          // one piece of work, published through shared memory (64 bytes)
     int valid;         // 0 = no more work
     int r, g;
-    int row0;          // first packed row of the pair inside the (r, g) group
-    int rows0, rows1;  // rows of q tile 0 / 1 that exist; rows1 > 0 <=> SHARED mode
+    int tok0;          // first query token (inside the request) of the pair of q tiles
+    int rows0, rows1;  // rows (tokens * G) of q tile 0 / 1 that exist; rows1 > 0 <=> SHARED mode
     int q_start;       // cu_q_lens[r]
     int c;             // context length
     int kv0, kv1;      // kv tile range [kv0, kv1)
@@ -71,7 +70,7 @@ struct Smem {
     static constexpr int B_KV_FULL = 0, B_KV_EMPTY = NSTAGE, B_ITEM_FULL = 2 * NSTAGE, B_ITEM_EMPTY = B_ITEM_FULL + 2,
                          B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 2, B_S_FULL = B_Q_EMPTY + 2,
                          B_P_FULL = B_S_FULL + 2, B_PV_DONE = B_P_FULL + 2, B_EPI_A = B_PV_DONE + 2,
-                         B_EPI_B = B_EPI_A + 1, B_EPI_C = B_EPI_B + 1, B_EPI_D = B_EPI_C + 1, NBAR = B_EPI_D + 1;
+                         B_EPI_B = B_EPI_A + 1, B_EPI_C = B_EPI_B + 1, B_EPI_D = B_EPI_C + 1, B_ZFILL = B_EPI_D + 1, NBAR = B_ZFILL + 1;
     static constexpr int OFF_ITEMS = OFF_BAR + ((NBAR * 8 + 15) / 16) * 16;
     static constexpr int OFF_ML = OFF_ITEMS + 2 * (int)sizeof(Item);    // (m, l) of stream 1, 128 rows
     static constexpr int OFF_MISC = OFF_ML + BM * 8;
@@ -82,7 +81,7 @@ static_assert(sizeof(Item) == 64, "Item is 64 bytes");
 static_assert(Smem<128>::ALLOC <= 232448, "shared memory budget (227 KB)");
 
 struct ReqInfo {
-    int q0, c, np, tiles_u, units, rows;
+    int q0, qn, c, np, tiles_u, units;
 };
 
 __device__ __forceinline__ ReqInfo req_info(const AttnParams& p, int r) {
@@ -94,8 +93,8 @@ __device__ __forceinline__ ReqInfo req_info(const AttnParams& p, int r) {
     if (c < 0) c = 0;
     if ((c + SANGAM_PAGE - 1) / SANGAM_PAGE > p.W) { raise_flag(p.flags, DEV_CTX_TOO_LONG); c = 0; }
     x.c = c;
-    x.rows = qn * p.G;
-    x.np = (x.rows + PAIR - 1) / PAIR;
+    x.qn = qn;
+    x.np = (qn + 2 * p.tpt - 1) / (2 * p.tpt);      // a q tile holds tpt = 128 / G whole tokens (all G heads of each)
     const int nkv = (c + BN - 1) / BN;
     x.tiles_u = nkv > 0 ? nkv : 1;
     x.units = p.Hkv * x.np;
@@ -141,7 +140,7 @@ struct OpWalk {
 };
 
 // ------------------------------------------------------------------------------------------------
-// warp 10: device-side plan (a3) + TMA page gather (a4)
+// warp 8: device-side plan (a3) + TMA page gather (a4)
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtensorMap* mapK, const CUtensorMap* mapV,
@@ -168,7 +167,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
     // walking state
     int r_cur = 0, ubase = 0, u_in_r = 0, kvoff = 0, remaining = 0, tile_base = 0, Geff = 1;
     ReqInfo cur;
-    cur.units = 0; cur.tiles_u = 1; cur.np = 1; cur.c = 0; cur.q0 = 0; cur.rows = 0;
+    cur.units = 0; cur.tiles_u = 1; cur.np = 1; cur.c = 0; cur.q0 = 0; cur.qn = 0;
     if (R > 0) cur = req_info(p, 0);
     if (!dynamic && T > 0) {
         Geff = G_ctas < T ? G_ctas : T;
@@ -212,7 +211,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
     while (true) {
         if (*abort_flag) break;
         Item it;
-        it.valid = 0; it.r = 0; it.g = 0; it.row0 = 0; it.rows0 = 0; it.rows1 = 0; it.q_start = 0; it.c = 0;
+        it.valid = 0; it.r = 0; it.g = 0; it.tok0 = 0; it.rows0 = 0; it.rows1 = 0; it.q_start = 0; it.c = 0;
         it.kv0 = 0; it.kv1 = 0; it.part_slot = -1; it.b_head = 0; it.npieces = 1; it.pad0 = 0; it.pad1 = 0; it.pad2 = 0;
         if (dynamic) {
             int u = 0;
@@ -227,14 +226,14 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                 if (r_cur < R) {
                     const int ul = u - ubase;
                     it.valid = 1; it.r = r_cur; it.g = ul / cur.np;
-                    it.row0 = (ul - it.g * cur.np) * PAIR;
+                    it.tok0 = (ul - it.g * cur.np) * 2 * p.tpt;
                     it.kv0 = 0; it.kv1 = cur.tiles_u;
                 }
             }
         } else if (remaining > 0 && r_cur < R) {
             const int take = remaining < cur.tiles_u - kvoff ? remaining : cur.tiles_u - kvoff;
             it.valid = 1; it.r = r_cur; it.g = u_in_r / cur.np;
-            it.row0 = (u_in_r - it.g * cur.np) * PAIR;
+            it.tok0 = (u_in_r - it.g * cur.np) * 2 * p.tpt;
             it.kv0 = kvoff; it.kv1 = kvoff + take;
             if (!(it.kv0 == 0 && it.kv1 == cur.tiles_u)) {
                 // a piece of a unit split across CTAs: CTA x holds flattened tiles [floor(xT/Geff), floor((x+1)T/Geff))
@@ -263,9 +262,9 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
         if (it.valid) {
             ReqInfo ri = cur;
             if (it.r != r_cur) ri = req_info(p, it.r);   // static walk may already have advanced
-            const int left = ri.rows - it.row0;
-            it.rows0 = left < BM ? left : BM;
-            it.rows1 = left > BM ? (left - BM < BM ? left - BM : BM) : 0;
+            const int left = ri.qn - it.tok0;
+            it.rows0 = (left < p.tpt ? left : p.tpt) * p.G;
+            it.rows1 = left > p.tpt ? (left - p.tpt < p.tpt ? left - p.tpt : p.tpt) * p.G : 0;
             it.q_start = ri.q0;
             it.c = ri.c;
             if (ri.c == 0) { it.kv0 = 0; it.kv1 = 0; }
@@ -317,18 +316,17 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
 }
 
 // ------------------------------------------------------------------------------------------------
-// warps 8-9: Q loader.  Packed row rg of the (r, g) group = (token rg / G, q head g*G + rg % G).
-// Rows go to a 2-slot ring of 128-row tiles in the K-major 128B-swizzled UMMA layout.
+// warp 9: Q loader.  q is viewed as a 3-D tensor [total_q][Hq][D]; one TMA box = 64 columns x the G heads
+// of the group x tpt tokens lands as rows (token * G + head) of a K-major 128B-swizzled UMMA tile.
+// Two q-tile slots form a ring; a slot is refilled as soon as the last QK reading it has completed.
+// Rows past the request's last token hold the next request's tokens or TMA zero fill: never stored.
 // ------------------------------------------------------------------------------------------------
 template <int D>
-__device__ __forceinline__ void qload_warps(const AttnParams& p, uint8_t* smem, uint32_t sbase, const Item* items,
-                                            volatile uint32_t* abort_flag, int tid64, int lane) {
+__device__ __forceinline__ void qload_warp(const AttnParams& p, const CUtensorMap* mapQ, uint32_t sbase, const Item* items,
+                                           volatile uint32_t* abort_flag, int lane) {
     using L = Smem<D>;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
-    constexpr int CPR = D / 8;                 // 16-byte chunks per row
-    constexpr int RPP = 64 / CPR;              // rows per pass of the 64 loader threads
-    const int chunk = tid64 % CPR, rsub = tid64 / CPR;
-    const int slab = chunk >> 3, c16 = chunk & 7;
+    const uint32_t tile_bytes = (uint32_t)(p.tpt * p.G * D * 2);
     uint32_t icount = 0, qcount = 0;
     while (true) {
         if (*abort_flag) break;
@@ -340,31 +338,11 @@ __device__ __forceinline__ void qload_warps(const AttnParams& p, uint8_t* smem, 
         for (int t = 0; t < nq; ++t) {
             const uint32_t qs = qcount & 1u;
             ptx::mbar_wait(bar(L::B_Q_EMPTY + qs), ((qcount >> 1) & 1u) ^ 1u, abort_flag);
-            const int rows = t ? it.rows1 : it.rows0;
-            const int rows_pad = (rows + 31) & ~31;      // partially valid warps see zeros, not stale bits
-            uint8_t* dst = smem + L::OFF_Q + qs * L::Q_BYTES + slab * SLAB;
-            constexpr int UN = 8;
-            for (int i0 = 0; i0 < rows_pad; i0 += RPP * UN) {
-                uint4 v[UN];
-#pragma unroll
-                for (int u = 0; u < UN; ++u) {
-                    const int rr = i0 + u * RPP + rsub;
-                    v[u] = make_uint4(0, 0, 0, 0);
-                    if (rr < rows) {
-                        const int rg = it.row0 + t * BM + rr;
-                        const int tl = rg / p.G, hh = rg - tl * p.G;
-                        v[u] = __ldg(reinterpret_cast<const uint4*>(p.q + ((int64_t)(it.q_start + tl) * p.Hq + it.g * p.G + hh) * D) + chunk);
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < UN; ++u) {
-                    const int rr = i0 + u * RPP + rsub;
-                    if (rr < rows_pad) *reinterpret_cast<uint4*>(dst + rr * 128 + ((c16 ^ (rr & 7)) << 4)) = v[u];
-                }
-            }
-            ptx::fence_proxy_async_smem();
+            if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_Q_FULL + qs), tile_bytes);
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(bar(L::B_Q_FULL + qs));
+            if (lane < D / 64)
+                ptx::tma_load_3d(sbase + (uint32_t)(L::OFF_Q + qs * L::Q_BYTES + lane * SLAB), mapQ, bar(L::B_Q_FULL + qs),
+                                 lane * 64, it.g * p.G, it.q_start + it.tok0 + t * p.tpt);
             ++qcount;
         }
         __syncwarp();
@@ -374,156 +352,181 @@ __device__ __forceinline__ void qload_warps(const AttnParams& p, uint8_t* smem, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// warp 11: MMA issuer (a5, a7).  TMEM columns: S_s = [128 s, 128 s + 128), O_s = [256 + 128 s, .. + D).
-// P_s (bf16, two per column) overwrites the first 64 columns of S_s.  Issue order per item (OpWalk):
-//   QK(0,0) QK(1,0) | PV(0,j) QK(0,j+1) PV(1,j) QK(1,j+1) | ...
-// This warp is the pacemaker of the CTA: the per-op path is kept to a few dozen instructions.
+// warps 10, 11: MMA issuers (a5, a7), one per softmax stream s.  TMEM columns: S_s = [128 s, 128 s + 128),
+// O_s = [256 + 128 s, .. + D).  P_s (bf16, two per column) overwrites the first 64 columns of S_s.
+// Per stream the chain is  QK(s,0) | wait P -> PV(s,j) + QK(s,j+1) in one issue block | ...
+// The two issuers are independent, so a stream's PV/QK go out the moment its P is ready even while the
+// other stream's MMAs are queued; the in-order tensor pipe interleaves them.  K/V ring stages are consumed
+// in the order of OpWalk: each issuer walks the whole order, acts on its own ops and skips the other's.
+// KV_EMPTY and Q_EMPTY expect two arrivals: SHARED stages / SPLIT q tiles are read by both issuers (one
+// commit each), SPLIT stages / SHARED q tiles by one issuer (which commits twice).
 // ------------------------------------------------------------------------------------------------
 template <int D>
 struct MmaState {
     uint32_t sbase, tmem;
     uint64_t q_desc0, k_desc0, v_desc0;
-    uint32_t stage, phase;            // next ring stage to acquire and its parity
-    uint32_t stage_k, stage_v;        // stages currently held
-    uint32_t pv_par0, pv_par1;        // parity of the next P_FULL wait per stream
+    uint32_t stage, phase;            // next ring position and its parity
+    uint32_t pv_par;                  // parity of the next P_FULL wait
+    uint32_t zf_par;                  // parity of the next ZFILL wait (SHARED tail tiles)
     volatile uint32_t* abort_flag;
+    __device__ __forceinline__ uint32_t bar(int i) const { return sbase + (uint32_t)(Smem<D>::OFF_BAR + i * 8); }
+    __device__ __forceinline__ void skip() { if (++stage == NSTAGE) { stage = 0; phase ^= 1u; } }
+    __device__ __forceinline__ uint32_t acquire() {
+        const uint32_t s0 = stage;
+        ptx::mbar_wait(bar(Smem<D>::B_KV_FULL + s0), phase, abort_flag);
+        skip();
+        return s0;
+    }
 };
 
+// stale rows [nv, ncols) of the last page of a V tile: zero them so that P = 0 meets V = 0, never NaN (reading S12)
 template <int D>
-__device__ __forceinline__ uint32_t mma_acquire(MmaState<D>& st) {
-    using L = Smem<D>;
-    const uint32_t stage = st.stage;
-    ptx::mbar_wait(st.sbase + (uint32_t)(L::OFF_BAR + (L::B_KV_FULL + stage) * 8), st.phase, st.abort_flag);
-    if (++st.stage == NSTAGE) { st.stage = 0; st.phase ^= 1u; }
-    return stage;
-}
-
-// S_s = Q K^T for kv tile `tile`
-template <int D>
-__device__ __forceinline__ void mma_qk(MmaState<D>& st, int s, int c, int tile, uint32_t qs, bool acquire, bool release, bool last_qk) {
-    using L = Smem<D>;
-    if (acquire) st.stage_k = mma_acquire<D>(st);
-    ptx::tc_fence_after();
-    int nv = c - tile * BN;
-    nv = nv > BN ? BN : nv;
-    const uint32_t ncols = (uint32_t)((nv + 15) & ~15);
-    if (ptx::elect_one()) {
-        const uint32_t bar0 = st.sbase + (uint32_t)L::OFF_BAR;
-        const uint64_t a_desc = st.q_desc0 + (uint64_t)(qs * (L::Q_BYTES >> 4));
-        const uint64_t b_desc = st.k_desc0 + (uint64_t)(st.stage_k * (L::KV_BYTES >> 4));
-        const uint32_t idesc = ptx::idesc_bf16(BM, ncols, 0, 0);
-        const uint32_t d_tmem = st.tmem + (uint32_t)s * 128u;
-        // K-steps of 16 elements = 32 bytes inside a 64-wide slab; the second slab is SLAB bytes further
-        ptx::mma_ss_x4(d_tmem, a_desc, b_desc, idesc, 0u, 2u);
-        if (D == 128) ptx::mma_ss_x4(d_tmem, a_desc + (SLAB >> 4), b_desc + (SLAB >> 4), idesc, 1u, 2u);
-        if (release) ptx::mma_commit(bar0 + (uint32_t)((L::B_KV_EMPTY + st.stage_k) * 8));
-        ptx::mma_commit(bar0 + (uint32_t)((L::B_S_FULL + s) * 8));
-        if (last_qk) ptx::mma_commit(bar0 + (uint32_t)((L::B_Q_EMPTY + qs) * 8));
+__device__ __forceinline__ void zero_v_tail(uint32_t v_addr, int nv, int ncols, int lane) {
+    const int nrows = ncols - nv;
+    for (int e = lane; e < nrows * 8 * (D / 64); e += 32) {
+        const int chunk = e & 7, rr = (e >> 3) % nrows, slab = (e >> 3) / nrows;
+        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(v_addr + (uint32_t)(slab * SLAB + (nv + rr) * 128 + chunk * 16)), "r"(0)
+                     : "memory");
     }
+    ptx::fence_proxy_async_smem();
     __syncwarp();
 }
 
-// O_s (+)= P_s V for kv tile `tile`; `first` overwrites the accumulator
+// One issue block of stream s:  [O_s (+)= P_s V(tile_v)]  then  [S_s = Q K(tile_k)^T].
+// do_pv / do_qk select the halves; rel = commits per consumed stage (2 = sole reader, 1 = shared with the other issuer).
 template <int D>
-__device__ __forceinline__ void mma_pv(MmaState<D>& st, int s, int c, int tile, bool first, bool acquire, bool release, int lane) {
+__device__ __forceinline__ void mma_block(MmaState<D>& st, int s, int c, bool do_pv, int tile_v, bool first_pv, uint32_t stage_v,
+                                          bool do_qk, int tile_k, uint32_t stage_k, uint32_t qs, int rel, int q_rel) {
     using L = Smem<D>;
-    int nv = c - tile * BN;
-    nv = nv > BN ? BN : nv;
-    const int ncols = (nv + 15) & ~15;
-    if (acquire) {
-        st.stage_v = mma_acquire<D>(st);
-        if (nv < ncols) {
-            // stale rows of the last page: zero them so that P = 0 meets V = 0, never NaN (reading S12)
-            const uint32_t v_addr = st.sbase + (uint32_t)(L::OFF_KV + st.stage_v * L::KV_BYTES);
-            const int nrows = ncols - nv;
-            for (int e = lane; e < nrows * 8 * (D / 64); e += 32) {
-                const int chunk = e & 7, rr = (e >> 3) % nrows, slab = (e >> 3) / nrows;
-                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(
-                                 v_addr + (uint32_t)(slab * SLAB + (nv + rr) * 128 + chunk * 16)),
-                             "r"(0)
-                             : "memory");
-            }
-            ptx::fence_proxy_async_smem();
-            __syncwarp();
-        }
+    int nvv = c - tile_v * BN; nvv = nvv > BN ? BN : nvv;
+    int nvk = c - tile_k * BN; nvk = nvk > BN ? BN : nvk;
+    const uint32_t ncols_v = (uint32_t)((nvv + 15) & ~15), ncols_k = (uint32_t)((nvk + 15) & ~15);
+    if (do_pv) {
+        ptx::mbar_wait(st.bar(L::B_P_FULL + s), st.pv_par, st.abort_flag);
+        st.pv_par ^= 1u;
     }
-    uint32_t& par = s ? st.pv_par1 : st.pv_par0;
-    ptx::mbar_wait(st.sbase + (uint32_t)(L::OFF_BAR + (L::B_P_FULL + s) * 8), par, st.abort_flag);
-    par ^= 1u;
     ptx::tc_fence_after();
     if (ptx::elect_one()) {
-        const uint32_t bar0 = st.sbase + (uint32_t)L::OFF_BAR;
-        const uint64_t b_desc = st.v_desc0 + (uint64_t)(st.stage_v * (L::KV_BYTES >> 4));
-        const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
-        const uint32_t d_tmem = st.tmem + 256u + (uint32_t)s * 128u, a_tmem = st.tmem + (uint32_t)s * 128u;
-        if (ncols == BN) {                                    // K-steps of 16 kv rows = 2048 bytes of V
-            ptx::mma_ts_x4(d_tmem, a_tmem, b_desc, idesc, first ? 0u : 1u, 128u);
-            ptx::mma_ts_x4(d_tmem, a_tmem + 32u, b_desc + 512u, idesc, 1u, 128u);
-        } else {
-            for (int ks = 0; ks < ncols / 16; ++ks)
-                ptx::mma_ts(d_tmem, a_tmem + (uint32_t)(ks * 8), b_desc + (uint64_t)(ks * 128), idesc, (!first || ks > 0) ? 1u : 0u);
+        if (do_pv) {
+            const uint64_t b_desc = st.v_desc0 + (uint64_t)(stage_v * (L::KV_BYTES >> 4));
+            const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
+            const uint32_t d_tmem = st.tmem + 256u + (uint32_t)s * 128u, a_tmem = st.tmem + (uint32_t)s * 128u;
+            if (ncols_v == BN) {                                  // K-steps of 16 kv rows = 2048 bytes of V
+                ptx::mma_ts_x4(d_tmem, a_tmem, b_desc, idesc, first_pv ? 0u : 1u, 128u);
+                ptx::mma_ts_x4(d_tmem, a_tmem + 32u, b_desc + 512u, idesc, 1u, 128u);
+            } else {
+                for (uint32_t ks = 0; ks < ncols_v / 16; ++ks)
+                    ptx::mma_ts(d_tmem, a_tmem + ks * 8u, b_desc + (uint64_t)(ks * 128u), idesc, (!first_pv || ks > 0) ? 1u : 0u);
+            }
+            ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_v));
+            if (rel == 2) ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_v));
+            ptx::mma_commit(st.bar(L::B_PV_DONE + s));
         }
-        if (release) ptx::mma_commit(bar0 + (uint32_t)((L::B_KV_EMPTY + st.stage_v) * 8));
-        ptx::mma_commit(bar0 + (uint32_t)((L::B_PV_DONE + s) * 8));
+        if (do_qk) {
+            const uint64_t a_desc = st.q_desc0 + (uint64_t)(qs * (L::Q_BYTES >> 4));
+            const uint64_t b_desc = st.k_desc0 + (uint64_t)(stage_k * (L::KV_BYTES >> 4));
+            const uint32_t idesc = ptx::idesc_bf16(BM, ncols_k, 0, 0);
+            const uint32_t d_tmem = st.tmem + (uint32_t)s * 128u;
+            // K-steps of 16 elements = 32 bytes inside a 64-wide slab; the second slab is SLAB bytes further
+            ptx::mma_ss_x4(d_tmem, a_desc, b_desc, idesc, 0u, 2u);
+            if (D == 128) ptx::mma_ss_x4(d_tmem, a_desc + (SLAB >> 4), b_desc + (SLAB >> 4), idesc, 1u, 2u);
+            ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_k));
+            if (rel == 2) ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_k));
+            ptx::mma_commit(st.bar(L::B_S_FULL + s));
+            for (int i = 0; i < q_rel; ++i) ptx::mma_commit(st.bar(L::B_Q_EMPTY + qs));
+        }
     }
     __syncwarp();
 }
 
 template <int D>
 __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, uint32_t tmem, const Item* items,
-                                         volatile uint32_t* abort_flag, int lane) {
+                                         volatile uint32_t* abort_flag, int s, int lane) {
     using L = Smem<D>;
-    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
     MmaState<D> st;
     st.sbase = sbase; st.tmem = tmem; st.abort_flag = abort_flag;
     st.q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);        // K-major operands (Q, K)
     st.k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, 1024);
     st.v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, SLAB, 1024);     // MN-major operand (V)
-    st.stage = 0; st.phase = 0; st.stage_k = 0; st.stage_v = 0; st.pv_par0 = 0; st.pv_par1 = 0;
+    st.stage = 0; st.phase = 0; st.pv_par = 0; st.zf_par = 0;
     uint32_t icount = 0, qcount = 0;
     while (true) {
         if (*abort_flag) break;
         const uint32_t islot = icount & 1u;
-        ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
+        ptx::mbar_wait(st.bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
         const Item it = items[islot];
         if (!it.valid) break;
         const int n = it.kv1 - it.kv0, c = it.c, kv0 = it.kv0;
         if (n > 0) {
             if (it.rows1 > 0) {
-                // SHARED: stream s = q tile s; both streams read the same K/V stage (stream 0 acquires, stream 1 releases)
-                const uint32_t qs0 = qcount & 1u, qs1 = qs0 ^ 1u;
-                ptx::mbar_wait(bar(L::B_Q_FULL + qs0), (qcount >> 1) & 1u, abort_flag);
-                mma_qk<D>(st, 0, c, kv0, qs0, true, false, n == 1);
-                ptx::mbar_wait(bar(L::B_Q_FULL + qs1), ((qcount + 1) >> 1) & 1u, abort_flag);
-                mma_qk<D>(st, 1, c, kv0, qs1, false, true, n == 1);
+                // SHARED: stream s = q tile s; ring order K_0 V_0 K_1 V_1 ..., every stage read by both issuers
+                const uint32_t qc = qcount + (uint32_t)s, qs = qc & 1u;
+                ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qc >> 1) & 1u, abort_flag);
+                uint32_t sk = st.acquire();
+                mma_block<D>(st, s, c, false, kv0, false, 0u, true, kv0, sk, qs, 1, n == 1 ? 2 : 0);
                 for (int j = 0; j < n; ++j) {
-                    const bool more = j + 1 < n, lastq = j + 2 == n;
-                    mma_pv<D>(st, 0, c, kv0 + j, j == 0, true, false, lane);
-                    if (more) mma_qk<D>(st, 0, c, kv0 + j + 1, qs0, true, false, lastq);
-                    mma_pv<D>(st, 1, c, kv0 + j, j == 0, false, true, lane);
-                    if (more) mma_qk<D>(st, 1, c, kv0 + j + 1, qs1, false, true, lastq);
+                    const bool more = j + 1 < n;
+                    const uint32_t sv = st.acquire();
+                    int nv = c - (kv0 + j) * BN;
+                    if (nv < BN && (nv & 15)) {              // tail tile: issuer 0 zero-fills, issuer 1 waits for it
+                        if (s == 0) {
+                            zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
+                            if (lane == 0) ptx::mbar_arrive(st.bar(L::B_ZFILL));
+                        } else {
+                            ptx::mbar_wait(st.bar(L::B_ZFILL), st.zf_par, abort_flag);
+                        }
+                        st.zf_par ^= 1u;
+                    }
+                    if (more) sk = st.acquire();
+                    mma_block<D>(st, s, c, true, kv0 + j, j == 0, sv, more, kv0 + j + 1, sk, qs, 1, (more && j + 2 == n) ? 2 : 0);
                 }
                 qcount += 2;
             } else {
-                // SPLIT: one q tile; stream s takes kv tiles kv0 + 2i + s, every op has its own stage
+                // SPLIT: one q tile read by both issuers; stream s owns kv tiles kv0 + 2i + s and their stages.
+                // Ring order: K(0,0) [K(1,0)] | V(0,i) [K(0,i+1)] [V(1,i)] [K(1,i+1)] | ...
                 const uint32_t qs = qcount & 1u;
-                const int n0 = (n + 1) >> 1, n1 = n >> 1;
-                ptx::mbar_wait(bar(L::B_Q_FULL + qs), (qcount >> 1) & 1u, abort_flag);
-                mma_qk<D>(st, 0, c, kv0, qs, true, true, n == 1);
-                if (n1 > 0) mma_qk<D>(st, 1, c, kv0 + 1, qs, true, true, n == 2);
+                const int n0 = (n + 1) >> 1, n1 = n >> 1, ns = s ? n1 : n0;
+                ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qcount >> 1) & 1u, abort_flag);
+                uint32_t sk = 0, sv = 0;
+                if (s == 0) sk = st.acquire(); else st.skip();
+                if (n1 > 0) { if (s == 1) sk = st.acquire(); else st.skip(); }
+                if (ns > 0) mma_block<D>(st, s, c, false, 0, false, 0u, true, kv0 + s, sk, qs, 2, ns == 1 ? 1 : 0);
+                else if (lane == 0) ptx::mbar_arrive(st.bar(L::B_Q_EMPTY + qs));      // nothing to read: release the q tile
                 for (int i = 0; i < n0; ++i) {
-                    mma_pv<D>(st, 0, c, kv0 + 2 * i, i == 0, true, true, lane);
-                    if (i + 1 < n0) mma_qk<D>(st, 0, c, kv0 + 2 * i + 2, qs, true, true, 2 * i + 3 == n);
+                    // stream 0's pair of stages
+                    bool more = i + 1 < n0;
+                    if (s == 0) {
+                        sv = st.acquire();
+                        const int tile = kv0 + 2 * i;
+                        const int nv = c - tile * BN;
+                        if (nv < BN && (nv & 15)) zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
+                        if (more) sk = st.acquire();
+                        mma_block<D>(st, 0, c, true, tile, i == 0, sv, more, tile + 2, sk, qs, 2, (more && i + 2 == n0) ? 1 : 0);
+                    } else {
+                        st.skip();
+                        if (more) st.skip();
+                    }
+                    // stream 1's pair of stages
                     if (i < n1) {
-                        mma_pv<D>(st, 1, c, kv0 + 2 * i + 1, i == 0, true, true, lane);
-                        if (i + 1 < n1) mma_qk<D>(st, 1, c, kv0 + 2 * i + 3, qs, true, true, 2 * i + 4 == n);
+                        more = i + 1 < n1;
+                        if (s == 1) {
+                            sv = st.acquire();
+                            const int tile = kv0 + 2 * i + 1;
+                            const int nv = c - tile * BN;
+                            if (nv < BN && (nv & 15)) zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
+                            if (more) sk = st.acquire();
+                            mma_block<D>(st, 1, c, true, tile, i == 0, sv, more, tile + 2, sk, qs, 2, (more && i + 2 == n1) ? 1 : 0);
+                        } else {
+                            st.skip();
+                            if (more) st.skip();
+                        }
                     }
                 }
                 qcount += 1;
             }
         }
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
+        if (lane == 0) ptx::mbar_arrive(st.bar(L::B_ITEM_EMPTY + islot));
         ++icount;
     }
 }
@@ -677,7 +680,9 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         float m = -INFINITY, l = 0.f;
         for (int i = 0; i < ns; ++i) {
             if (*abort_flag) break;
+            TRACE_EV(20 + s);
             ptx::mbar_wait(bar(L::B_S_FULL + s), tcount & 1u, abort_flag);
+            TRACE_EV(22 + s);
             ptx::tc_fence_after();
             const int tile = shared ? it.kv0 + i : it.kv0 + 2 * i + s;
             int nv = it.c - tile * BN;
@@ -707,6 +712,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
             }
             ptx::tc_fence_before();
             __syncwarp();
+            TRACE_EV(24 + s);
             if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL + s));
             ++tcount;
         }
@@ -716,9 +722,9 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         }
         // ---------------- epilogue
         const bool row_ok = row < rows_valid;
-        const int rg = it.row0 + ((shared && s == 1) ? BM : 0) + row;
-        const int tl = rg / p.G, hh = rg - tl * p.G;
-        uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)(it.q_start + tl) * p.Hq + it.g * p.G + hh) * D);
+        const int tl = row / p.G, hh = row - tl * p.G;                       // row = token * G + head of the group
+        const int tok = it.q_start + it.tok0 + ((shared && s == 1) ? p.tpt : 0) + tl;
+        uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + it.g * p.G + hh) * D);
         const int prow = ((shared && s == 1) ? BM : 0) + row;                 // row inside the partial slot
         float* po = p.part_o + ((int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * PAIR + prow) * D;
         float2* pml = reinterpret_cast<float2*>(p.part_ml) + (int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * PAIR + prow;
@@ -789,7 +795,8 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
                 const int w8 = s * 4 + wg_warp, rows_u = it.rows0 + it.rows1, np = it.npieces;
                 const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
                 constexpr int EPL = D / 32;
-                for (int rr = w8; rr < rows_u; rr += 8) {
+                for (int ru = w8; ru < rows_u; ru += 8) {
+                    const int t1 = ru >= it.rows0, rloc = ru - (t1 ? it.rows0 : 0), rr = t1 * BM + rloc;   // row inside the slot
                     float ms = -INFINITY;
                     for (int base = 0; base < np; base += 32) {
                         const int pi = base + lane;
@@ -820,9 +827,9 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
                         }
                     }
                     const float inv = ls > 0.f ? 1.f / ls : 0.f;
-                    const int rg2 = it.row0 + rr;
-                    const int tl2 = rg2 / p.G, hh2 = rg2 - tl2 * p.G;
-                    __nv_bfloat16* d2 = p.out + ((int64_t)(it.q_start + tl2) * p.Hq + it.g * p.G + hh2) * D + lane * EPL;
+                    const int tl2 = rloc / p.G, hh2 = rloc - tl2 * p.G;
+                    const int tok2 = it.q_start + it.tok0 + t1 * p.tpt + tl2;
+                    __nv_bfloat16* d2 = p.out + ((int64_t)tok2 * p.Hq + it.g * p.G + hh2) * D + lane * EPL;
                     if (EPL == 4) {
                         uint2 w2;
                         w2.x = ptx::pack_bf16(acc[0] * inv, acc[1] * inv);
@@ -846,7 +853,8 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __global__ void __launch_bounds__(NTHREADS, 1)
-attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV, const AttnParams p) {
+attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
+            const __grid_constant__ CUtensorMap mapQ, const AttnParams p) {
     using L = Smem<D>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -855,14 +863,15 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::OFF_MISC);
     volatile uint32_t* abort_flag = reinterpret_cast<volatile uint32_t*>(smem + L::OFF_MISC + 4);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    TRACE_INIT();
     if (tid == 0) {
         auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
-        for (int s = 0; s < NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 1); }
+        for (int s = 0; s < NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 2); }
         for (int s = 0; s < 2; ++s) {
             ptx::mbar_init(bar(L::B_ITEM_FULL + s), 1);
-            ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 11);  // MMA lane + 2 loader warps + 8 softmax warps
-            ptx::mbar_init(bar(L::B_Q_FULL + s), 2);       // the two loader warps
-            ptx::mbar_init(bar(L::B_Q_EMPTY + s), 1);
+            ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 11);  // 2 MMA issuers + loader warp + 8 softmax warps
+            ptx::mbar_init(bar(L::B_Q_FULL + s), 1);
+            ptx::mbar_init(bar(L::B_Q_EMPTY + s), 2);
             ptx::mbar_init(bar(L::B_S_FULL + s), 1);
             ptx::mbar_init(bar(L::B_P_FULL + s), 4);
             ptx::mbar_init(bar(L::B_PV_DONE + s), 1);
@@ -871,10 +880,12 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
         ptx::mbar_init(bar(L::B_EPI_B), 128);
         ptx::mbar_init(bar(L::B_EPI_C), 256);
         ptx::mbar_init(bar(L::B_EPI_D), 1);
+        ptx::mbar_init(bar(L::B_ZFILL), 1);
         *abort_flag = 0u;
         ptx::fence_mbar_init();
         ptx::prefetch_tensormap(&mapK);
         ptx::prefetch_tensormap(&mapV);
+        ptx::prefetch_tensormap(&mapQ);
     }
     if (warp == 8) {
         ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
@@ -886,16 +897,16 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
     const uint32_t tmem = *tmem_slot;
 
     // Warpgroups 0 and 1 are the softmax streams (TMEM lane quarter = warp % 4); warpgroup 2 holds the
-    // service warps.  The MMA issuer is the highest warp id: the SM sub-partition arbiter favours it over
-    // the softmax warps it shares a scheduler with, so a tile's MMAs are issued the moment P is ready.
+    // service warps.  The MMA issuers are the highest warp ids: the SM sub-partition arbiter favours them
+    // over the softmax warps they share a scheduler with, so a tile's MMAs go out the moment P is ready.
     if (warp < 8) {
         ptx::setmaxnreg_inc<208>();   // 8*32*208 + 4*32*80 <= 384*168: the pool is what the CTA got at launch
         softmax_wg<D>(p, smem, sbase, tmem, items, abort_flag, warp >> 2, warp & 3, lane);
     } else {
         ptx::setmaxnreg_dec<80>();
-        if (warp == 10) producer_warp<D>(p, &mapK, &mapV, sbase, items, abort_flag, lane);
-        else if (warp == 11) mma_warp<D>(p, sbase, tmem, items, abort_flag, lane);
-        else qload_warps<D>(p, smem, sbase, items, abort_flag, tid - 256, lane);
+        if (warp == 8) producer_warp<D>(p, &mapK, &mapV, sbase, items, abort_flag, lane);
+        else if (warp == 9) qload_warp<D>(p, &mapQ, sbase, items, abort_flag, lane);
+        else mma_warp<D>(p, sbase, tmem, items, abort_flag, warp - 10, lane);
     }
     ptx::tc_fence_before();
     __syncthreads();
@@ -942,10 +953,28 @@ static inline int tc_encode_maps(TcMaps* maps, const void* k_pages, const void* 
     return 0;
 }
 
+// q viewed as [total_q][Hq][D] bf16; one box = tpt tokens x G heads x 64 columns, 128-byte swizzled
+static inline int tc_encode_q(TcMaps* maps, const void* q, int total_q, int Hq, int D, int G, int tpt) {
+    sangam_encode_fn enc = nullptr;
+    {
+        cudaDriverEntryPointQueryResult qr;
+        void* fn = nullptr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn) return -1;
+        enc = reinterpret_cast<sangam_encode_fn>(fn);
+    }
+    const cuuint64_t gdim[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)total_q};
+    const cuuint64_t gstr[2] = {(cuuint64_t)D * 2, (cuuint64_t)Hq * D * 2};
+    const cuuint32_t box[3] = {64, (cuuint32_t)G, (cuuint32_t)tpt}, estr[3] = {1, 1, 1};
+    CUresult r = enc(&maps->q, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), gdim, gstr, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? 0 : -1;
+}
+
 static inline cudaError_t tc_launch(const AttnParams& p, const TcMaps& maps, int head_dim, int sm_count,
                                     cudaStream_t stream, int* launched) {
-    if (head_dim == 128) tc::attn_kernel<128><<<sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream>>>(maps.k, maps.v, p);
-    else tc::attn_kernel<64><<<sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream>>>(maps.k, maps.v, p);
+    if (head_dim == 128) tc::attn_kernel<128><<<sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
+    else tc::attn_kernel<64><<<sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
     *launched = 1;
     return cudaGetLastError();
 }

@@ -28,6 +28,8 @@ struct sangam_ctx {
     TcMaps maps;
     const void* maps_k;
     const void* maps_v;
+    const void* maps_q;
+    int32_t maps_q_rows;
     // staging for sangam_iteration_host (allocated on first use)
     void *s_q, *s_k, *s_v, *s_out;
     int32_t *s_slot, *s_bt, *s_cu, *s_ctx;
@@ -63,6 +65,7 @@ extern "C" int sangam_create(const sangam_config* cfg, sangam_ctx** out) {
     if (cfg->page_size != SANGAM_PAGE) return SANGAM_ERR_UNSUPPORTED;
     if (cfg->head_dim != 64 && cfg->head_dim != 128) return SANGAM_ERR_UNSUPPORTED;
     if (cfg->num_q_heads <= 0 || cfg->num_kv_heads <= 0 || cfg->num_q_heads % cfg->num_kv_heads) return SANGAM_ERR_INVALID_ARG;
+    if (cfg->num_q_heads / cfg->num_kv_heads > 128) return SANGAM_ERR_UNSUPPORTED;   // a q tile holds whole tokens of one group
     if (cfg->num_pages <= 0 || cfg->max_batch <= 0 || cfg->max_total_q <= 0 || cfg->max_pages_per_req <= 0)
         return SANGAM_ERR_INVALID_ARG;
     if ((int64_t)cfg->num_pages * SANGAM_PAGE > 0x7fffffffLL) return SANGAM_ERR_INVALID_ARG;
@@ -163,6 +166,7 @@ static AttnParams make_params(sangam_ctx* ctx, const void* q, const void* k_page
     p.batch = batch; p.total_q = total_q;
     p.Hq = ctx->cfg.num_q_heads; p.Hkv = ctx->cfg.num_kv_heads; p.G = ctx->G;
     p.W = ctx->cfg.max_pages_per_req; p.P = ctx->cfg.num_pages;
+    p.tpt = 128 / ctx->G;
     p.scale = scale;
     p.scale_log2 = scale * 1.4426950408889634f;
     p.part_o = ctx->d_part_o; p.part_ml = ctx->d_part_ml; p.num_slots = ctx->num_slots; p.unit_count = ctx->d_unit_count;
@@ -194,6 +198,11 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
         if (tc_encode_maps(&ctx->maps, k_pages, v_pages, ctx->cfg.num_pages, ctx->cfg.num_kv_heads, ctx->cfg.head_dim) != 0)
             return fail(ctx, SANGAM_ERR_CUDA, "block_attn: cuTensorMapEncodeTiled failed");
         ctx->maps_k = k_pages; ctx->maps_v = v_pages;
+    }
+    if (ctx->maps_q != q || ctx->maps_q_rows != total_q) {
+        if (tc_encode_q(&ctx->maps, q, total_q, ctx->cfg.num_q_heads, ctx->cfg.head_dim, ctx->G, 128 / ctx->G) != 0)
+            return fail(ctx, SANGAM_ERR_CUDA, "block_attn: cuTensorMapEncodeTiled (q) failed");
+        ctx->maps_q = q; ctx->maps_q_rows = total_q;
     }
     AttnParams p = make_params(ctx, q, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, batch, total_q, scale, out);
     int launched = 0;
@@ -252,3 +261,18 @@ extern "C" int sangam_iteration_host(sangam_ctx* ctx, const void* q_host, const 
     CK(cudaStreamSynchronize(st));
     return SANGAM_OK;
 }
+
+#ifdef SANGAM_TRACE
+// debug builds only: copy the event trace of CTA 0 (per-warp rings, concatenated) to the host
+extern "C" int sangam_trace_read(unsigned long long* host_buf, int cap) {
+    unsigned int n[16];
+    static unsigned long long tmp[16 * SANGAM_TRACE_CAP];
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(n, g_trace_n, sizeof n);
+    cudaMemcpyFromSymbol(tmp, g_trace, sizeof tmp);
+    int k = 0;
+    for (int w = 0; w < 16; ++w)
+        for (unsigned i = 0; i < n[w] && i < SANGAM_TRACE_CAP && k < cap; ++i) host_buf[k++] = tmp[w * SANGAM_TRACE_CAP + i];
+    return k;
+}
+#endif
