@@ -628,9 +628,10 @@ __device__ __forceinline__ void store_final_row(uint32_t o0_taddr, uint32_t o1_t
         }
     }
 }
-// partial row (fp32, unnormalised) <- w0 * O0 [+ w1 * O1]
+// partial row (fp32, unnormalised) <- w0 * O0 [+ w1 * O1].  Slot layout [D/4 column groups][256 rows][4 floats]:
+// a warp's 32 rows of one column group are 512 contiguous bytes, so these stores and the merge's loads coalesce.
 template <int D, bool TWO>
-__device__ __forceinline__ void store_partial_row(uint32_t o0_taddr, uint32_t o1_taddr, float w0, float w1, bool row_ok, float* po) {
+__device__ __forceinline__ void store_partial_row(uint32_t o0_taddr, uint32_t o1_taddr, float w0, float w1, bool row_ok, float4* po) {
 #pragma unroll
     for (int c = 0; c < D / 32; ++c) {
         uint32_t o[32], o1[32];
@@ -646,7 +647,7 @@ __device__ __forceinline__ void store_partial_row(uint32_t o0_taddr, uint32_t o1
                     f[e] = __uint_as_float(o[v * 4 + e]) * w0;
                     if (TWO) f[e] = fmaf(__uint_as_float(o1[v * 4 + e]), w1, f[e]);
                 }
-                reinterpret_cast<float4*>(po)[c * 8 + v] = make_float4(f[0], f[1], f[2], f[3]);
+                po[(c * 8 + v) * PAIR] = make_float4(f[0], f[1], f[2], f[3]);
             }
         }
     }
@@ -666,12 +667,15 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
     float2* ml_x = reinterpret_cast<float2*>(smem + L::OFF_ML);
     volatile int* last_flag = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 8);
     uint32_t icount = 0, tcount = 0, ecount = 0, ccount = 0;
+    TRACE_NS(40);
+    TRACE_EV(36);
     while (true) {
         if (*abort_flag) break;
         const uint32_t islot = icount & 1u;
         ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
         const Item it = items[islot];
         if (!it.valid) break;
+        TRACE_EV(30);
         const bool shared = it.rows1 > 0;
         const int n = it.kv1 - it.kv0;
         const int ns = shared ? n : (s == 0 ? (n + 1) / 2 : n / 2);
@@ -721,12 +725,13 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
             ptx::tc_fence_after();
         }
         // ---------------- epilogue
+        TRACE_EV(31);
         const bool row_ok = row < rows_valid;
         const int tl = row / p.G, hh = row - tl * p.G;                       // row = token * G + head of the group
         const int tok = it.q_start + it.tok0 + ((shared && s == 1) ? p.tpt : 0) + tl;
         uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + it.g * p.G + hh) * D);
         const int prow = ((shared && s == 1) ? BM : 0) + row;                 // row inside the partial slot
-        float* po = p.part_o + ((int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * PAIR + prow) * D;
+        float4* po = reinterpret_cast<float4*>(p.part_o) + (int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * (D / 4) * PAIR + prow;
         float2* pml = reinterpret_cast<float2*>(p.part_ml) + (int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * PAIR + prow;
         if (n == 0) {
             // empty context: zeros (reading S13); never split
@@ -773,79 +778,72 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
             ++ecount;
         }
         // ---------------- fused split-KV merge across CTAs (a9): the CTA finishing a unit's last piece merges
+        TRACE_EV(32);
         if (it.part_slot >= 0) {
-            __threadfence();
+            // every thread's partial stores happen-before its arrival; thread 0 then publishes them with one
+            // cumulative gpu-scope fence and counts this piece
             ptx::mbar_arrive(bar(L::B_EPI_C));
-            ptx::mbar_wait(bar(L::B_EPI_C), ccount & 1u, abort_flag);
             if (s == 0 && row == 0) {
+                ptx::mbar_wait(bar(L::B_EPI_C), ccount & 1u, abort_flag);
                 __threadfence();
                 const int old = atomicAdd(p.unit_count + it.b_head, 1);
                 __threadfence();
                 const int last = old == it.npieces - 1;
-                if (last) { p.unit_count[it.b_head] = 0; __threadfence(); }     // re-armed for the next launch
+                if (last) p.unit_count[it.b_head] = 0;                           // re-armed for the next launch
                 *last_flag = last;
                 ptx::mbar_arrive(bar(L::B_EPI_D));
             }
             ptx::mbar_wait(bar(L::B_EPI_D), ccount & 1u, abort_flag);
             const int last = *last_flag;
             ++ccount;
-            if (last) {
+            TRACE_EV(33);
+            const int rr = s * BM + row;                                         // row inside the slot
+            if (last && row < (s ? it.rows1 : it.rows0)) {
                 // pieces in fixed order: head slot 2*b_head+1, then slots 2*b' of CTAs b' = b_head+1 ..; m in log2 units:
                 //   m* = max m_i;  l* = sum l_i 2^(m_i-m*);  O* = sum O_i 2^(m_i-m*);  out = bf16(O*/l*)
-                const int w8 = s * 4 + wg_warp, rows_u = it.rows0 + it.rows1, np = it.npieces;
+                // One thread per row; consecutive rows of a column group are contiguous, so every load coalesces.
+                const int np = it.npieces;
                 const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
-                constexpr int EPL = D / 32;
-                for (int ru = w8; ru < rows_u; ru += 8) {
-                    const int t1 = ru >= it.rows0, rloc = ru - (t1 ? it.rows0 : 0), rr = t1 * BM + rloc;   // row inside the slot
-                    float ms = -INFINITY;
-                    for (int base = 0; base < np; base += 32) {
-                        const int pi = base + lane;
-                        float mm = -INFINITY;
-                        if (pi < np) mm = __ldcg(&ml[(int64_t)(pi == 0 ? 2 * it.b_head + 1 : 2 * (it.b_head + pi)) * PAIR + rr].x);
+                float ms = -INFINITY;
+                for (int pi = 0; pi < np; ++pi)
+                    ms = fmaxf(ms, __ldcg(&ml[(int64_t)(pi == 0 ? 2 * it.b_head + 1 : 2 * (it.b_head + pi)) * PAIR + rr].x));
+                float acc[D];
 #pragma unroll
-                        for (int o = 16; o > 0; o >>= 1) mm = fmaxf(mm, __shfl_xor_sync(FULL, mm, o));
-                        ms = fmaxf(ms, mm);
-                    }
-                    float acc[EPL];
+                for (int e = 0; e < D; ++e) acc[e] = 0.f;
+                float ls = 0.f;
+                for (int pi = 0; pi < np; ++pi) {
+                    const int64_t slot = pi == 0 ? 2 * it.b_head + 1 : 2 * (it.b_head + pi);
+                    const float2 x = __ldcg(&ml[slot * PAIR + rr]);
+                    const float w = ptx::ex2(x.x - ms);
+                    ls = fmaf(x.y, w, ls);
+                    const float4* src = reinterpret_cast<const float4*>(p.part_o) + slot * (D / 4) * PAIR + rr;
 #pragma unroll
-                    for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
-                    float ls = 0.f;
-#pragma unroll 4
-                    for (int pi = 0; pi < np; ++pi) {
-                        const int64_t slot = pi == 0 ? 2 * it.b_head + 1 : 2 * (it.b_head + pi);
-                        const float2 x = __ldcg(&ml[slot * PAIR + rr]);
-                        const float w = ptx::ex2(x.x - ms);
-                        ls = fmaf(x.y, w, ls);
-                        const float* src = p.part_o + (slot * PAIR + rr) * D + lane * EPL;
-                        if (EPL == 4) {
-                            const float4 o = __ldcg(reinterpret_cast<const float4*>(src));
-                            acc[0] = fmaf(o.x, w, acc[0]); acc[1] = fmaf(o.y, w, acc[1]);
-                            acc[2] = fmaf(o.z, w, acc[2]); acc[EPL - 1] = fmaf(o.w, w, acc[EPL - 1]);
-                        } else {
-                            const float2 o = __ldcg(reinterpret_cast<const float2*>(src));
-                            acc[0] = fmaf(o.x, w, acc[0]); acc[1] = fmaf(o.y, w, acc[1]);
-                        }
+                    for (int c4 = 0; c4 < D / 4; ++c4) {
+                        const float4 o = __ldcg(src + c4 * PAIR);
+                        acc[c4 * 4 + 0] = fmaf(o.x, w, acc[c4 * 4 + 0]); acc[c4 * 4 + 1] = fmaf(o.y, w, acc[c4 * 4 + 1]);
+                        acc[c4 * 4 + 2] = fmaf(o.z, w, acc[c4 * 4 + 2]); acc[c4 * 4 + 3] = fmaf(o.w, w, acc[c4 * 4 + 3]);
                     }
-                    const float inv = ls > 0.f ? 1.f / ls : 0.f;
-                    const int tl2 = rloc / p.G, hh2 = rloc - tl2 * p.G;
-                    const int tok2 = it.q_start + it.tok0 + t1 * p.tpt + tl2;
-                    __nv_bfloat16* d2 = p.out + ((int64_t)tok2 * p.Hq + it.g * p.G + hh2) * D + lane * EPL;
-                    if (EPL == 4) {
-                        uint2 w2;
-                        w2.x = ptx::pack_bf16(acc[0] * inv, acc[1] * inv);
-                        w2.y = ptx::pack_bf16(acc[2] * inv, acc[EPL - 1] * inv);
-                        *reinterpret_cast<uint2*>(d2) = w2;
-                    } else {
-                        *reinterpret_cast<uint32_t*>(d2) = ptx::pack_bf16(acc[0] * inv, acc[1] * inv);
-                    }
+                }
+                const float inv = ls > 0.f ? 1.f / ls : 0.f;
+#pragma unroll
+                for (int c8 = 0; c8 < D / 8; ++c8) {
+                    uint4 w4;
+                    w4.x = ptx::pack_bf16(acc[c8 * 8 + 0] * inv, acc[c8 * 8 + 1] * inv);
+                    w4.y = ptx::pack_bf16(acc[c8 * 8 + 2] * inv, acc[c8 * 8 + 3] * inv);
+                    w4.z = ptx::pack_bf16(acc[c8 * 8 + 4] * inv, acc[c8 * 8 + 5] * inv);
+                    w4.w = ptx::pack_bf16(acc[c8 * 8 + 6] * inv, acc[c8 * 8 + 7] * inv);
+                    dst[c8] = w4;
                 }
             }
         }
+        TRACE_EV(34);
         ptx::tc_fence_before();
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
         ++icount;
     }
+    TRACE_EV(35);
+    TRACE_NS(41);
 }
 
 // ------------------------------------------------------------------------------------------------

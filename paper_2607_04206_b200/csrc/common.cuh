@@ -44,13 +44,14 @@ __device__ __forceinline__ void raise_flag(uint32_t* flags, uint32_t f) {
 #define SANGAM_TRACE_CAP 8192            // events per warp
 __device__ unsigned long long g_trace[16 * SANGAM_TRACE_CAP];
 __device__ unsigned int g_trace_n[16];
+__device__ unsigned int g_trace_cta;     // which CTA records (sangam_trace_set_cta)
 __device__ __forceinline__ unsigned int* trace_cnt() {
     __shared__ unsigned int cnt[16];
     return cnt;
 }
 __device__ __forceinline__ void trace_ev(unsigned ev) {
     unsigned int* cnt = trace_cnt();
-    if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) {
+    if (blockIdx.x == g_trace_cta && (threadIdx.x & 31) == 0) {
         unsigned long long t;
         asm volatile("mov.u64 %0, %%clock64;" : "=l"(t));
         const unsigned w = threadIdx.x >> 5, i = cnt[w];
@@ -59,9 +60,23 @@ __device__ __forceinline__ void trace_ev(unsigned ev) {
         g_trace_n[w] = i + 1;
     }
 }
+// same record, but the time stamp is %globaltimer (ns): start/end pair gives the effective SM clock
+__device__ __forceinline__ void trace_ns(unsigned ev) {
+    unsigned int* cnt = trace_cnt();
+    if (blockIdx.x == g_trace_cta && (threadIdx.x & 31) == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        const unsigned w = threadIdx.x >> 5, i = cnt[w];
+        cnt[w] = i + 1;
+        if (i < SANGAM_TRACE_CAP) g_trace[w * SANGAM_TRACE_CAP + i] = (t << 16) | ((unsigned long long)w << 8) | ev;
+        g_trace_n[w] = i + 1;
+    }
+}
 #define TRACE_EV(ev) trace_ev(ev)
+#define TRACE_NS(ev) trace_ns(ev)
 #define TRACE_INIT() do { if (threadIdx.x < 16) trace_cnt()[threadIdx.x] = 0; } while (0)
 #else
 #define TRACE_EV(ev) ((void)0)
+#define TRACE_NS(ev) ((void)0)
 #define TRACE_INIT() ((void)0)
 #endif

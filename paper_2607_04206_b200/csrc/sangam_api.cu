@@ -263,7 +263,14 @@ extern "C" int sangam_iteration_host(sangam_ctx* ctx, const void* q_host, const 
 }
 
 #ifdef SANGAM_TRACE
-// debug builds only: copy the event trace of CTA 0 (per-warp rings, concatenated) to the host
+extern "C" int sangam_trace_set_cta(int cta) {
+    unsigned int v = (unsigned int)cta, z[16] = {0};
+    cudaDeviceSynchronize();
+    cudaMemcpyToSymbol(g_trace_cta, &v, sizeof v);
+    cudaMemcpyToSymbol(g_trace_n, z, sizeof z);
+    return 0;
+}
+// debug builds only: copy the event trace of the recording CTA (per-warp rings, concatenated) to the host
 extern "C" int sangam_trace_read(unsigned long long* host_buf, int cap) {
     unsigned int n[16];
     static unsigned long long tmp[16 * SANGAM_TRACE_CAP];
