@@ -68,8 +68,8 @@ struct Smem {
     static constexpr int OFF_BAR = OFF_KV + NSTAGE * KV_BYTES;
     // barrier indices
     static constexpr int B_KV_FULL = 0, B_KV_EMPTY = NSTAGE, B_ITEM_FULL = 2 * NSTAGE, B_ITEM_EMPTY = B_ITEM_FULL + 2,
-                         B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 2, B_S_FULL = B_Q_EMPTY + 2,
-                         B_P_FULL = B_S_FULL + 2, B_PV_DONE = B_P_FULL + 2, B_EPI_A = B_PV_DONE + 2,
+                         B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 2, B_S_FULL = B_Q_EMPTY + 2,   // [stream][half]
+                         B_P_FULL = B_S_FULL + 4, B_PV_DONE = B_P_FULL + 4, B_EPI_A = B_PV_DONE + 4,
                          B_EPI_B = B_EPI_A + 1, B_EPI_C = B_EPI_B + 1, B_EPI_D = B_EPI_C + 1, B_ZFILL = B_EPI_D + 1, NBAR = B_ZFILL + 1;
     static constexpr int OFF_ITEMS = OFF_BAR + ((NBAR * 8 + 15) / 16) * 16;
     static constexpr int OFF_ML = OFF_ITEMS + 2 * (int)sizeof(Item);    // (m, l) of stream 1, 128 rows
@@ -352,11 +352,15 @@ __device__ __forceinline__ void qload_warp(const AttnParams& p, const CUtensorMa
 }
 
 // ------------------------------------------------------------------------------------------------
-// warps 10, 11: MMA issuers (a5, a7), one per softmax stream s.  TMEM columns: S_s = [128 s, 128 s + 128),
-// O_s = [256 + 128 s, .. + D).  P_s (bf16, two per column) overwrites the first 64 columns of S_s.
-// Per stream the chain is  QK(s,0) | wait P -> PV(s,j) + QK(s,j+1) in one issue block | ...
-// The two issuers are independent, so a stream's PV/QK go out the moment its P is ready even while the
-// other stream's MMAs are queued; the in-order tensor pipe interleaves them.  K/V ring stages are consumed
+// warps 10, 11: MMA issuers (a5, a7), one per softmax stream s.
+// A 128-column kv tile is processed as two HALVES of 64 columns with their own S/P buffers in TMEM:
+//   S_s,h = columns [128 s + 64 h, +64),  P_s,h (bf16, two per column) over the first 32 of them,
+//   O_s   = columns [256 + 128 s, +D).
+// Per stream the steps alternate A B A B ...; step k waits for P of its half, issues
+//   O_s += P_s,h V(tile, half h)   and then   S_s,h = Q K(next tile, half h)^T
+// so the softmax warpgroup always has the other half's logits waiting: it never idles on the tensor pipe.
+// (Only the last kv tile of a context can lack half B: fewer than 65 valid columns.)
+// The two issuers are independent; the in-order tensor pipe interleaves them.  K/V ring stages are consumed
 // in the order of OpWalk: each issuer walks the whole order, acts on its own ops and skips the other's.
 // KV_EMPTY and Q_EMPTY expect two arrivals: SHARED stages / SPLIT q tiles are read by both issuers (one
 // commit each), SPLIT stages / SHARED q tiles by one issuer (which commits twice).
@@ -366,7 +370,7 @@ struct MmaState {
     uint32_t sbase, tmem;
     uint64_t q_desc0, k_desc0, v_desc0;
     uint32_t stage, phase;            // next ring position and its parity
-    uint32_t pv_par;                  // parity of the next P_FULL wait
+    uint32_t p_par0, p_par1;          // parity of the next P_FULL wait, half A / B
     uint32_t zf_par;                  // parity of the next ZFILL wait (SHARED tail tiles)
     volatile uint32_t* abort_flag;
     __device__ __forceinline__ uint32_t bar(int i) const { return sbase + (uint32_t)(Smem<D>::OFF_BAR + i * 8); }
@@ -392,51 +396,67 @@ __device__ __forceinline__ void zero_v_tail(uint32_t v_addr, int nv, int ncols, 
     __syncwarp();
 }
 
-// One issue block of stream s:  [O_s (+)= P_s V(tile_v)]  then  [S_s = Q K(tile_k)^T].
-// do_pv / do_qk select the halves; rel = commits per consumed stage (2 = sole reader, 1 = shared with the other issuer).
+// valid (16-padded) columns of half h of kv tile `tile`; <= 0: the half does not exist
+__device__ __forceinline__ int half_cols(int c, int tile, int h) {
+    int nv = c - tile * BN;
+    nv = nv > BN ? BN : nv;
+    const int nc = ((nv + 15) & ~15) - h * 64;
+    return nc > 64 ? 64 : nc;
+}
+
+// One step of stream s on half h:  [O_s (+)= P_s,h V]  then  [S_s,h = Q K^T].
+// pv_cols / qk_cols = padded columns of the half (0: skip that part); rel_* = KV_EMPTY commits after the part
+// (0 none, 1 stage shared with the other issuer, 2 sole reader); q_rel = Q_EMPTY commits after the QK.
 template <int D>
-__device__ __forceinline__ void mma_block(MmaState<D>& st, int s, int c, bool do_pv, int tile_v, bool first_pv, uint32_t stage_v,
-                                          bool do_qk, int tile_k, uint32_t stage_k, uint32_t qs, int rel, int q_rel) {
+__device__ __forceinline__ void half_step(MmaState<D>& st, int s, int h, int pv_cols, bool first_pv, uint32_t stage_v, int rel_v,
+                                          int qk_cols, uint32_t stage_k, uint32_t qs, int rel_k, int q_rel) {
     using L = Smem<D>;
-    int nvv = c - tile_v * BN; nvv = nvv > BN ? BN : nvv;
-    int nvk = c - tile_k * BN; nvk = nvk > BN ? BN : nvk;
-    const uint32_t ncols_v = (uint32_t)((nvv + 15) & ~15), ncols_k = (uint32_t)((nvk + 15) & ~15);
-    if (do_pv) {
-        ptx::mbar_wait(st.bar(L::B_P_FULL + s), st.pv_par, st.abort_flag);
-        st.pv_par ^= 1u;
+    if (pv_cols > 0) {
+        uint32_t& par = h ? st.p_par1 : st.p_par0;
+        ptx::mbar_wait(st.bar(L::B_P_FULL + 2 * s + h), par, st.abort_flag);
+        par ^= 1u;
     }
     ptx::tc_fence_after();
     if (ptx::elect_one()) {
-        if (do_pv) {
-            const uint64_t b_desc = st.v_desc0 + (uint64_t)(stage_v * (L::KV_BYTES >> 4));
+        const uint32_t sh_tmem = st.tmem + (uint32_t)(s * 128 + h * 64);          // S_s,h / P_s,h
+        if (pv_cols > 0) {
+            // K-steps of 16 kv rows = 2048 bytes of V; half h starts 64 rows in
+            const uint64_t b_desc = st.v_desc0 + (uint64_t)(stage_v * (L::KV_BYTES >> 4) + h * 512);
             const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
-            const uint32_t d_tmem = st.tmem + 256u + (uint32_t)s * 128u, a_tmem = st.tmem + (uint32_t)s * 128u;
-            if (ncols_v == BN) {                                  // K-steps of 16 kv rows = 2048 bytes of V
-                ptx::mma_ts_x4(d_tmem, a_tmem, b_desc, idesc, first_pv ? 0u : 1u, 128u);
-                ptx::mma_ts_x4(d_tmem, a_tmem + 32u, b_desc + 512u, idesc, 1u, 128u);
+            const uint32_t d_tmem = st.tmem + 256u + (uint32_t)s * 128u;
+            if (pv_cols == 64) {
+                ptx::mma_ts_x4(d_tmem, sh_tmem, b_desc, idesc, first_pv ? 0u : 1u, 128u);
             } else {
-                for (uint32_t ks = 0; ks < ncols_v / 16; ++ks)
-                    ptx::mma_ts(d_tmem, a_tmem + ks * 8u, b_desc + (uint64_t)(ks * 128u), idesc, (!first_pv || ks > 0) ? 1u : 0u);
+                for (int ks = 0; ks < pv_cols / 16; ++ks)
+                    ptx::mma_ts(d_tmem, sh_tmem + (uint32_t)(ks * 8), b_desc + (uint64_t)(ks * 128), idesc, (!first_pv || ks > 0) ? 1u : 0u);
             }
-            ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_v));
-            if (rel == 2) ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_v));
-            ptx::mma_commit(st.bar(L::B_PV_DONE + s));
+            for (int i = 0; i < rel_v; ++i) ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_v));
+            ptx::mma_commit(st.bar(L::B_PV_DONE + 2 * s + h));
         }
-        if (do_qk) {
+        if (qk_cols > 0) {
+            // K-steps of 16 elements = 32 bytes inside a 64-wide slab, second slab SLAB bytes further; half h of K = rows 64 h ..
             const uint64_t a_desc = st.q_desc0 + (uint64_t)(qs * (L::Q_BYTES >> 4));
-            const uint64_t b_desc = st.k_desc0 + (uint64_t)(stage_k * (L::KV_BYTES >> 4));
-            const uint32_t idesc = ptx::idesc_bf16(BM, ncols_k, 0, 0);
-            const uint32_t d_tmem = st.tmem + (uint32_t)s * 128u;
-            // K-steps of 16 elements = 32 bytes inside a 64-wide slab; the second slab is SLAB bytes further
-            ptx::mma_ss_x4(d_tmem, a_desc, b_desc, idesc, 0u, 2u);
-            if (D == 128) ptx::mma_ss_x4(d_tmem, a_desc + (SLAB >> 4), b_desc + (SLAB >> 4), idesc, 1u, 2u);
-            ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_k));
-            if (rel == 2) ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_k));
-            ptx::mma_commit(st.bar(L::B_S_FULL + s));
+            const uint64_t b_desc = st.k_desc0 + (uint64_t)(stage_k * (L::KV_BYTES >> 4) + h * 512);
+            const uint32_t idesc = ptx::idesc_bf16(BM, (uint32_t)qk_cols, 0, 0);
+            ptx::mma_ss_x4(sh_tmem, a_desc, b_desc, idesc, 0u, 2u);
+            if (D == 128) ptx::mma_ss_x4(sh_tmem, a_desc + (SLAB >> 4), b_desc + (SLAB >> 4), idesc, 1u, 2u);
+            for (int i = 0; i < rel_k; ++i) ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_k));
+            ptx::mma_commit(st.bar(L::B_S_FULL + 2 * s + h));
             for (int i = 0; i < q_rel; ++i) ptx::mma_commit(st.bar(L::B_Q_EMPTY + qs));
         }
     }
     __syncwarp();
+}
+
+// all steps of stream s on kv tile `tile` (PV) and `next` (QK; next < 0: none).  rel = 1 (SHARED) or 2 (SPLIT);
+// q_rel = Q_EMPTY commits owed when `next` is the stream's last tile.
+template <int D>
+__device__ __forceinline__ void tile_steps(MmaState<D>& st, int s, int c, int tile, bool first, uint32_t sv, int next, uint32_t sk,
+                                           uint32_t qs, int rel, int q_rel) {
+    const int pa = tile >= 0 ? half_cols(c, tile, 0) : 0, pb = tile >= 0 ? half_cols(c, tile, 1) : 0;
+    const int qa = next >= 0 ? half_cols(c, next, 0) : 0, qb = next >= 0 ? half_cols(c, next, 1) : 0;
+    half_step<D>(st, s, 0, pa, first, sv, pb > 0 ? 0 : rel, qa, sk, qs, qb > 0 ? 0 : rel, qb > 0 ? 0 : q_rel);
+    if (pb > 0 || qb > 0) half_step<D>(st, s, 1, pb > 0 ? pb : 0, false, sv, rel, qb > 0 ? qb : 0, sk, qs, rel, q_rel);
 }
 
 template <int D>
@@ -448,7 +468,7 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
     st.q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);        // K-major operands (Q, K)
     st.k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, 1024);
     st.v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, SLAB, 1024);     // MN-major operand (V)
-    st.stage = 0; st.phase = 0; st.pv_par = 0; st.zf_par = 0;
+    st.stage = 0; st.phase = 0; st.p_par0 = 0; st.p_par1 = 0; st.zf_par = 0;
     uint32_t icount = 0, qcount = 0;
     while (true) {
         if (*abort_flag) break;
@@ -463,11 +483,11 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
                 const uint32_t qc = qcount + (uint32_t)s, qs = qc & 1u;
                 ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qc >> 1) & 1u, abort_flag);
                 uint32_t sk = st.acquire();
-                mma_block<D>(st, s, c, false, kv0, false, 0u, true, kv0, sk, qs, 1, n == 1 ? 2 : 0);
+                tile_steps<D>(st, s, c, -1, false, 0u, kv0, sk, qs, 1, n == 1 ? 2 : 0);
                 for (int j = 0; j < n; ++j) {
                     const bool more = j + 1 < n;
                     const uint32_t sv = st.acquire();
-                    int nv = c - (kv0 + j) * BN;
+                    const int nv = c - (kv0 + j) * BN;
                     if (nv < BN && (nv & 15)) {              // tail tile: issuer 0 zero-fills, issuer 1 waits for it
                         if (s == 0) {
                             zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
@@ -478,7 +498,7 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
                         st.zf_par ^= 1u;
                     }
                     if (more) sk = st.acquire();
-                    mma_block<D>(st, s, c, true, kv0 + j, j == 0, sv, more, kv0 + j + 1, sk, qs, 1, (more && j + 2 == n) ? 2 : 0);
+                    tile_steps<D>(st, s, c, kv0 + j, j == 0, sv, more ? kv0 + j + 1 : -1, sk, qs, 1, (more && j + 2 == n) ? 2 : 0);
                 }
                 qcount += 2;
             } else {
@@ -490,32 +510,21 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
                 uint32_t sk = 0, sv = 0;
                 if (s == 0) sk = st.acquire(); else st.skip();
                 if (n1 > 0) { if (s == 1) sk = st.acquire(); else st.skip(); }
-                if (ns > 0) mma_block<D>(st, s, c, false, 0, false, 0u, true, kv0 + s, sk, qs, 2, ns == 1 ? 1 : 0);
+                if (ns > 0) tile_steps<D>(st, s, c, -1, false, 0u, kv0 + s, sk, qs, 2, ns == 1 ? 1 : 0);
                 else if (lane == 0) ptx::mbar_arrive(st.bar(L::B_Q_EMPTY + qs));      // nothing to read: release the q tile
                 for (int i = 0; i < n0; ++i) {
-                    // stream 0's pair of stages
-                    bool more = i + 1 < n0;
-                    if (s == 0) {
-                        sv = st.acquire();
-                        const int tile = kv0 + 2 * i;
-                        const int nv = c - tile * BN;
-                        if (nv < BN && (nv & 15)) zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
-                        if (more) sk = st.acquire();
-                        mma_block<D>(st, 0, c, true, tile, i == 0, sv, more, tile + 2, sk, qs, 2, (more && i + 2 == n0) ? 1 : 0);
-                    } else {
-                        st.skip();
-                        if (more) st.skip();
-                    }
-                    // stream 1's pair of stages
-                    if (i < n1) {
-                        more = i + 1 < n1;
-                        if (s == 1) {
+#pragma unroll
+                    for (int x = 0; x < 2; ++x) {            // stream x's pair of stages: V(x, i) [K(x, i+1)]
+                        const int nx = x ? n1 : n0;
+                        if (i >= nx) continue;
+                        const bool more = i + 1 < nx;
+                        if (s == x) {
                             sv = st.acquire();
-                            const int tile = kv0 + 2 * i + 1;
+                            const int tile = kv0 + 2 * i + x;
                             const int nv = c - tile * BN;
                             if (nv < BN && (nv & 15)) zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
                             if (more) sk = st.acquire();
-                            mma_block<D>(st, 1, c, true, tile, i == 0, sv, more, tile + 2, sk, qs, 2, (more && i + 2 == n1) ? 1 : 0);
+                            tile_steps<D>(st, s, c, tile, i == 0, sv, more ? tile + 2 : -1, sk, qs, 2, (more && i + 2 == nx) ? 1 : 0);
                         } else {
                             st.skip();
                             if (more) st.skip();
@@ -547,26 +556,28 @@ __device__ __forceinline__ float ex2_poly(float x) {
     return __int_as_float(__float_as_int(y) + (__float_as_int(t) << 23));
 }
 
-// One 128-column tile of one row: returns alpha (the factor by which O and l shrink; 1 if the
-// reference maximum m_ref stays).  m_ref is in log2 units and is only raised when the tile maximum
+// One 64-column half tile of one row: returns alpha (the factor by which O and l shrink; 1 if the
+// reference maximum m_ref stays).  m_ref is in log2 units and is only raised when the half's maximum
 // exceeds it by more than LAZY_T, so p = 2^(x - m_ref) <= 2^LAZY_T: exact in range for bf16 / fp32.
+// P (bf16 pairs) overwrites the first 32 columns of the half's S buffer.
 template <bool MASK, bool NEG>
-__device__ __forceinline__ float softmax_tile(uint32_t s_taddr, int nv, float scale_log2, float& m_ref, float& l) {
-    uint32_t r[4][32];
+__device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float scale_log2, float& m_ref, float& l) {
+    uint32_t r[2][32];
 #pragma unroll
-    for (int c = 0; c < 4; ++c) ptx::tmem_ld32(s_taddr + (uint32_t)(c * 32), r[c]);
+    for (int c = 0; c < 2; ++c) ptx::tmem_ld32(s_taddr + (uint32_t)(c * 32), r[c]);
     ptx::tmem_wait_ld();
     float mx4[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
         float a = -INFINITY;
 #pragma unroll
-        for (int i = 0; i < 32; i += 2) {
-            float v0 = __uint_as_float(r[c][i]), v1 = __uint_as_float(r[c][i + 1]);
+        for (int i = 0; i < 16; i += 2) {
+            const int col = c * 16 + i;
+            float v0 = __uint_as_float(r[col >> 5][col & 31]), v1 = __uint_as_float(r[col >> 5][(col & 31) + 1]);
             if (NEG) { v0 = -v0; v1 = -v1; }
             if (MASK) {
-                if (c * 32 + i >= nv) v0 = -INFINITY;
-                if (c * 32 + i + 1 >= nv) v1 = -INFINITY;
+                if (col >= nv) v0 = -INFINITY;
+                if (col + 1 >= nv) v1 = -INFINITY;
             }
             a = fmaxf(a, fmaxf(v0, v1));
         }
@@ -579,7 +590,7 @@ __device__ __forceinline__ float softmax_tile(uint32_t s_taddr, int nv, float sc
     const float neg = -m_new;
     float sum0 = 0.f, sum1 = 0.f;
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
+    for (int c = 0; c < 2; ++c) {
         uint32_t pk[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
@@ -666,7 +677,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
     const uint32_t o_other = tmem + lane_base + 256u + (uint32_t)(s ^ 1) * 128u;
     float2* ml_x = reinterpret_cast<float2*>(smem + L::OFF_ML);
     volatile int* last_flag = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 8);
-    uint32_t icount = 0, tcount = 0, ecount = 0, ccount = 0;
+    uint32_t icount = 0, hcount0 = 0, hcount1 = 0, pv0 = 0, pv1 = 0, ecount = 0, ccount = 0;
     TRACE_NS(40);
     TRACE_EV(36);
     while (true) {
@@ -682,46 +693,62 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         const int rows_valid = (shared && s == 1) ? it.rows1 : it.rows0;
         const bool warp_active = wg_warp * 32 < rows_valid;
         float m = -INFINITY, l = 0.f;
+        uint32_t steps = 0;                                    // half tiles of this item handed to the issuer
         for (int i = 0; i < ns; ++i) {
             if (*abort_flag) break;
-            TRACE_EV(20 + s);
-            ptx::mbar_wait(bar(L::B_S_FULL + s), tcount & 1u, abort_flag);
-            TRACE_EV(22 + s);
-            ptx::tc_fence_after();
             const int tile = shared ? it.kv0 + i : it.kv0 + 2 * i + s;
-            int nv = it.c - tile * BN;
-            nv = nv > BN ? BN : nv;
-            if (warp_active) {
-                float alpha;
-                if (p.scale_log2 >= 0.f) {
-                    if (nv == BN) alpha = softmax_tile<false, false>(s_taddr, nv, p.scale_log2, m, l);
-                    else alpha = softmax_tile<true, false>(s_taddr, nv, p.scale_log2, m, l);
-                } else {
-                    if (nv == BN) alpha = softmax_tile<false, true>(s_taddr, nv, p.scale_log2, m, l);
-                    else alpha = softmax_tile<true, true>(s_taddr, nv, p.scale_log2, m, l);
-                }
-                // S_FULL(i) was committed after PV(i-1) of this stream: O is quiescent here
-                if (i > 0 && __any_sync(FULL, alpha != 1.f)) {
+            int nvt = it.c - tile * BN;
+            nvt = nvt > BN ? BN : nvt;
 #pragma unroll
-                    for (int c = 0; c < D / 32; ++c) {
-                        uint32_t o[32];
-                        ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
-                        ptx::tmem_wait_ld();
-#pragma unroll
-                        for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
-                        ptx::tmem_st32(o_taddr + (uint32_t)(c * 32), o);
+            for (int h = 0; h < 2; ++h) {
+                const int nv = nvt - h * 64 > 64 ? 64 : nvt - h * 64;
+                if (nv <= 0) continue;                       // the context's last tile may lack half B
+                uint32_t& hcnt = h ? hcount1 : hcount0;
+                TRACE_EV(20 + s);
+                ptx::mbar_wait(bar(L::B_S_FULL + 2 * s + h), hcnt & 1u, abort_flag);
+                TRACE_EV(22 + s);
+                ptx::tc_fence_after();
+                ++hcnt;
+                if (warp_active) {
+                    const uint32_t sh = s_taddr + (uint32_t)(h * 64);
+                    float alpha;
+                    if (p.scale_log2 >= 0.f) {
+                        if (nv == 64) alpha = softmax_half<false, false>(sh, nv, p.scale_log2, m, l);
+                        else alpha = softmax_half<true, false>(sh, nv, p.scale_log2, m, l);
+                    } else {
+                        if (nv == 64) alpha = softmax_half<false, true>(sh, nv, p.scale_log2, m, l);
+                        else alpha = softmax_half<true, true>(sh, nv, p.scale_log2, m, l);
                     }
+                    if (steps > 0 && __any_sync(FULL, alpha != 1.f)) {
+                        // rare (lazy reference maximum): every PV handed over so far must have landed in O first.
+                        // Per half at most the latest one is still in flight (the S_FULL just seen was committed
+                        // behind the one before), so each parity wait is unambiguous.
+                        ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s), (pv0 - 1u) & 1u, abort_flag);
+                        ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s + 1), (pv1 - 1u) & 1u, abort_flag);
+                        ptx::tc_fence_after();
+#pragma unroll
+                        for (int c = 0; c < D / 32; ++c) {
+                            uint32_t o[32];
+                            ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
+                            ptx::tmem_wait_ld();
+#pragma unroll
+                            for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
+                            ptx::tmem_st32(o_taddr + (uint32_t)(c * 32), o);
+                        }
+                    }
+                    ptx::tmem_wait_st();
                 }
-                ptx::tmem_wait_st();
+                ptx::tc_fence_before();
+                __syncwarp();
+                TRACE_EV(24 + s);
+                if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL + 2 * s + h));
+                ++steps;
+                if (h) ++pv1; else ++pv0;
             }
-            ptx::tc_fence_before();
-            __syncwarp();
-            TRACE_EV(24 + s);
-            if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL + s));
-            ++tcount;
         }
-        if (ns > 0) {
-            ptx::mbar_wait(bar(L::B_PV_DONE + s), (tcount - 1u) & 1u, abort_flag);
+        if (steps > 0) {
+            ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s), (pv0 - 1u) & 1u, abort_flag);
+            ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s + 1), (pv1 - 1u) & 1u, abort_flag);
             ptx::tc_fence_after();
         }
         // ---------------- epilogue
@@ -870,9 +897,11 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
             ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 11);  // 2 MMA issuers + loader warp + 8 softmax warps
             ptx::mbar_init(bar(L::B_Q_FULL + s), 1);
             ptx::mbar_init(bar(L::B_Q_EMPTY + s), 2);
-            ptx::mbar_init(bar(L::B_S_FULL + s), 1);
-            ptx::mbar_init(bar(L::B_P_FULL + s), 4);
-            ptx::mbar_init(bar(L::B_PV_DONE + s), 1);
+            for (int h = 0; h < 2; ++h) {
+                ptx::mbar_init(bar(L::B_S_FULL + 2 * s + h), 1);
+                ptx::mbar_init(bar(L::B_P_FULL + 2 * s + h), 4);
+                ptx::mbar_init(bar(L::B_PV_DONE + 2 * s + h), 1);
+            }
         }
         ptx::mbar_init(bar(L::B_EPI_A), 128);
         ptx::mbar_init(bar(L::B_EPI_B), 128);
