@@ -587,27 +587,29 @@ __device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float sc
     const bool grow = mx > m_ref + LAZY_T;
     const float m_new = grow ? mx : m_ref;
     const float alpha = grow ? ptx::ex2(m_ref - m_new) : 1.f;
-    const float neg = -m_new;
-    float sum0 = 0.f, sum1 = 0.f;
+    // packed fp32x2 arithmetic (FFMA2 / FADD2): one instruction per two columns
+    const float2 sc2 = make_float2(scale_log2, scale_log2), ng2 = make_float2(-m_new, -m_new);
+    float2 sum_a = make_float2(0.f, 0.f), sum_b = make_float2(0.f, 0.f);
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
         uint32_t pk[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-            const float x0 = fmaf(__uint_as_float(r[c][2 * i]), scale_log2, neg);
-            const float x1 = fmaf(__uint_as_float(r[c][2 * i + 1]), scale_log2, neg);
-            float p0 = ((2 * i) & 7) < SANGAM_POLY_EXP ? ex2_poly(x0) : ptx::ex2(x0);
-            float p1 = ((2 * i + 1) & 7) < SANGAM_POLY_EXP ? ex2_poly(x1) : ptx::ex2(x1);
+            const float2 x = __ffma2_rn(make_float2(__uint_as_float(r[c][2 * i]), __uint_as_float(r[c][2 * i + 1])), sc2, ng2);
+            float2 pp;
+            pp.x = ((2 * i) & 7) < SANGAM_POLY_EXP ? ex2_poly(x.x) : ptx::ex2(x.x);
+            pp.y = ((2 * i + 1) & 7) < SANGAM_POLY_EXP ? ex2_poly(x.y) : ptx::ex2(x.y);
             if (MASK) {
-                if (c * 32 + 2 * i >= nv) p0 = 0.f;
-                if (c * 32 + 2 * i + 1 >= nv) p1 = 0.f;
+                if (c * 32 + 2 * i >= nv) pp.x = 0.f;
+                if (c * 32 + 2 * i + 1 >= nv) pp.y = 0.f;
             }
-            sum0 += p0;
-            sum1 += p1;
-            pk[i] = ptx::pack_bf16(p0, p1);
+            if (i & 1) sum_b = __fadd2_rn(sum_b, pp); else sum_a = __fadd2_rn(sum_a, pp);
+            pk[i] = ptx::pack_bf16(pp.x, pp.y);
         }
         ptx::tmem_st16(s_taddr + (uint32_t)(c * 16), pk);
     }
+    const float2 sum2 = __fadd2_rn(sum_a, sum_b);
+    const float sum0 = sum2.x, sum1 = sum2.y;
     l = l * alpha + (sum0 + sum1);
     m_ref = m_new;
     return alpha;
@@ -693,6 +695,9 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         const int rows_valid = (shared && s == 1) ? it.rows1 : it.rows0;
         const bool warp_active = wg_warp * 32 < rows_valid;
         float m = -INFINITY, l = 0.f;
+#ifdef SANGAM_DESYNC_NS
+        if (s == 1) __nanosleep(SANGAM_DESYNC_NS);           // experiment: start stream 1 out of phase with stream 0
+#endif
         uint32_t steps = 0;                                    // half tiles of this item handed to the issuer
         for (int i = 0; i < ns; ++i) {
             if (*abort_flag) break;
