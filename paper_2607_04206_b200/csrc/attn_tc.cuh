@@ -80,64 +80,68 @@ struct Smem {
 static_assert(sizeof(Item) == 64, "Item is 64 bytes");
 static_assert(Smem<128>::ALLOC <= 232448, "shared memory budget (227 KB)");
 
+// floor(a * b / d) for non-negative a, b and d > 0: 32-bit division whenever the product fits (64-bit division is slow)
+__device__ __forceinline__ int mul_div(int a, int b, int d) {
+    const uint64_t prod = (uint64_t)(uint32_t)a * (uint32_t)b;
+    return (prod >> 32) == 0 ? (int)((uint32_t)prod / (uint32_t)d) : (int)(prod / (uint32_t)d);
+}
+__device__ __forceinline__ int mul_div_ceil(int64_t a, int b, int d) {   // ceil(a * b / d), a < 2^31
+    const uint64_t prod = (uint64_t)a * (uint32_t)b + (uint32_t)d - 1u;
+    return (prod >> 32) == 0 ? (int)((uint32_t)prod / (uint32_t)d) : (int)(prod / (uint32_t)d);
+}
+
 struct ReqInfo {
     int q0, qn, c, np, tiles_u, units;
 };
 
-__device__ __forceinline__ ReqInfo req_info(const AttnParams& p, int r) {
-    ReqInfo x;
-    x.q0 = __ldg(p.cu_q_lens + r);
-    int qn = __ldg(p.cu_q_lens + r + 1) - x.q0;
-    if (qn < 0) qn = 0;
-    int c = __ldg(p.ctx_lens + r);
-    if (c < 0) c = 0;
-    if ((c + SANGAM_PAGE - 1) / SANGAM_PAGE > p.W) { raise_flag(p.flags, DEV_CTX_TOO_LONG); c = 0; }
-    x.c = c;
-    x.qn = qn;
-    x.np = (qn + 2 * p.tpt - 1) / (2 * p.tpt);      // a q tile holds tpt = 128 / G whole tokens (all G heads of each)
-    const int nkv = (c + BN - 1) / BN;
-    x.tiles_u = nkv > 0 ? nkv : 1;
-    x.units = p.Hkv * x.np;
-    return x;
-}
-
-// The order in which the MMA warp consumes K/V tiles of one item; the producer loads in the same
-// order.  Op k = 0, 1: QK of stream k, tile index 0.  Then rounds j = 0, 1, ...:
-//   PV(0, j), QK(0, j+1), PV(1, j), QK(1, j+1).
-// SHARED: stream 0 acquires a ring stage, stream 1 reuses and releases it.  SPLIT: every op has its own.
-struct Op {
-    int is_pv, s, i, tile, acquire, release;
-};
-struct OpWalk {
-    int shared, kv0, n0, n1, nops, k;
-    __device__ __forceinline__ OpWalk(const Item& it) {
-        const int n = it.kv1 - it.kv0;
-        shared = it.rows1 > 0;
-        kv0 = it.kv0;
-        n0 = shared ? n : (n + 1) / 2;
-        n1 = shared ? n : n / 2;
-        nops = n > 0 ? 2 + 4 * n0 : 0;
-        k = 0;
+// Request metadata of the batch, read once: lane r of the producer warp keeps request r (< 32) in registers
+// and every later look-up is a shuffle.  (With 227 KB of shared memory the L1 holds next to nothing, so a
+// repeated global read costs an L2 round trip each time.)  Requests >= 32 are read from global memory.
+struct ReqCache {
+    int q0, qn, c;      // of request `lane`
+    __device__ __forceinline__ static void load(const AttnParams& p, int r, int& q0, int& qn, int& c) {
+        q0 = __ldg(p.cu_q_lens + r);
+        qn = __ldg(p.cu_q_lens + r + 1) - q0;
+        if (qn < 0) qn = 0;
+        c = __ldg(p.ctx_lens + r);
+        if (c < 0) c = 0;
+        if ((c + SANGAM_PAGE - 1) / SANGAM_PAGE > p.W) { raise_flag(p.flags, DEV_CTX_TOO_LONG); c = 0; }
     }
-    __device__ __forceinline__ bool next(Op& op) {
-        while (k < nops) {
-            const int kk = k++;
-            if (kk < 2) { op.is_pv = 0; op.s = kk; op.i = 0; }
-            else {
-                const int j = (kk - 2) >> 2, ph = (kk - 2) & 3;
-                op.is_pv = (ph & 1) ^ 1;
-                op.s = ph >> 1;
-                op.i = op.is_pv ? j : j + 1;
-            }
-            if (op.i >= (op.s ? n1 : n0)) continue;
-            op.tile = shared ? kv0 + op.i : kv0 + 2 * op.i + op.s;
-            op.acquire = shared ? (op.s == 0) : 1;
-            op.release = shared ? (op.s == 1) : 1;
-            return true;
+    __device__ __forceinline__ void init(const AttnParams& p, int lane) {
+        q0 = 0; qn = 0; c = 0;
+        if (lane < p.batch) load(p, lane, q0, qn, c);
+    }
+    __device__ __forceinline__ static ReqInfo derive(const AttnParams& p, int q0_, int qn_, int c_) {
+        ReqInfo x;
+        x.q0 = q0_; x.qn = qn_; x.c = c_;
+        x.np = (qn_ + 2 * p.tpt - 1) / (2 * p.tpt);      // a q tile holds tpt = 128 / G whole tokens (all G heads of each)
+        const int nkv = (c_ + BN - 1) / BN;
+        x.tiles_u = nkv > 0 ? nkv : 1;
+        x.units = p.Hkv * x.np;
+        return x;
+    }
+    // warp-uniform r: all 32 lanes call
+    __device__ __forceinline__ ReqInfo get(const AttnParams& p, int r) const {
+        int a, b, d;
+        if (r < 32) {
+            a = __shfl_sync(0xffffffffu, q0, r); b = __shfl_sync(0xffffffffu, qn, r); d = __shfl_sync(0xffffffffu, c, r);
+        } else {
+            load(p, r, a, b, d);
         }
-        return false;
+        return derive(p, a, b, d);
+    }
+    // per-lane r = base + lane (r < batch)
+    __device__ __forceinline__ ReqInfo get_lane(const AttnParams& p, int base, int lane) const {
+        if (base == 0) return derive(p, q0, qn, c);
+        int a, b, d;
+        load(p, base + lane, a, b, d);
+        return derive(p, a, b, d);
     }
 };
+
+// Order in which the K/V tiles of one item pass through the shared-memory ring (producer loads, issuers consume):
+//   K(0) .. K(lead-1),  then for j = 0, 1, ..:  V(j), K(j + lead)        lead = 1 (SHARED) or 2 (SPLIT)
+// SHARED: both issuers read every stage.  SPLIT: tile j belongs to stream j & 1, the other issuer skips it.
 
 // ------------------------------------------------------------------------------------------------
 // warp 8: device-side plan (a3) + TMA page gather (a4)
@@ -149,13 +153,19 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
     const unsigned FULL = 0xffffffffu;
     const int G_ctas = gridDim.x, b = blockIdx.x, R = p.batch;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    TRACE_EV(50);
+    ReqCache rc;
+    rc.init(p, lane);
+    TRACE_EV(59);
 
     // totals over the batch: units U and kv tiles T
     int U = 0, T = 0;
-    for (int r = lane; r < R; r += 32) {
-        const ReqInfo x = req_info(p, r);
-        U += x.units;
-        T += x.units * x.tiles_u;
+    for (int base = 0; base < R; base += 32) {
+        if (base + lane < R) {
+            const ReqInfo x = rc.get_lane(p, base, lane);
+            U += x.units;
+            T += x.units * x.tiles_u;
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -163,23 +173,25 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
         T += __shfl_xor_sync(FULL, T, o);
     }
     const bool dynamic = U >= DYN_UNITS_PER_CTA * G_ctas;
+    TRACE_EV(51);
 
     // walking state
     int r_cur = 0, ubase = 0, u_in_r = 0, kvoff = 0, remaining = 0, tile_base = 0, Geff = 1;
-    ReqInfo cur;
-    cur.units = 0; cur.tiles_u = 1; cur.np = 1; cur.c = 0; cur.q0 = 0; cur.qn = 0;
-    if (R > 0) cur = req_info(p, 0);
+    ReqInfo cur = ReqCache::derive(p, 0, 0, 0);
+    cur.units = 0;
+    if (R > 0) cur = rc.get(p, 0);
+    TRACE_EV(55);
     if (!dynamic && T > 0) {
         Geff = G_ctas < T ? G_ctas : T;
         if (b < Geff) {
-            const int t0 = (int)(((int64_t)b * T) / Geff), t1 = (int)(((int64_t)(b + 1) * T) / Geff);
+            const int t0 = mul_div(b, T, Geff), t1 = mul_div(b + 1, T, Geff);
             remaining = t1 - t0;
+            TRACE_EV(56);
             // locate the request holding flattened tile t0 (chunked warp scan over requests)
             int acc = 0, found = -1;
             for (int base = 0; base < R && found < 0; base += 32) {
-                const int r = base + lane;
                 int tl = 0;
-                if (r < R) { const ReqInfo x = req_info(p, r); tl = x.units * x.tiles_u; }
+                if (base + lane < R) { const ReqInfo x = rc.get_lane(p, base, lane); tl = x.units * x.tiles_u; }
                 int incl = tl;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -195,9 +207,10 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                     acc += __shfl_sync(FULL, incl, 31);
                 }
             }
+            TRACE_EV(57);
             r_cur = found < 0 ? R : found;
             if (r_cur < R) {
-                cur = req_info(p, r_cur);
+                cur = rc.get(p, r_cur);
                 const int pos = t0 - tile_base;
                 u_in_r = pos / cur.tiles_u;
                 kvoff = pos - u_in_r * cur.tiles_u;
@@ -206,13 +219,15 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
             }
         }
     }
+    TRACE_EV(52);
 
-    uint32_t kvi = 0, icount = 0;
+    uint32_t stage = 0, phase = 0, icount = 0;       // next K/V ring position and its parity
     while (true) {
         if (*abort_flag) break;
         Item it;
         it.valid = 0; it.r = 0; it.g = 0; it.tok0 = 0; it.rows0 = 0; it.rows1 = 0; it.q_start = 0; it.c = 0;
         it.kv0 = 0; it.kv1 = 0; it.part_slot = -1; it.b_head = 0; it.npieces = 1; it.pad0 = 0; it.pad1 = 0; it.pad2 = 0;
+        ReqInfo ri = cur;                               // the request of this item
         if (dynamic) {
             int u = 0;
             if (lane == 0) u = atomicAdd(p.sched, 1);
@@ -221,13 +236,14 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                 while (r_cur < R && u >= ubase + cur.units) {
                     ubase += cur.units;
                     ++r_cur;
-                    if (r_cur < R) cur = req_info(p, r_cur);
+                    if (r_cur < R) cur = rc.get(p, r_cur);
                 }
                 if (r_cur < R) {
                     const int ul = u - ubase;
                     it.valid = 1; it.r = r_cur; it.g = ul / cur.np;
                     it.tok0 = (ul - it.g * cur.np) * 2 * p.tpt;
                     it.kv0 = 0; it.kv1 = cur.tiles_u;
+                    ri = cur;
                 }
             }
         } else if (remaining > 0 && r_cur < R) {
@@ -235,12 +251,13 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
             it.valid = 1; it.r = r_cur; it.g = u_in_r / cur.np;
             it.tok0 = (u_in_r - it.g * cur.np) * 2 * p.tpt;
             it.kv0 = kvoff; it.kv1 = kvoff + take;
+            ri = cur;
             if (!(it.kv0 == 0 && it.kv1 == cur.tiles_u)) {
                 // a piece of a unit split across CTAs: CTA x holds flattened tiles [floor(xT/Geff), floor((x+1)T/Geff))
                 it.part_slot = 2 * b + (it.kv0 == 0 ? 1 : 0);
-                const int64_t ut0 = (int64_t)tile_base + (int64_t)u_in_r * cur.tiles_u, ut1 = ut0 + cur.tiles_u;
-                const int bh = (int)(((ut0 + 1) * Geff + T - 1) / T) - 1;
-                int bl = (int)((ut1 * Geff + T - 1) / T) - 1;
+                const int ut0 = tile_base + u_in_r * cur.tiles_u, ut1 = ut0 + cur.tiles_u;      // < T < 2^31
+                const int bh = mul_div_ceil(ut0 + 1, Geff, T) - 1;
+                int bl = mul_div_ceil(ut1, Geff, T) - 1;
                 bl = bl > Geff - 1 ? Geff - 1 : bl;
                 it.b_head = bh;
                 it.npieces = bl - bh + 1;
@@ -254,14 +271,12 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                     do {
                         tile_base += cur.units * cur.tiles_u;
                         ++r_cur;
-                        if (r_cur < R) cur = req_info(p, r_cur);
+                        if (r_cur < R) cur = rc.get(p, r_cur);
                     } while (r_cur < R && cur.units == 0);
                 }
             }
         }
         if (it.valid) {
-            ReqInfo ri = cur;
-            if (it.r != r_cur) ri = req_info(p, it.r);   // static walk may already have advanced
             const int left = ri.qn - it.tok0;
             it.rows0 = (left < p.tpt ? left : p.tpt) * p.G;
             it.rows1 = left > p.tpt ? (left - p.tpt < p.tpt ? left - p.tpt : p.tpt) * p.G : 0;
@@ -269,6 +284,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
             it.c = ri.c;
             if (ri.c == 0) { it.kv0 = 0; it.kv1 = 0; }
         }
+        TRACE_EV(58);
         // publish
         const uint32_t islot = icount & 1u;
         ptx::mbar_wait(bar(L::B_ITEM_EMPTY + islot), ((icount >> 1) & 1u) ^ 1u, abort_flag);
@@ -277,33 +293,49 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
             ptx::mbar_arrive(bar(L::B_ITEM_FULL + islot));
         }
         __syncwarp();
+        TRACE_EV(53);
         ++icount;
         if (!it.valid) break;
 
-        // K/V tile loads in the order the MMA warp consumes them (OpWalk)
-        const int pages_total = (it.c + SANGAM_PAGE - 1) / SANGAM_PAGE;
-        const int32_t* bt = p.block_table + (int64_t)it.r * p.W;
-        OpWalk walk(it);
-        Op op;
-        while (walk.next(op)) {
-            if (!op.acquire) continue;
-            if (*abort_flag) break;
-            const uint32_t stage = kvi % NSTAGE;
-            ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), ((kvi / NSTAGE) & 1u) ^ 1u, abort_flag);
-            int np = pages_total - op.tile * 8;
-            np = np > 8 ? 8 : np;
+        // K/V tile loads in ring order (see above).  The block-table entries of a tile serve its K and its V load
+        // and are fetched three tiles ahead: lane (2 pg + slab) keeps page pg of tiles j, j+1, j+2 in w0, w1, w2.
+        const int n = it.kv1 - it.kv0;
+        if (n > 0) {
+            const int pages_total = (it.c + SANGAM_PAGE - 1) / SANGAM_PAGE;
+            const int32_t* bt = p.block_table + (int64_t)it.r * p.W;
             constexpr int BOX_PER_PAGE = D / 64;
-            if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_KV_FULL + stage), (uint32_t)(np * SANGAM_PAGE * D * 2));
-            __syncwarp();
-            if (lane < np * BOX_PER_PAGE) {
-                const int pg = lane / BOX_PER_PAGE, slab = lane % BOX_PER_PAGE;
-                const int page = __ldg(bt + op.tile * 8 + pg);
-                if ((unsigned)page >= (unsigned)p.P) raise_flag(p.flags, DEV_BAD_PAGE);   // TMA zero-fills out of range
-                ptx::tma_load_2d(sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES + slab * SLAB + pg * 2048),
-                                 op.is_pv ? mapV : mapK, bar(L::B_KV_FULL + stage), slab * 64,
-                                 (page * p.Hkv + it.g) * SANGAM_PAGE);
+            const int pg = lane / BOX_PER_PAGE, slab = lane % BOX_PER_PAGE;
+            const int lead = it.rows1 > 0 ? 1 : 2;
+            auto ld_page = [&](int j) {                  // page pg of the item's j-th tile (0 if it does not exist)
+                const int tile = it.kv0 + j;
+                return (j < n && pg < 8 && pg < pages_total - tile * 8) ? __ldg(bt + tile * 8 + pg) : 0;
+            };
+            auto load_tile = [&](int j, int page, bool is_v) {
+                const int tile = it.kv0 + j;
+                ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), phase ^ 1u, abort_flag);
+                int np = pages_total - tile * 8;
+                np = np > 8 ? 8 : np;
+                if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_KV_FULL + stage), (uint32_t)(np * SANGAM_PAGE * D * 2));
+                __syncwarp();
+                if (pg < np) {
+                    if ((unsigned)page >= (unsigned)p.P) raise_flag(p.flags, DEV_BAD_PAGE);   // TMA zero-fills out of range
+                    ptx::tma_load_2d(sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES + slab * SLAB + pg * 2048),
+                                     is_v ? mapV : mapK, bar(L::B_KV_FULL + stage), slab * 64,
+                                     (page * p.Hkv + it.g) * SANGAM_PAGE);
+                }
+                TRACE_EV(54);
+                if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+            };
+            int w0 = ld_page(0), w1 = ld_page(1), w2 = ld_page(2);
+            load_tile(0, w0, false);
+            if (lead == 2 && n > 1) load_tile(1, w1, false);
+            for (int j = 0; j < n; ++j) {
+                const int nxt = ld_page(j + 3);
+                load_tile(j, w0, true);
+                if (j + lead < n) load_tile(j + lead, lead == 1 ? w1 : w2, false);
+                w0 = w1; w1 = w2; w2 = nxt;
+                if (*abort_flag) break;
             }
-            ++kvi;
         }
     }
     if (dynamic && lane == 0) {
@@ -361,7 +393,7 @@ __device__ __forceinline__ void qload_warp(const AttnParams& p, const CUtensorMa
 // so the softmax warpgroup always has the other half's logits waiting: it never idles on the tensor pipe.
 // (Only the last kv tile of a context can lack half B: fewer than 65 valid columns.)
 // The two issuers are independent; the in-order tensor pipe interleaves them.  K/V ring stages are consumed
-// in the order of OpWalk: each issuer walks the whole order, acts on its own ops and skips the other's.
+// in the ring order stated above the producer: each issuer walks the whole order, acts on its own tiles and skips the rest.
 // KV_EMPTY and Q_EMPTY expect two arrivals: SHARED stages / SPLIT q tiles are read by both issuers (one
 // commit each), SPLIT stages / SHARED q tiles by one issuer (which commits twice).
 // ------------------------------------------------------------------------------------------------
@@ -476,6 +508,7 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
         ptx::mbar_wait(st.bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
         const Item it = items[islot];
         if (!it.valid) break;
+        TRACE_EV(1 + s);
         const int n = it.kv1 - it.kv0, c = it.c, kv0 = it.kv0;
         if (n > 0) {
             if (it.rows1 > 0) {
@@ -507,10 +540,12 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
                 const uint32_t qs = qcount & 1u;
                 const int n0 = (n + 1) >> 1, n1 = n >> 1, ns = s ? n1 : n0;
                 ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qcount >> 1) & 1u, abort_flag);
+                TRACE_EV(3 + s);
                 uint32_t sk = 0, sv = 0;
                 if (s == 0) sk = st.acquire(); else st.skip();
                 if (n1 > 0) { if (s == 1) sk = st.acquire(); else st.skip(); }
-                if (ns > 0) tile_steps<D>(st, s, c, -1, false, 0u, kv0 + s, sk, qs, 2, ns == 1 ? 1 : 0);
+                TRACE_EV(5 + s);
+                if (ns > 0) { tile_steps<D>(st, s, c, -1, false, 0u, kv0 + s, sk, qs, 2, ns == 1 ? 1 : 0); TRACE_EV(7 + s); }
                 else if (lane == 0) ptx::mbar_arrive(st.bar(L::B_Q_EMPTY + qs));      // nothing to read: release the q tile
                 for (int i = 0; i < n0; ++i) {
 #pragma unroll
@@ -788,6 +823,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
                 ptx::mbar_wait(bar(L::B_EPI_B), ecount & 1u, abort_flag);       // stream 0 is done reading O_1
             } else {
                 ptx::mbar_wait(bar(L::B_EPI_A), ecount & 1u, abort_flag);
+                TRACE_EV(37);
                 const float2 x = ml_x[row];
                 const float ms = fmaxf(m, x.x);
                 const bool two = n > 1;                                    // stream 1 had tiles
@@ -894,6 +930,7 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
     volatile uint32_t* abort_flag = reinterpret_cast<volatile uint32_t*>(smem + L::OFF_MISC + 4);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     TRACE_INIT();
+    TRACE_CTA(0);
     if (tid == 0) {
         auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
         for (int s = 0; s < NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 2); }
@@ -942,6 +979,7 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
     }
     ptx::tc_fence_before();
     __syncthreads();
+    TRACE_CTA(1);
     if (tid == 0 && *abort_flag) raise_flag(p.flags, DEV_TIMEOUT);
     if (warp == 8) ptx::tmem_dealloc(tmem, 512);
 }

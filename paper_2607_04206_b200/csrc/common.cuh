@@ -44,6 +44,7 @@ __device__ __forceinline__ void raise_flag(uint32_t* flags, uint32_t f) {
 #define SANGAM_TRACE_CAP 8192            // events per warp
 __device__ unsigned long long g_trace[16 * SANGAM_TRACE_CAP];
 __device__ unsigned int g_trace_n[16];
+__device__ unsigned long long g_cta_times[2 * 256];   // per CTA: %globaltimer at entry / exit
 __device__ unsigned int g_trace_cta;     // which CTA records (sangam_trace_set_cta)
 __device__ __forceinline__ unsigned int* trace_cnt() {
     __shared__ unsigned int cnt[16];
@@ -74,9 +75,11 @@ __device__ __forceinline__ void trace_ns(unsigned ev) {
 }
 #define TRACE_EV(ev) trace_ev(ev)
 #define TRACE_NS(ev) trace_ns(ev)
+#define TRACE_CTA(which) do { if (threadIdx.x == 0 && blockIdx.x < 256) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_cta_times[2 * blockIdx.x + (which)] = t_; } } while (0)
 #define TRACE_INIT() do { if (threadIdx.x < 16) trace_cnt()[threadIdx.x] = 0; } while (0)
 #else
 #define TRACE_EV(ev) ((void)0)
 #define TRACE_NS(ev) ((void)0)
+#define TRACE_CTA(which) ((void)0)
 #define TRACE_INIT() ((void)0)
 #endif

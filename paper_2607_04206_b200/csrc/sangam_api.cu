@@ -263,6 +263,11 @@ extern "C" int sangam_iteration_host(sangam_ctx* ctx, const void* q_host, const 
 }
 
 #ifdef SANGAM_TRACE
+extern "C" int sangam_trace_cta_times(unsigned long long* host_buf) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(host_buf, g_cta_times, sizeof(unsigned long long) * 512);
+    return 0;
+}
 extern "C" int sangam_trace_set_cta(int cta) {
     unsigned int v = (unsigned int)cta, z[16] = {0};
     cudaDeviceSynchronize();
