@@ -212,7 +212,8 @@ def measure_config(cfg: int, steps: int, warmup: int, peaks, reps: int = 3):
     res.update({"flops": b.flops(), "attn_bytes": b.attn_bytes(), "write_bytes": b.write_bytes(),
                 "attn_tflops": round(b.flops() / a / 1e6, 2), "attn_gbs": round(b.attn_bytes() / a / 1e3, 1),
                 "kv_write_gbs": round(b.write_bytes() / max(res["kv_write_us"], 1e-9) / 1e3, 1),
-                "bound": BOUND[cfg], "t_roof_us": round(t_roof, 2), "roofline_frac": round(t_roof / a, 4)})
+                "bound": BOUND[cfg], "t_roof_us": round(t_roof, 2), "roofline_frac": round(t_roof / a, 4),
+                "device_flags": int(w.eng.device_status())})
     return res, w
 
 
@@ -385,7 +386,7 @@ def main():
     ms_total = max_over_ranks(ms_total, dist)
     ms_step = ms_total / steps
     value = world * b.flops() / (ms_step * 1e-3) / 1e12
-    kernels_per_step = 2                      # kv_write, attention (plan + split-KV merge fused in; captured, replayed K times)
+    kernels_per_step = 3                      # kv_write, attention (device-side plan inside), split-KV combine (captured; replayed K times)
     gpu_launches = steps * kernels_per_step
 
     # ---- dominant kernel (attention), timed alone, L2-cold
@@ -425,7 +426,8 @@ def main():
             "us_per_iteration": round(ms_step * 1e3, 3), "attn_us": round(attn_ms * 1e3, 3),
             "kv_write_us": round(write_ms * 1e3, 3),
             "clocks": cs.summary(), "e2e": e2e, "gpu_launches": gpu_launches,
-            "launch_count_check": w.eng.launch_count() - launches0, "roofline": roof}
+            "launch_count_check": w.eng.launch_count() - launches0, "device_flags": int(w.eng.device_status()),
+            "roofline": roof}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(b)

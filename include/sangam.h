@@ -66,6 +66,7 @@ typedef enum {
 #define SANGAM_DEV_BAD_PAGE   2u      /* block_attn: page id out of [0,num_pages), request skipped */
 #define SANGAM_DEV_CTX_TOO_LONG 4u    /* block_attn: ctx_len needs more than max_pages_per_req pages */
 #define SANGAM_DEV_TIMEOUT    8u      /* an in-kernel barrier wait gave up (internal error) */
+#define SANGAM_DEV_INTERNAL  16u      /* an internal bounds guard tripped; the access was skipped (internal error) */
 
 typedef struct {
     int32_t num_q_heads;        /* Hq */

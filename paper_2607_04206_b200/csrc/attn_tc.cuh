@@ -59,6 +59,13 @@ struct Item {          // one piece of work, published through shared memory (64
     int pad0, pad1, pad2;
 };
 
+struct SlotMeta {      // global, one per CTA: the split unit whose head piece (kv tile 0) this CTA computed, if any
+    int valid;
+    int npieces;       // CTAs b .. b + npieces - 1 hold its pieces: slot 2b+1, then slots 2(b+1), 2(b+2), ..
+    int g, tok0, rows0, rows1, q_start;
+    int pad0;
+};
+
 template <int D>
 struct Smem {
     static constexpr int Q_BYTES = BM * D * 2;
@@ -153,6 +160,8 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
     const unsigned FULL = 0xffffffffu;
     const int G_ctas = gridDim.x, b = blockIdx.x, R = p.batch;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    SlotMeta* meta = reinterpret_cast<SlotMeta*>(p.slot_meta);
+    if (lane == 0) meta[b].valid = 0;
     TRACE_EV(50);
     ReqCache rc;
     rc.init(p, lane);
@@ -283,6 +292,12 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
             it.q_start = ri.q0;
             it.c = ri.c;
             if (ri.c == 0) { it.kv0 = 0; it.kv1 = 0; }
+            if (it.part_slot >= 0 && it.kv0 == 0 && lane == 0) {      // head piece: tell combine_kernel what to merge
+                SlotMeta mm;
+                mm.valid = 1; mm.npieces = it.npieces; mm.g = it.g; mm.tok0 = it.tok0; mm.rows0 = it.rows0; mm.rows1 = it.rows1;
+                mm.q_start = it.q_start; mm.pad0 = it.r;
+                meta[b] = mm;
+            }
         }
         TRACE_EV(58);
         // publish
@@ -338,6 +353,12 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
             }
         }
     }
+    // Tail: every tcgen05.commit aimed at a KV_EMPTY barrier must have landed before this CTA may exit -- a late
+    // asynchronous arrive would hit the shared memory of whatever CTA runs here next.
+    for (int k = 0; k < NSTAGE; ++k) {
+        ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), phase ^ 1u, abort_flag);
+        if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+    }
     if (dynamic && lane == 0) {
         if (atomicAdd(p.sched + 1, 1) == G_ctas - 1) {   // last CTA out re-arms the counters for the next launch
             p.sched[0] = 0;
@@ -381,6 +402,9 @@ __device__ __forceinline__ void qload_warp(const AttnParams& p, const CUtensorMa
         if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
         ++icount;
     }
+    // tail: the commits aimed at the Q_EMPTY barriers must have landed before the CTA exits
+    for (int k = 0; k < 2; ++k, ++qcount)
+        ptx::mbar_wait(bar(L::B_Q_EMPTY + (qcount & 1u)), ((qcount >> 1) & 1u) ^ 1u, abort_flag);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -713,8 +737,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
     const uint32_t o_taddr = tmem + lane_base + 256u + (uint32_t)s * 128u;     // own accumulator
     const uint32_t o_other = tmem + lane_base + 256u + (uint32_t)(s ^ 1) * 128u;
     float2* ml_x = reinterpret_cast<float2*>(smem + L::OFF_ML);
-    volatile int* last_flag = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 8);
-    uint32_t icount = 0, hcount0 = 0, hcount1 = 0, pv0 = 0, pv1 = 0, ecount = 0, ccount = 0;
+    uint32_t icount = 0, hcount0 = 0, hcount1 = 0, pv0 = 0, pv1 = 0, ecount = 0;
     TRACE_NS(40);
     TRACE_EV(36);
     while (true) {
@@ -793,9 +816,13 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         }
         // ---------------- epilogue
         TRACE_EV(31);
-        const bool row_ok = row < rows_valid;
+        bool row_ok = row < rows_valid;
         const int tl = row / p.G, hh = row - tl * p.G;                       // row = token * G + head of the group
         const int tok = it.q_start + it.tok0 + ((shared && s == 1) ? p.tpt : 0) + tl;
+        if (row_ok && ((unsigned)tok >= (unsigned)p.total_q || (unsigned)it.g >= (unsigned)p.Hkv || it.part_slot >= p.num_slots)) {
+            raise_flag(p.flags, DEV_INTERNAL | 0x400u);      // never store through a bad item
+            row_ok = false;
+        }
         uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + it.g * p.G + hh) * D);
         const int prow = ((shared && s == 1) ? BM : 0) + row;                 // row inside the partial slot
         float4* po = reinterpret_cast<float4*>(p.part_o) + (int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * (D / 4) * PAIR + prow;
@@ -845,65 +872,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
             }
             ++ecount;
         }
-        // ---------------- fused split-KV merge across CTAs (a9): the CTA finishing a unit's last piece merges
         TRACE_EV(32);
-        if (it.part_slot >= 0) {
-            // every thread's partial stores happen-before its arrival; thread 0 then publishes them with one
-            // cumulative gpu-scope fence and counts this piece
-            ptx::mbar_arrive(bar(L::B_EPI_C));
-            if (s == 0 && row == 0) {
-                ptx::mbar_wait(bar(L::B_EPI_C), ccount & 1u, abort_flag);
-                __threadfence();
-                const int old = atomicAdd(p.unit_count + it.b_head, 1);
-                __threadfence();
-                const int last = old == it.npieces - 1;
-                if (last) p.unit_count[it.b_head] = 0;                           // re-armed for the next launch
-                *last_flag = last;
-                ptx::mbar_arrive(bar(L::B_EPI_D));
-            }
-            ptx::mbar_wait(bar(L::B_EPI_D), ccount & 1u, abort_flag);
-            const int last = *last_flag;
-            ++ccount;
-            TRACE_EV(33);
-            const int rr = s * BM + row;                                         // row inside the slot
-            if (last && row < (s ? it.rows1 : it.rows0)) {
-                // pieces in fixed order: head slot 2*b_head+1, then slots 2*b' of CTAs b' = b_head+1 ..; m in log2 units:
-                //   m* = max m_i;  l* = sum l_i 2^(m_i-m*);  O* = sum O_i 2^(m_i-m*);  out = bf16(O*/l*)
-                // One thread per row; consecutive rows of a column group are contiguous, so every load coalesces.
-                const int np = it.npieces;
-                const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
-                float ms = -INFINITY;
-                for (int pi = 0; pi < np; ++pi)
-                    ms = fmaxf(ms, __ldcg(&ml[(int64_t)(pi == 0 ? 2 * it.b_head + 1 : 2 * (it.b_head + pi)) * PAIR + rr].x));
-                float acc[D];
-#pragma unroll
-                for (int e = 0; e < D; ++e) acc[e] = 0.f;
-                float ls = 0.f;
-                for (int pi = 0; pi < np; ++pi) {
-                    const int64_t slot = pi == 0 ? 2 * it.b_head + 1 : 2 * (it.b_head + pi);
-                    const float2 x = __ldcg(&ml[slot * PAIR + rr]);
-                    const float w = ptx::ex2(x.x - ms);
-                    ls = fmaf(x.y, w, ls);
-                    const float4* src = reinterpret_cast<const float4*>(p.part_o) + slot * (D / 4) * PAIR + rr;
-#pragma unroll
-                    for (int c4 = 0; c4 < D / 4; ++c4) {
-                        const float4 o = __ldcg(src + c4 * PAIR);
-                        acc[c4 * 4 + 0] = fmaf(o.x, w, acc[c4 * 4 + 0]); acc[c4 * 4 + 1] = fmaf(o.y, w, acc[c4 * 4 + 1]);
-                        acc[c4 * 4 + 2] = fmaf(o.z, w, acc[c4 * 4 + 2]); acc[c4 * 4 + 3] = fmaf(o.w, w, acc[c4 * 4 + 3]);
-                    }
-                }
-                const float inv = ls > 0.f ? 1.f / ls : 0.f;
-#pragma unroll
-                for (int c8 = 0; c8 < D / 8; ++c8) {
-                    uint4 w4;
-                    w4.x = ptx::pack_bf16(acc[c8 * 8 + 0] * inv, acc[c8 * 8 + 1] * inv);
-                    w4.y = ptx::pack_bf16(acc[c8 * 8 + 2] * inv, acc[c8 * 8 + 3] * inv);
-                    w4.z = ptx::pack_bf16(acc[c8 * 8 + 4] * inv, acc[c8 * 8 + 5] * inv);
-                    w4.w = ptx::pack_bf16(acc[c8 * 8 + 6] * inv, acc[c8 * 8 + 7] * inv);
-                    dst[c8] = w4;
-                }
-            }
-        }
         TRACE_EV(34);
         ptx::tc_fence_before();
         __syncwarp();
@@ -984,6 +953,58 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
     if (warp == 8) ptx::tmem_dealloc(tmem, 512);
 }
 
+// ------------------------------------------------------------------------------------------------
+// combine (a9): merge the split-KV pieces of one unit.  Block b owns the unit whose head piece CTA b of
+// attn_kernel computed (SlotMeta); pieces in fixed order, no atomics: bitwise reproducible.  m in log2 units:
+//   m* = max m_i;  l* = sum l_i 2^(m_i-m*);  O* = sum O_i 2^(m_i-m*);  out = bf16(O*/l*)
+// One thread per row; a column group's consecutive rows are contiguous in a slot, so every load coalesces.
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(PAIR)
+combine_kernel(const AttnParams p) {
+    const int b = blockIdx.x;
+    const SlotMeta h = reinterpret_cast<const SlotMeta*>(p.slot_meta)[b];
+    if (!h.valid) return;
+    const int s = threadIdx.x >> 7, row = threadIdx.x & 127, rr = threadIdx.x;      // rr = row inside the slot
+    if (row >= (s ? h.rows1 : h.rows0)) return;
+    const int np = h.npieces;
+    if (np < 1 || 2 * (b + np - 1) >= p.num_slots) { raise_flag(p.flags, DEV_INTERNAL | 0x100u); return; }
+    const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
+    float ms = -INFINITY;
+    for (int pi = 0; pi < np; ++pi) ms = fmaxf(ms, ml[(int64_t)(pi == 0 ? 2 * b + 1 : 2 * (b + pi)) * PAIR + rr].x);
+    float acc[D];
+#pragma unroll
+    for (int e = 0; e < D; ++e) acc[e] = 0.f;
+    float ls = 0.f;
+    for (int pi = 0; pi < np; ++pi) {
+        const int64_t slot = pi == 0 ? 2 * b + 1 : 2 * (b + pi);
+        const float2 x = ml[slot * PAIR + rr];
+        const float w = ptx::ex2(x.x - ms);
+        ls = fmaf(x.y, w, ls);
+        const float4* src = reinterpret_cast<const float4*>(p.part_o) + slot * (D / 4) * PAIR + rr;
+#pragma unroll
+        for (int c4 = 0; c4 < D / 4; ++c4) {
+            const float4 o = __ldcs(src + c4 * PAIR);
+            acc[c4 * 4 + 0] = fmaf(o.x, w, acc[c4 * 4 + 0]); acc[c4 * 4 + 1] = fmaf(o.y, w, acc[c4 * 4 + 1]);
+            acc[c4 * 4 + 2] = fmaf(o.z, w, acc[c4 * 4 + 2]); acc[c4 * 4 + 3] = fmaf(o.w, w, acc[c4 * 4 + 3]);
+        }
+    }
+    const float inv = ls > 0.f ? 1.f / ls : 0.f;
+    const int tl = row / p.G, hh = row - tl * p.G;
+    const int tok = h.q_start + h.tok0 + s * p.tpt + tl;
+    if ((unsigned)tok >= (unsigned)p.total_q || (unsigned)h.g >= (unsigned)p.Hkv) { raise_flag(p.flags, DEV_INTERNAL | 0x200u); return; }
+    uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + h.g * p.G + hh) * D);
+#pragma unroll
+    for (int c8 = 0; c8 < D / 8; ++c8) {
+        uint4 w4;
+        w4.x = ptx::pack_bf16(acc[c8 * 8 + 0] * inv, acc[c8 * 8 + 1] * inv);
+        w4.y = ptx::pack_bf16(acc[c8 * 8 + 2] * inv, acc[c8 * 8 + 3] * inv);
+        w4.z = ptx::pack_bf16(acc[c8 * 8 + 4] * inv, acc[c8 * 8 + 5] * inv);
+        w4.w = ptx::pack_bf16(acc[c8 * 8 + 6] * inv, acc[c8 * 8 + 7] * inv);
+        dst[c8] = w4;
+    }
+}
+
 }  // namespace tc
 
 // ------------------------------------------------------------------------------------------------
@@ -1043,8 +1064,13 @@ static inline int tc_encode_q(TcMaps* maps, const void* q, int total_q, int Hq, 
 
 static inline cudaError_t tc_launch(const AttnParams& p, const TcMaps& maps, int head_dim, int sm_count,
                                     cudaStream_t stream, int* launched) {
-    if (head_dim == 128) tc::attn_kernel<128><<<sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
-    else tc::attn_kernel<64><<<sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
-    *launched = 1;
+    if (head_dim == 128) {
+        tc::attn_kernel<128><<<sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
+        tc::combine_kernel<128><<<sm_count, tc::PAIR, 0, stream>>>(p);
+    } else {
+        tc::attn_kernel<64><<<sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
+        tc::combine_kernel<64><<<sm_count, tc::PAIR, 0, stream>>>(p);
+    }
+    *launched = 2;
     return cudaGetLastError();
 }

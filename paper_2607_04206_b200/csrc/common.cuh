@@ -12,6 +12,7 @@
 #define DEV_BAD_PAGE 2u
 #define DEV_CTX_TOO_LONG 4u
 #define DEV_TIMEOUT 8u
+#define DEV_INTERNAL 16u           // an internal bounds guard tripped (library bug; the access was skipped)
 
 struct AttnParams {
     const __nv_bfloat16* q;        // [total_q][Hq][D]
@@ -30,7 +31,7 @@ struct AttnParams {
     float* part_o;                 // [num_slots][256][D]  unnormalised partial sums
     float* part_ml;                // [num_slots][256][2]  (m in log2 units, l)
     int32_t num_slots;
-    int32_t* unit_count;           // [num_ctas] pieces of a split unit finished so far (self-resetting)
+    void* slot_meta;               // [num_ctas] tc::SlotMeta, rewritten by every launch
     uint32_t* flags;               // sticky device flags
     int32_t* sched;                // [0] dynamic work counter (self-resetting), [1] finished-CTA count
 };
