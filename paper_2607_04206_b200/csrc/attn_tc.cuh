@@ -40,6 +40,10 @@ constexpr int NSTAGE = 5;        // K/V tile ring depth
 constexpr int NTHREADS = 384;
 constexpr int SLAB = 128 * 128;  // bytes of one 64-wide swizzled slab of a 128-row tile
 constexpr int DYN_UNITS_PER_CTA = 4;   // >= this many units per CTA: whole units, dynamic hand-out
+#ifndef SANGAM_UNIT_OV
+#define SANGAM_UNIT_OV 3
+#endif
+constexpr int UNIT_OV = SANGAM_UNIT_OV;  // static partition: fixed cost of starting/finishing a unit, in kv-tile equivalents
 constexpr float LAZY_T = 8.f;    // the reference maximum moves only when a tile exceeds it by 2^8
 #ifndef SANGAM_POLY_EXP
 #define SANGAM_POLY_EXP 0        // of every 8 exponentials, this many run on the FMA pipe instead of MUFU
@@ -173,7 +177,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
         if (base + lane < R) {
             const ReqInfo x = rc.get_lane(p, base, lane);
             U += x.units;
-            T += x.units * x.tiles_u;
+            T += x.units * (x.tiles_u + UNIT_OV);
         }
     }
 #pragma unroll
@@ -200,7 +204,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
             int acc = 0, found = -1;
             for (int base = 0; base < R && found < 0; base += 32) {
                 int tl = 0;
-                if (base + lane < R) { const ReqInfo x = rc.get_lane(p, base, lane); tl = x.units * x.tiles_u; }
+                if (base + lane < R) { const ReqInfo x = rc.get_lane(p, base, lane); tl = x.units * (x.tiles_u + UNIT_OV); }
                 int incl = tl;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -221,8 +225,8 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
             if (r_cur < R) {
                 cur = rc.get(p, r_cur);
                 const int pos = t0 - tile_base;
-                u_in_r = pos / cur.tiles_u;
-                kvoff = pos - u_in_r * cur.tiles_u;
+                u_in_r = pos / (cur.tiles_u + UNIT_OV);
+                kvoff = pos - u_in_r * (cur.tiles_u + UNIT_OV);
             } else {
                 remaining = 0;
             }
@@ -255,33 +259,42 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                     ri = cur;
                 }
             }
-        } else if (remaining > 0 && r_cur < R) {
-            const int take = remaining < cur.tiles_u - kvoff ? remaining : cur.tiles_u - kvoff;
-            it.valid = 1; it.r = r_cur; it.g = u_in_r / cur.np;
-            it.tok0 = (u_in_r - it.g * cur.np) * 2 * p.tpt;
-            it.kv0 = kvoff; it.kv1 = kvoff + take;
-            ri = cur;
-            if (!(it.kv0 == 0 && it.kv1 == cur.tiles_u)) {
-                // a piece of a unit split across CTAs: CTA x holds flattened tiles [floor(xT/Geff), floor((x+1)T/Geff))
-                it.part_slot = 2 * b + (it.kv0 == 0 ? 1 : 0);
-                const int ut0 = tile_base + u_in_r * cur.tiles_u, ut1 = ut0 + cur.tiles_u;      // < T < 2^31
-                const int bh = mul_div_ceil(ut0 + 1, Geff, T) - 1;
-                int bl = mul_div_ceil(ut1, Geff, T) - 1;
-                bl = bl > Geff - 1 ? Geff - 1 : bl;
-                it.b_head = bh;
-                it.npieces = bl - bh + 1;
-            }
-            remaining -= take;
-            kvoff += take;
-            if (kvoff == cur.tiles_u) {
-                kvoff = 0;
-                if (++u_in_r == cur.units) {
-                    u_in_r = 0;
-                    do {
-                        tile_base += cur.units * cur.tiles_u;
-                        ++r_cur;
-                        if (r_cur < R) cur = rc.get(p, r_cur);
-                    } while (r_cur < R && cur.units == 0);
+        } else {
+            // static partition: this CTA owns the weighted coordinates [x0, x1) of the flattened unit list; a unit
+            // spans UNIT_OV + tiles_u of them, coordinate UNIT_OV + j being its kv tile j.  A range that covers only
+            // part of a unit's overhead span yields no work there.
+            while (remaining > 0 && r_cur < R && !it.valid) {
+                const int wu = cur.tiles_u + UNIT_OV;
+                const int take = remaining < wu - kvoff ? remaining : wu - kvoff;
+                const int a = kvoff > UNIT_OV ? kvoff - UNIT_OV : 0, e = kvoff + take > UNIT_OV ? kvoff + take - UNIT_OV : 0;
+                if (e > a) {
+                    it.valid = 1; it.r = r_cur; it.g = u_in_r / cur.np;
+                    it.tok0 = (u_in_r - it.g * cur.np) * 2 * p.tpt;
+                    it.kv0 = a; it.kv1 = e;
+                    ri = cur;
+                    if (!(a == 0 && e == cur.tiles_u)) {
+                        // a piece of a unit split across CTAs: CTA x owns coordinates [floor(xT/Geff), floor((x+1)T/Geff))
+                        it.part_slot = 2 * b + (a == 0 ? 1 : 0);
+                        const int ut0 = tile_base + u_in_r * wu + UNIT_OV;           // coordinate of kv tile 0; < T < 2^31
+                        const int bh = mul_div_ceil(ut0 + 1, Geff, T) - 1;
+                        int bl = mul_div_ceil(ut0 + cur.tiles_u, Geff, T) - 1;
+                        bl = bl > Geff - 1 ? Geff - 1 : bl;
+                        it.b_head = bh;
+                        it.npieces = bl - bh + 1;
+                    }
+                }
+                remaining -= take;
+                kvoff += take;
+                if (kvoff == wu) {
+                    kvoff = 0;
+                    if (++u_in_r == cur.units) {
+                        u_in_r = 0;
+                        do {
+                            tile_base += cur.units * wu;
+                            ++r_cur;
+                            if (r_cur < R) cur = rc.get(p, r_cur);
+                        } while (r_cur < R && cur.units == 0);
+                    }
                 }
             }
         }
