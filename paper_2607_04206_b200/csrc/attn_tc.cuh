@@ -970,7 +970,7 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
 // combine (a9): merge the split-KV pieces of one unit.  Block b owns the unit whose head piece CTA b of
 // attn_kernel computed (SlotMeta); pieces in fixed order, no atomics: bitwise reproducible.  m in log2 units:
 //   m* = max m_i;  l* = sum l_i 2^(m_i-m*);  O* = sum O_i 2^(m_i-m*);  out = bf16(O*/l*)
-// One thread per row; a column group's consecutive rows are contiguous in a slot, so every load coalesces.
+// A column group's consecutive rows are contiguous in a slot, so every load coalesces.
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __global__ void __launch_bounds__(PAIR)
@@ -978,43 +978,80 @@ combine_kernel(const AttnParams p) {
     const int b = blockIdx.x;
     const SlotMeta h = reinterpret_cast<const SlotMeta*>(p.slot_meta)[b];
     if (!h.valid) return;
-    const int s = threadIdx.x >> 7, row = threadIdx.x & 127, rr = threadIdx.x;      // rr = row inside the slot
-    if (row >= (s ? h.rows1 : h.rows0)) return;
-    const int np = h.npieces;
-    if (np < 1 || 2 * (b + np - 1) >= p.num_slots) { raise_flag(p.flags, DEV_INTERNAL | 0x100u); return; }
+    const int np = h.npieces, R = h.rows0 + h.rows1;
+    if (np < 1 || 2 * (b + np - 1) >= p.num_slots || (unsigned)h.g >= (unsigned)p.Hkv) { raise_flag(p.flags, DEV_INTERNAL | 0x100u); return; }
     const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
-    float ms = -INFINITY;
-    for (int pi = 0; pi < np; ++pi) ms = fmaxf(ms, ml[(int64_t)(pi == 0 ? 2 * b + 1 : 2 * (b + pi)) * PAIR + rr].x);
-    float acc[D];
+    if (R > 64) {
+        // many rows (GQA decode): one thread per row, 32 independent 16-byte loads per piece in flight
+        const int s = threadIdx.x >> 7, row = threadIdx.x & 127, rr = threadIdx.x;
+        if (row >= (s ? h.rows1 : h.rows0)) return;
+        float ms = -INFINITY;
+        for (int pi = 0; pi < np; ++pi) ms = fmaxf(ms, ml[(int64_t)(pi == 0 ? 2 * b + 1 : 2 * (b + pi)) * PAIR + rr].x);
+        float acc[D];
 #pragma unroll
-    for (int e = 0; e < D; ++e) acc[e] = 0.f;
-    float ls = 0.f;
-    for (int pi = 0; pi < np; ++pi) {
-        const int64_t slot = pi == 0 ? 2 * b + 1 : 2 * (b + pi);
-        const float2 x = ml[slot * PAIR + rr];
-        const float w = ptx::ex2(x.x - ms);
-        ls = fmaf(x.y, w, ls);
-        const float4* src = reinterpret_cast<const float4*>(p.part_o) + slot * (D / 4) * PAIR + rr;
+        for (int e = 0; e < D; ++e) acc[e] = 0.f;
+        float ls = 0.f;
+        for (int pi = 0; pi < np; ++pi) {
+            const int64_t slot = pi == 0 ? 2 * b + 1 : 2 * (b + pi);
+            const float2 x = ml[slot * PAIR + rr];
+            const float w = ptx::ex2(x.x - ms);
+            ls = fmaf(x.y, w, ls);
+            const float4* src = reinterpret_cast<const float4*>(p.part_o) + slot * (D / 4) * PAIR + rr;
 #pragma unroll
-        for (int c4 = 0; c4 < D / 4; ++c4) {
-            const float4 o = __ldcs(src + c4 * PAIR);
-            acc[c4 * 4 + 0] = fmaf(o.x, w, acc[c4 * 4 + 0]); acc[c4 * 4 + 1] = fmaf(o.y, w, acc[c4 * 4 + 1]);
-            acc[c4 * 4 + 2] = fmaf(o.z, w, acc[c4 * 4 + 2]); acc[c4 * 4 + 3] = fmaf(o.w, w, acc[c4 * 4 + 3]);
+            for (int c4 = 0; c4 < D / 4; ++c4) {
+                const float4 o = __ldcs(src + c4 * PAIR);
+                acc[c4 * 4 + 0] = fmaf(o.x, w, acc[c4 * 4 + 0]); acc[c4 * 4 + 1] = fmaf(o.y, w, acc[c4 * 4 + 1]);
+                acc[c4 * 4 + 2] = fmaf(o.z, w, acc[c4 * 4 + 2]); acc[c4 * 4 + 3] = fmaf(o.w, w, acc[c4 * 4 + 3]);
+            }
         }
-    }
-    const float inv = ls > 0.f ? 1.f / ls : 0.f;
-    const int tl = row / p.G, hh = row - tl * p.G;
-    const int tok = h.q_start + h.tok0 + s * p.tpt + tl;
-    if ((unsigned)tok >= (unsigned)p.total_q || (unsigned)h.g >= (unsigned)p.Hkv) { raise_flag(p.flags, DEV_INTERNAL | 0x200u); return; }
-    uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + h.g * p.G + hh) * D);
+        const float inv = ls > 0.f ? 1.f / ls : 0.f;
+        const int tl = row / p.G, hh = row - tl * p.G;
+        const int tok = h.q_start + h.tok0 + s * p.tpt + tl;
+        if ((unsigned)tok >= (unsigned)p.total_q) { raise_flag(p.flags, DEV_INTERNAL | 0x200u); return; }
+        uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + h.g * p.G + hh) * D);
 #pragma unroll
-    for (int c8 = 0; c8 < D / 8; ++c8) {
+        for (int c8 = 0; c8 < D / 8; ++c8) {
+            uint4 w4;
+            w4.x = ptx::pack_bf16(acc[c8 * 8 + 0] * inv, acc[c8 * 8 + 1] * inv);
+            w4.y = ptx::pack_bf16(acc[c8 * 8 + 2] * inv, acc[c8 * 8 + 3] * inv);
+            w4.z = ptx::pack_bf16(acc[c8 * 8 + 4] * inv, acc[c8 * 8 + 5] * inv);
+            w4.w = ptx::pack_bf16(acc[c8 * 8 + 6] * inv, acc[c8 * 8 + 7] * inv);
+            dst[c8] = w4;
+        }
+        return;
+    }
+    // few rows (MHA decode): work item = (8-column group cg, row), consecutive threads take consecutive rows of one
+    // column group, so a 32-row unit still spreads over all 256 threads
+    for (int item = threadIdx.x; item < R * (D / 8); item += PAIR) {
+        const int cg = item / R, ri = item - cg * R;
+        const int s = ri >= h.rows0, row = ri - (s ? h.rows0 : 0), rr = s * BM + row;      // rr = row inside the slot
+        float ms = -INFINITY;
+        for (int pi = 0; pi < np; ++pi) ms = fmaxf(ms, ml[(int64_t)(pi == 0 ? 2 * b + 1 : 2 * (b + pi)) * PAIR + rr].x);
+        float acc[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) acc[e] = 0.f;
+        float ls = 0.f;
+#pragma unroll 4
+        for (int pi = 0; pi < np; ++pi) {
+            const int64_t slot = pi == 0 ? 2 * b + 1 : 2 * (b + pi);
+            const float2 x = ml[slot * PAIR + rr];
+            const float w = ptx::ex2(x.x - ms);
+            ls = fmaf(x.y, w, ls);
+            const float4* src = reinterpret_cast<const float4*>(p.part_o) + (slot * (D / 4) + 2 * cg) * PAIR + rr;
+            const float4 o0 = __ldcs(src), o1 = __ldcs(src + PAIR);
+            acc[0] = fmaf(o0.x, w, acc[0]); acc[1] = fmaf(o0.y, w, acc[1]); acc[2] = fmaf(o0.z, w, acc[2]); acc[3] = fmaf(o0.w, w, acc[3]);
+            acc[4] = fmaf(o1.x, w, acc[4]); acc[5] = fmaf(o1.y, w, acc[5]); acc[6] = fmaf(o1.z, w, acc[6]); acc[7] = fmaf(o1.w, w, acc[7]);
+        }
+        const float inv = ls > 0.f ? 1.f / ls : 0.f;
+        const int tl = row / p.G, hh = row - tl * p.G;
+        const int tok = h.q_start + h.tok0 + s * p.tpt + tl;
+        if ((unsigned)tok >= (unsigned)p.total_q) { raise_flag(p.flags, DEV_INTERNAL | 0x200u); continue; }
         uint4 w4;
-        w4.x = ptx::pack_bf16(acc[c8 * 8 + 0] * inv, acc[c8 * 8 + 1] * inv);
-        w4.y = ptx::pack_bf16(acc[c8 * 8 + 2] * inv, acc[c8 * 8 + 3] * inv);
-        w4.z = ptx::pack_bf16(acc[c8 * 8 + 4] * inv, acc[c8 * 8 + 5] * inv);
-        w4.w = ptx::pack_bf16(acc[c8 * 8 + 6] * inv, acc[c8 * 8 + 7] * inv);
-        dst[c8] = w4;
+        w4.x = ptx::pack_bf16(acc[0] * inv, acc[1] * inv);
+        w4.y = ptx::pack_bf16(acc[2] * inv, acc[3] * inv);
+        w4.z = ptx::pack_bf16(acc[4] * inv, acc[5] * inv);
+        w4.w = ptx::pack_bf16(acc[6] * inv, acc[7] * inv);
+        reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + h.g * p.G + hh) * D)[cg] = w4;
     }
 }
 
