@@ -1,10 +1,10 @@
 // attn_tc.cuh -- steps a3..a9: paged, varlen, non-causal block attention on tcgen05 (sm_100a).
 //
 // One persistent CTA per SM, 12 warps, warp-specialised, TWO softmax streams per CTA:
-//   warp 8      scheduler + TMA producer: plans the work on the device (a3) and gathers K/V pages of
+//   warp 9      scheduler + TMA producer: plans the work on the device (a3) and gathers K/V pages of
 //               the current (request, kv head) through the block table with TMA into a ring of
-//               128-row, 128B-swizzled shared-memory tiles (a4); also owns the TMEM allocation
-//   warp 9      Q loader: packed (query row, q head of the group) rows -> swizzled smem, 2-slot ring
+//               128-row, 128B-swizzled shared-memory tiles (a4)
+//   warp 8      Q loader (TMA, 2-slot ring of 128-row q tiles); also owns the TMEM allocation
 //   warps 10,11 MMA issuers, one per stream s: S_s = Q_s K^T (tcgen05.mma, operands in smem, S in
 //               TMEM; a5) and O_s += P_s V (P read from TMEM, V from smem, O in TMEM; a7)
 //   warps 0-3   softmax warpgroup of stream 0;  warps 4-7: stream 1.  Thread i owns row i of the
@@ -31,6 +31,10 @@ struct TcMaps {
     CUtensorMap k, v, q;
 };
 
+#ifdef SANGAM_DEBUG_ITEM
+__device__ int g_bad_item[16];
+#endif
+
 namespace tc {
 
 constexpr int BM = 128;          // rows per q tile  (UMMA M)
@@ -39,7 +43,10 @@ constexpr int PAIR = 2 * BM;     // packed rows per work unit
 constexpr int NSTAGE = 5;        // K/V tile ring depth
 constexpr int NTHREADS = 384;
 constexpr int SLAB = 128 * 128;  // bytes of one 64-wide swizzled slab of a 128-row tile
-constexpr int DYN_UNITS_PER_CTA = 4;   // >= this many units per CTA: whole units, dynamic hand-out
+#ifndef SANGAM_DYN_UNITS
+#define SANGAM_DYN_UNITS 4
+#endif
+constexpr int DYN_UNITS_PER_CTA = SANGAM_DYN_UNITS;   // >= this many units per CTA: whole units, dynamic hand-out
 #ifndef SANGAM_UNIT_OV
 #define SANGAM_UNIT_OV 3
 #endif
@@ -85,7 +92,8 @@ struct Smem {
     static constexpr int OFF_ITEMS = OFF_BAR + ((NBAR * 8 + 15) / 16) * 16;
     static constexpr int OFF_ML = OFF_ITEMS + 2 * (int)sizeof(Item);    // (m, l) of stream 1, 128 rows
     static constexpr int OFF_MISC = OFF_ML + BM * 8;
-    static constexpr int TOTAL = OFF_MISC + 16;
+    static constexpr int OFF_SEQ = OFF_MISC + 16 + 64;   // tmem slot, abort word, pad; per-warp wait table (diagnostics)
+    static constexpr int TOTAL = OFF_SEQ + 32;           // kv_seq[NSTAGE]
     static constexpr int ALLOC = TOTAL + 1024;   // slack to align the base to 1024 B (128B swizzle atoms)
 };
 static_assert(sizeof(Item) == 64, "Item is 64 bytes");
@@ -155,11 +163,12 @@ struct ReqCache {
 // SHARED: both issuers read every stage.  SPLIT: tile j belongs to stream j & 1, the other issuer skips it.
 
 // ------------------------------------------------------------------------------------------------
-// warp 8: device-side plan (a3) + TMA page gather (a4)
+// warp 9: device-side plan (a3) + TMA page gather (a4)
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtensorMap* mapK, const CUtensorMap* mapV,
-                                              uint32_t sbase, Item* items, volatile uint32_t* abort_flag, int lane) {
+                                              uint32_t sbase, Item* items, volatile uint32_t* abort_flag,
+                                              volatile uint32_t* kv_seq, int lane) {
     using L = Smem<D>;
     const unsigned FULL = 0xffffffffu;
     const int G_ctas = gridDim.x, b = blockIdx.x, R = p.batch;
@@ -234,7 +243,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
     }
     TRACE_EV(52);
 
-    uint32_t stage = 0, phase = 0, icount = 0;       // next K/V ring position and its parity
+    uint32_t stage = 0, phase = 0, pos = 0, icount = 0;   // next K/V ring position: stage, parity, running index
     while (true) {
         if (*abort_flag) break;
         Item it;
@@ -343,7 +352,11 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                 ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), phase ^ 1u, abort_flag);
                 int np = pages_total - tile * 8;
                 np = np > 8 ? 8 : np;
-                if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_KV_FULL + stage), (uint32_t)(np * SANGAM_PAGE * D * 2));
+                if (lane == 0) {
+                    kv_seq[stage] = pos;                     // the issuers check this before trusting the barrier's parity
+                    ptx::mbar_arrive_expect_tx(bar(L::B_KV_FULL + stage), (uint32_t)(np * SANGAM_PAGE * D * 2));
+                }
+                ++pos;
                 __syncwarp();
                 if (pg < np) {
                     if ((unsigned)page >= (unsigned)p.P) raise_flag(p.flags, DEV_BAD_PAGE);   // TMA zero-fills out of range
@@ -382,7 +395,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
 }
 
 // ------------------------------------------------------------------------------------------------
-// warp 9: Q loader.  q is viewed as a 3-D tensor [total_q][Hq][D]; one TMA box = 64 columns x the G heads
+// warp 8: Q loader.  q is viewed as a 3-D tensor [total_q][Hq][D]; one TMA box = 64 columns x the G heads
 // of the group x tpt tokens lands as rows (token * G + head) of a K-major 128B-swizzled UMMA tile.
 // Two q-tile slots form a ring; a slot is refilled as soon as the last QK reading it has completed.
 // Rows past the request's last token hold the next request's tokens or TMA zero fill: never stored.
@@ -438,17 +451,32 @@ template <int D>
 struct MmaState {
     uint32_t sbase, tmem;
     uint64_t q_desc0, k_desc0, v_desc0;
-    uint32_t stage, phase;            // next ring position and its parity
+    uint32_t stage, phase, pos;       // next ring position: stage, parity, running index
+    volatile uint32_t* kv_seq;        // [NSTAGE] position being loaded into each stage (written by the producer)
     uint32_t p_par0, p_par1;          // parity of the next P_FULL wait, half A / B
     uint32_t zf_par;                  // parity of the next ZFILL wait (SHARED tail tiles)
     volatile uint32_t* abort_flag;
     __device__ __forceinline__ uint32_t bar(int i) const { return sbase + (uint32_t)(Smem<D>::OFF_BAR + i * 8); }
-    __device__ __forceinline__ void skip() { if (++stage == NSTAGE) { stage = 0; phase ^= 1u; } }
+    // Wait for ring position `pos` (stage = pos % NSTAGE).  In SPLIT mode an issuer does not consume every use
+    // of a stage, and an mbarrier parity wait only tells adjacent phases apart (TMA loads complete out of order:
+    // the skipped use may still be in flight when the next-but-one is awaited).  So the producer publishes the
+    // position it is loading into each stage (kv_seq) and the issuer first waits for ITS position to be the one
+    // in flight; from then on the barrier's current phase is exactly that load's.
     __device__ __forceinline__ uint32_t acquire() {
         const uint32_t s0 = stage;
+        if (kv_seq[s0] != pos) {                       // the issuer is ahead of the producer
+            uint32_t spins = 0;
+            while (kv_seq[s0] != pos)
+                if ((++spins & 0x3ffu) == 0 && *abort_flag) break;
+        }
         ptx::mbar_wait(bar(Smem<D>::B_KV_FULL + s0), phase, abort_flag);
         skip();
         return s0;
+    }
+    // a ring position that belongs to the other issuer (SPLIT mode)
+    __device__ __forceinline__ void skip() {
+        ++pos;
+        if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
     }
 };
 
@@ -530,14 +558,15 @@ __device__ __forceinline__ void tile_steps(MmaState<D>& st, int s, int c, int ti
 
 template <int D>
 __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, uint32_t tmem, const Item* items,
-                                         volatile uint32_t* abort_flag, int s, int lane) {
+                                         volatile uint32_t* abort_flag, uint32_t* kv_seq_smem, int s, int lane) {
     using L = Smem<D>;
     MmaState<D> st;
     st.sbase = sbase; st.tmem = tmem; st.abort_flag = abort_flag;
     st.q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);        // K-major operands (Q, K)
     st.k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, 1024);
     st.v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, SLAB, 1024);     // MN-major operand (V)
-    st.stage = 0; st.phase = 0; st.p_par0 = 0; st.p_par1 = 0; st.zf_par = 0;
+    st.stage = 0; st.phase = 0; st.pos = 0; st.kv_seq = reinterpret_cast<volatile uint32_t*>(kv_seq_smem);
+    st.p_par0 = 0; st.p_par1 = 0; st.zf_par = 0;
     uint32_t icount = 0, qcount = 0;
     while (true) {
         if (*abort_flag) break;
@@ -550,7 +579,10 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
         if (n > 0) {
             if (it.rows1 > 0) {
                 // SHARED: stream s = q tile s; ring order K_0 V_0 K_1 V_1 ..., every stage read by both issuers
-                const uint32_t qc = qcount + (uint32_t)s, qs = qc & 1u;
+                const uint32_t qc = qcount + (uint32_t)s, qs = qc & 1u, qo = qcount + (uint32_t)(s ^ 1);
+                // The other stream's q tile is only observed, and only for items so short that this issuer could
+                // finish them before that tile has landed (same parity-aliasing hazard as for the K/V ring).
+                if (n <= NSTAGE) ptx::mbar_wait(st.bar(L::B_Q_FULL + (qo & 1u)), (qo >> 1) & 1u, abort_flag);
                 ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qc >> 1) & 1u, abort_flag);
                 uint32_t sk = st.acquire();
                 tile_steps<D>(st, s, c, -1, false, 0u, kv0, sk, qs, 1, n == 1 ? 2 : 0);
@@ -834,6 +866,13 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         const int tok = it.q_start + it.tok0 + ((shared && s == 1) ? p.tpt : 0) + tl;
         if (row_ok && ((unsigned)tok >= (unsigned)p.total_q || (unsigned)it.g >= (unsigned)p.Hkv || it.part_slot >= p.num_slots)) {
             raise_flag(p.flags, DEV_INTERNAL | 0x400u);      // never store through a bad item
+#ifdef SANGAM_DEBUG_ITEM
+            if (atomicCAS(&ptx::g_timeout_info[0], 0u, 0xdead0000u | (unsigned)s) == 0u) {
+                const int* w = reinterpret_cast<const int*>(&it);
+                for (int k = 0; k < 13; ++k) g_bad_item[k] = w[k];
+                g_bad_item[13] = tok; g_bad_item[14] = row; g_bad_item[15] = (int)icount;
+            }
+#endif
             row_ok = false;
         }
         uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + it.g * p.G + hh) * D);
@@ -910,6 +949,7 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
     Item* items = reinterpret_cast<Item*>(smem + L::OFF_ITEMS);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::OFF_MISC);
     volatile uint32_t* abort_flag = reinterpret_cast<volatile uint32_t*>(smem + L::OFF_MISC + 4);
+    uint32_t* kv_seq = reinterpret_cast<uint32_t*>(smem + L::OFF_SEQ);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     TRACE_INIT();
     TRACE_CTA(0);
@@ -933,6 +973,8 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
         ptx::mbar_init(bar(L::B_EPI_D), 1);
         ptx::mbar_init(bar(L::B_ZFILL), 1);
         *abort_flag = 0u;
+        for (int k = 0; k < 16; ++k) abort_flag[3 + k] = 0u;
+        for (int k = 0; k < NSTAGE; ++k) kv_seq[k] = 0xffffffffu;
         ptx::fence_mbar_init();
         ptx::prefetch_tensormap(&mapK);
         ptx::prefetch_tensormap(&mapV);
@@ -955,10 +997,14 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
         softmax_wg<D>(p, smem, sbase, tmem, items, abort_flag, warp >> 2, warp & 3, lane);
     } else {
         ptx::setmaxnreg_dec<80>();
-        if (warp == 8) producer_warp<D>(p, &mapK, &mapV, sbase, items, abort_flag, lane);
-        else if (warp == 9) qload_warp<D>(p, &mapQ, sbase, items, abort_flag, lane);
-        else mma_warp<D>(p, sbase, tmem, items, abort_flag, warp - 10, lane);
+        // the producer sits on sub-partition 1: sub-partition 0 hosts the only active softmax warps of 32-row decodes
+        if (warp == 9) producer_warp<D>(p, &mapK, &mapV, sbase, items, abort_flag, kv_seq, lane);
+        else if (warp == 8) qload_warp<D>(p, &mapQ, sbase, items, abort_flag, lane);
+        else mma_warp<D>(p, sbase, tmem, items, abort_flag, kv_seq, warp - 10, lane);
     }
+#ifdef SANGAM_EXIT_DRAIN_NS
+    __nanosleep(SANGAM_EXIT_DRAIN_NS);                       // experiment: let stray asynchronous arrivals land
+#endif
     ptx::tc_fence_before();
     __syncthreads();
     TRACE_CTA(1);

@@ -262,6 +262,18 @@ extern "C" int sangam_iteration_host(sangam_ctx* ctx, const void* q_host, const 
     return SANGAM_OK;
 }
 
+#ifdef SANGAM_DEBUG_ITEM
+extern "C" int sangam_debug_bad_item(int* out16) {
+    cudaDeviceSynchronize();
+    return cudaMemcpyFromSymbol(out16, g_bad_item, 64) == cudaSuccess ? 0 : -4;
+}
+#endif
+// internal diagnostic (not part of include/sangam.h): which barrier the first watchdog timeout hit
+extern "C" int sangam_debug_timeout_info(unsigned int* out20) {
+    cudaDeviceSynchronize();
+    return cudaMemcpyFromSymbol(out20, ptx::g_timeout_info, 80) == cudaSuccess ? 0 : -4;
+}
+
 #ifdef SANGAM_TRACE
 extern "C" int sangam_trace_cta_times(unsigned long long* host_buf) {
     cudaDeviceSynchronize();
