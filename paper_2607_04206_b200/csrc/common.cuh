@@ -48,12 +48,12 @@ __device__ unsigned int g_trace_n[16];
 __device__ unsigned long long g_cta_times[2 * 256];   // per CTA: %globaltimer at entry / exit
 __device__ unsigned int g_trace_cta;     // which CTA records (sangam_trace_set_cta)
 __device__ __forceinline__ unsigned int* trace_cnt() {
-    __shared__ unsigned int cnt[16];
+    __shared__ unsigned int cnt[17];      // [16] = 1 if this CTA records (g_trace_cta read once: a global read per event costs an L2 trip)
     return cnt;
 }
 __device__ __forceinline__ void trace_ev(unsigned ev) {
     unsigned int* cnt = trace_cnt();
-    if (blockIdx.x == g_trace_cta && (threadIdx.x & 31) == 0) {
+    if (cnt[16] && (threadIdx.x & 31) == 0) {
         unsigned long long t;
         asm volatile("mov.u64 %0, %%clock64;" : "=l"(t));
         const unsigned w = threadIdx.x >> 5, i = cnt[w];
@@ -65,7 +65,7 @@ __device__ __forceinline__ void trace_ev(unsigned ev) {
 // same record, but the time stamp is %globaltimer (ns): start/end pair gives the effective SM clock
 __device__ __forceinline__ void trace_ns(unsigned ev) {
     unsigned int* cnt = trace_cnt();
-    if (blockIdx.x == g_trace_cta && (threadIdx.x & 31) == 0) {
+    if (cnt[16] && (threadIdx.x & 31) == 0) {
         unsigned long long t;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
         const unsigned w = threadIdx.x >> 5, i = cnt[w];
@@ -77,7 +77,7 @@ __device__ __forceinline__ void trace_ns(unsigned ev) {
 #define TRACE_EV(ev) trace_ev(ev)
 #define TRACE_NS(ev) trace_ns(ev)
 #define TRACE_CTA(which) do { if (threadIdx.x == 0 && blockIdx.x < 256) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_cta_times[2 * blockIdx.x + (which)] = t_; } } while (0)
-#define TRACE_INIT() do { if (threadIdx.x < 16) trace_cnt()[threadIdx.x] = 0; } while (0)
+#define TRACE_INIT() do { if (threadIdx.x < 16) trace_cnt()[threadIdx.x] = 0; if (threadIdx.x == 16) trace_cnt()[16] = blockIdx.x == g_trace_cta; __syncthreads(); } while (0)
 #else
 #define TRACE_EV(ev) ((void)0)
 #define TRACE_NS(ev) ((void)0)

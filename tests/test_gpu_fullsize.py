@@ -49,3 +49,12 @@ def test_full_size_config(oracle, cfg, per_req):
     torch.cuda.synchronize()
     assert np.array_equal(first, bits_of(s["out"]))
     assert w.eng.device_status() == 0
+    # back-to-back replays (kv_write -> attention -> combine with no host sync in between): timing-dependent
+    # protocol slips (a regression once showed up only here, in the hybrid config) would raise a device flag
+    # or change bits
+    for _ in range(3):
+        for _ in range(60):
+            w.iter_graphs[0].replay()
+        torch.cuda.synchronize()
+        assert w.eng.device_status() == 0
+        assert np.array_equal(first, bits_of(s["out"]))
