@@ -664,12 +664,19 @@ __device__ __forceinline__ float ex2_poly(float x) {
 // reference maximum m_ref stays).  m_ref is in log2 units and is only raised when the half's maximum
 // exceeds it by more than LAZY_T, so p = 2^(x - m_ref) <= 2^LAZY_T: exact in range for bf16 / fp32.
 // P (bf16 pairs) overwrites the first 32 columns of the half's S buffer.
-template <bool MASK, bool NEG>
+template <bool MASK>
 __device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float scale_log2, float& m_ref, float& l) {
     uint32_t r[2][32];
 #pragma unroll
     for (int c = 0; c < 2; ++c) ptx::tmem_ld32(s_taddr + (uint32_t)(c * 32), r[c]);
     ptx::tmem_wait_ld();
+    if (scale_log2 < 0.f) {                       // rare: max_j(scale * s_j) with scale < 0 -- work on -s with |scale|
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int i = 0; i < 32; ++i) r[c][i] ^= 0x80000000u;
+        scale_log2 = -scale_log2;
+    }
     float mx4[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
@@ -678,7 +685,6 @@ __device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float sc
         for (int i = 0; i < 16; i += 2) {
             const int col = c * 16 + i;
             float v0 = __uint_as_float(r[col >> 5][col & 31]), v1 = __uint_as_float(r[col >> 5][(col & 31) + 1]);
-            if (NEG) { v0 = -v0; v1 = -v1; }
             if (MASK) {
                 if (col >= nv) v0 = -INFINITY;
                 if (col + 1 >= nv) v1 = -INFINITY;
@@ -722,7 +728,7 @@ __device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float sc
 // out row (bf16) <- (w0 * O0 [+ w1 * O1]) scaled;  TMEM loads are warp-collective, stores predicated
 template <int D, bool TWO>
 __device__ __forceinline__ void store_final_row(uint32_t o0_taddr, uint32_t o1_taddr, float w0, float w1, bool row_ok, uint4* dst) {
-#pragma unroll
+#pragma unroll 1
     for (int c = 0; c < D / 32; ++c) {
         uint32_t o[32], o1[32];
         ptx::tmem_ld32(o0_taddr + (uint32_t)(c * 32), o);
@@ -749,7 +755,7 @@ __device__ __forceinline__ void store_final_row(uint32_t o0_taddr, uint32_t o1_t
 // a warp's 32 rows of one column group are 512 contiguous bytes, so these stores and the merge's loads coalesce.
 template <int D, bool TWO>
 __device__ __forceinline__ void store_partial_row(uint32_t o0_taddr, uint32_t o1_taddr, float w0, float w1, bool row_ok, float4* po) {
-#pragma unroll
+#pragma unroll 1
     for (int c = 0; c < D / 32; ++c) {
         uint32_t o[32], o1[32];
         ptx::tmem_ld32(o0_taddr + (uint32_t)(c * 32), o);
@@ -807,8 +813,8 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
             const int tile = shared ? it.kv0 + i : it.kv0 + 2 * i + s;
             int nvt = it.c - tile * BN;
             nvt = nvt > BN ? BN : nvt;
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
+#pragma unroll 1
+            for (int h = 0; h < 2; ++h) {                     // not unrolled: one copy of the softmax code (instruction cache)
                 const int nv = nvt - h * 64 > 64 ? 64 : nvt - h * 64;
                 if (nv <= 0) continue;                       // the context's last tile may lack half B
                 uint32_t& hcnt = h ? hcount1 : hcount0;
@@ -820,13 +826,8 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
                 if (warp_active) {
                     const uint32_t sh = s_taddr + (uint32_t)(h * 64);
                     float alpha;
-                    if (p.scale_log2 >= 0.f) {
-                        if (nv == 64) alpha = softmax_half<false, false>(sh, nv, p.scale_log2, m, l);
-                        else alpha = softmax_half<true, false>(sh, nv, p.scale_log2, m, l);
-                    } else {
-                        if (nv == 64) alpha = softmax_half<false, true>(sh, nv, p.scale_log2, m, l);
-                        else alpha = softmax_half<true, true>(sh, nv, p.scale_log2, m, l);
-                    }
+                    if (nv == 64) alpha = softmax_half<false>(sh, nv, p.scale_log2, m, l);
+                    else alpha = softmax_half<true>(sh, nv, p.scale_log2, m, l);
                     if (steps > 0 && __any_sync(FULL, alpha != 1.f)) {
                         // rare (lazy reference maximum): every PV handed over so far must have landed in O first.
                         // Per half at most the latest one is still in flight (the S_FULL just seen was committed
@@ -834,7 +835,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
                         ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s), (pv0 - 1u) & 1u, abort_flag);
                         ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s + 1), (pv1 - 1u) & 1u, abort_flag);
                         ptx::tc_fence_after();
-#pragma unroll
+#pragma unroll 1
                         for (int c = 0; c < D / 32; ++c) {
                             uint32_t o[32];
                             ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
