@@ -347,7 +347,16 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                 const int tile = it.kv0 + j;
                 return (j < n && pg < 8 && pg < pages_total - tile * 8) ? __ldg(bt + tile * 8 + pg) : 0;
             };
-            auto load_tile = [&](int j, int page, bool is_v) {
+            // One loop, one copy of the load code (instruction footprint): K runs `lead` tiles ahead of V.  The page
+            // ids of the tiles in flight (at most lead + 2) live in a 4-entry register window indexed by tile & 3; the
+            // entry of tile kq + 1 is fetched while tile kq's K load is issued, one K step before it is needed.
+            int w0 = ld_page(0), w1 = ld_page(1), w2 = 0, w3 = 0;
+            int kq = 0, vq = 0;
+            while (vq < n) {
+                const bool is_v = !(kq < n && kq < vq + lead);
+                const int j = is_v ? vq : kq;
+                const int sel = j & 3;
+                const int page = sel == 0 ? w0 : sel == 1 ? w1 : sel == 2 ? w2 : w3;
                 const int tile = it.kv0 + j;
                 ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), phase ^ 1u, abort_flag);
                 int np = pages_total - tile * 8;
@@ -366,15 +375,13 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                 }
                 TRACE_EV(54);
                 if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
-            };
-            int w0 = ld_page(0), w1 = ld_page(1), w2 = ld_page(2);
-            load_tile(0, w0, false);
-            if (lead == 2 && n > 1) load_tile(1, w1, false);
-            for (int j = 0; j < n; ++j) {
-                const int nxt = ld_page(j + 3);
-                load_tile(j, w0, true);
-                if (j + lead < n) load_tile(j + lead, lead == 1 ? w1 : w2, false);
-                w0 = w1; w1 = w2; w2 = nxt;
+                if (is_v) {
+                    ++vq;
+                } else {
+                    ++kq;
+                    const int nx = ld_page(kq + 1), s2 = (kq + 1) & 3;       // prefetch for the K load after the next
+                    if (s2 == 0) w0 = nx; else if (s2 == 1) w1 = nx; else if (s2 == 2) w2 = nx; else w3 = nx;
+                }
                 if (*abort_flag) break;
             }
         }
@@ -577,66 +584,61 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
         TRACE_EV(1 + s);
         const int n = it.kv1 - it.kv0, c = it.c, kv0 = it.kv0;
         if (n > 0) {
-            if (it.rows1 > 0) {
-                // SHARED: stream s = q tile s; ring order K_0 V_0 K_1 V_1 ..., every stage read by both issuers
-                const uint32_t qc = qcount + (uint32_t)s, qs = qc & 1u, qo = qcount + (uint32_t)(s ^ 1);
+            // One loop serves both modes (a single copy of the issue code: instruction footprint).
+            //   SHARED: stream s = q tile s; ring order K_0 | V_0 K_1 | V_1 K_2 ..., every stage read by both issuers.
+            //   SPLIT:  one q tile read by both issuers; stream x owns kv tiles kv0 + 2i + x and their stages; ring order
+            //           K(0,0) [K(1,0)] | V(0,i) [K(0,i+1)] [V(1,i)] [K(1,i+1)] | ...
+            // Round i = -1 is the prologue (first QK only); round i >= 0 issues PV of step i and QK of step i + 1.
+            const bool shared = it.rows1 > 0;
+            const int n0 = shared ? n : (n + 1) >> 1, n1 = shared ? n : n >> 1, ns = s ? n1 : n0;
+            const uint32_t qc = shared ? qcount + (uint32_t)s : qcount, qs = qc & 1u;
+            if (shared) {
                 // The other stream's q tile is only observed, and only for items so short that this issuer could
                 // finish them before that tile has landed (same parity-aliasing hazard as for the K/V ring).
+                const uint32_t qo = qcount + (uint32_t)(s ^ 1);
                 if (n <= NSTAGE) ptx::mbar_wait(st.bar(L::B_Q_FULL + (qo & 1u)), (qo >> 1) & 1u, abort_flag);
-                ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qc >> 1) & 1u, abort_flag);
-                uint32_t sk = st.acquire();
-                tile_steps<D>(st, s, c, -1, false, 0u, kv0, sk, qs, 1, n == 1 ? 2 : 0);
-                for (int j = 0; j < n; ++j) {
-                    const bool more = j + 1 < n;
-                    const uint32_t sv = st.acquire();
-                    const int nv = c - (kv0 + j) * BN;
-                    if (nv < BN && (nv & 15)) {              // tail tile: issuer 0 zero-fills, issuer 1 waits for it
-                        if (s == 0) {
-                            zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
-                            if (lane == 0) ptx::mbar_arrive(st.bar(L::B_ZFILL));
-                        } else {
-                            ptx::mbar_wait(st.bar(L::B_ZFILL), st.zf_par, abort_flag);
-                        }
-                        st.zf_par ^= 1u;
-                    }
-                    if (more) sk = st.acquire();
-                    tile_steps<D>(st, s, c, kv0 + j, j == 0, sv, more ? kv0 + j + 1 : -1, sk, qs, 1, (more && j + 2 == n) ? 2 : 0);
-                }
-                qcount += 2;
-            } else {
-                // SPLIT: one q tile read by both issuers; stream s owns kv tiles kv0 + 2i + s and their stages.
-                // Ring order: K(0,0) [K(1,0)] | V(0,i) [K(0,i+1)] [V(1,i)] [K(1,i+1)] | ...
-                const uint32_t qs = qcount & 1u;
-                const int n0 = (n + 1) >> 1, n1 = n >> 1, ns = s ? n1 : n0;
-                ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qcount >> 1) & 1u, abort_flag);
-                TRACE_EV(3 + s);
-                uint32_t sk = 0, sv = 0;
-                if (s == 0) sk = st.acquire(); else st.skip();
-                if (n1 > 0) { if (s == 1) sk = st.acquire(); else st.skip(); }
-                TRACE_EV(5 + s);
-                if (ns > 0) { tile_steps<D>(st, s, c, -1, false, 0u, kv0 + s, sk, qs, 2, ns == 1 ? 1 : 0); TRACE_EV(7 + s); }
-                else if (lane == 0) ptx::mbar_arrive(st.bar(L::B_Q_EMPTY + qs));      // nothing to read: release the q tile
-                for (int i = 0; i < n0; ++i) {
-#pragma unroll
-                    for (int x = 0; x < 2; ++x) {            // stream x's pair of stages: V(x, i) [K(x, i+1)]
-                        const int nx = x ? n1 : n0;
-                        if (i >= nx) continue;
-                        const bool more = i + 1 < nx;
-                        if (s == x) {
-                            sv = st.acquire();
-                            const int tile = kv0 + 2 * i + x;
-                            const int nv = c - tile * BN;
-                            if (nv < BN && (nv & 15)) zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
-                            if (more) sk = st.acquire();
-                            tile_steps<D>(st, s, c, tile, i == 0, sv, more ? tile + 2 : -1, sk, qs, 2, (more && i + 2 == nx) ? 1 : 0);
-                        } else {
-                            st.skip();
-                            if (more) st.skip();
-                        }
-                    }
-                }
-                qcount += 1;
             }
+            ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qc >> 1) & 1u, abort_flag);
+            TRACE_EV(3 + s);
+            if (!shared && ns == 0 && lane == 0) ptx::mbar_arrive(st.bar(L::B_Q_EMPTY + qs));   // nothing to read: release the q tile
+            uint32_t sk = 0, sv = 0;
+            for (int i = -1; i < n0; ++i) {
+                bool work = false;
+                int tile = -1, next = -1;
+#pragma unroll
+                for (int x = 0; x < 2; ++x) {                // SHARED: one pass (x = s); SPLIT: stream 0's stages, then stream 1's
+                    if (shared && x != s) continue;
+                    const int nx = x ? n1 : n0;
+                    const bool has_v = i >= 0 && i < nx, has_k = i + 1 < nx;
+                    if (x != s) {                            // the other issuer's stages (SPLIT)
+                        if (has_v) st.skip();
+                        if (has_k) st.skip();
+                        continue;
+                    }
+                    if (has_v) {
+                        sv = st.acquire();
+                        tile = shared ? kv0 + i : kv0 + 2 * i + x;
+                        const int nv = c - tile * BN;
+                        if (nv < BN && (nv & 15)) {          // tail tile: stale rows of the last page
+                            if (!shared || s == 0) zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
+                            if (shared) {                    // issuer 0 zero-fills, issuer 1 waits for it
+                                if (s == 0) { if (lane == 0) ptx::mbar_arrive(st.bar(L::B_ZFILL)); }
+                                else ptx::mbar_wait(st.bar(L::B_ZFILL), st.zf_par, abort_flag);
+                                st.zf_par ^= 1u;
+                            }
+                        }
+                    }
+                    if (has_k) {
+                        sk = st.acquire();
+                        next = shared ? kv0 + i + 1 : kv0 + 2 * (i + 1) + x;
+                    }
+                    work = has_v || has_k;
+                }
+                if (work)
+                    tile_steps<D>(st, s, c, tile, i == 0, sv, next, sk, qs, shared ? 1 : 2,
+                                  (next >= 0 && i + 2 == ns) ? (shared ? 2 : 1) : 0);
+            }
+            qcount += shared ? 2u : 1u;
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(st.bar(L::B_ITEM_EMPTY + islot));
@@ -725,52 +727,40 @@ __device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float sc
     return alpha;
 }
 
-// out row (bf16) <- (w0 * O0 [+ w1 * O1]) scaled;  TMEM loads are warp-collective, stores predicated
-template <int D, bool TWO>
-__device__ __forceinline__ void store_final_row(uint32_t o0_taddr, uint32_t o1_taddr, float w0, float w1, bool row_ok, uint4* dst) {
+// One row of the epilogue from TMEM, 32 columns at a time (TMEM loads are warp-collective, stores predicated):
+//   final:   out row (bf16)          <- w0 * O0 [+ w1 * O1]      (w's already contain 1 / l)
+//   partial: slot row (fp32, unnormalised) <- w0 * O0 [+ w1 * O1];  slot layout [D/4 column groups][256 rows][4 floats]:
+//            a warp's 32 rows of one column group are 512 contiguous bytes, so these stores and the merge's loads coalesce.
+// One copy of this code serves every mode (`two`, `partial` are warp-uniform run-time flags): the kernel's instruction
+// footprint matters more than the few predicated instructions.
+template <int D>
+__device__ __forceinline__ void store_row(uint32_t o0_taddr, uint32_t o1_taddr, bool two, float w0, float w1, bool row_ok,
+                                          bool partial, uint4* dst, float4* po) {
 #pragma unroll 1
     for (int c = 0; c < D / 32; ++c) {
         uint32_t o[32], o1[32];
         ptx::tmem_ld32(o0_taddr + (uint32_t)(c * 32), o);
-        if (TWO) ptx::tmem_ld32(o1_taddr + (uint32_t)(c * 32), o1);
+        if (two) ptx::tmem_ld32(o1_taddr + (uint32_t)(c * 32), o1);
         ptx::tmem_wait_ld();
-        if (row_ok) {
+        float f[32];
 #pragma unroll
-            for (int v = 0; v < 4; ++v) {
-                float f[8];
+        for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(o[e]) * w0;
+        if (two) {
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    f[e] = __uint_as_float(o[v * 8 + e]) * w0;
-                    if (TWO) f[e] = fmaf(__uint_as_float(o1[v * 8 + e]), w1, f[e]);
-                }
-                uint4 w;
-                w.x = ptx::pack_bf16(f[0], f[1]); w.y = ptx::pack_bf16(f[2], f[3]);
-                w.z = ptx::pack_bf16(f[4], f[5]); w.w = ptx::pack_bf16(f[6], f[7]);
-                dst[c * 4 + v] = w;
-            }
+            for (int e = 0; e < 32; ++e) f[e] = fmaf(__uint_as_float(o1[e]), w1, f[e]);
         }
-    }
-}
-// partial row (fp32, unnormalised) <- w0 * O0 [+ w1 * O1].  Slot layout [D/4 column groups][256 rows][4 floats]:
-// a warp's 32 rows of one column group are 512 contiguous bytes, so these stores and the merge's loads coalesce.
-template <int D, bool TWO>
-__device__ __forceinline__ void store_partial_row(uint32_t o0_taddr, uint32_t o1_taddr, float w0, float w1, bool row_ok, float4* po) {
-#pragma unroll 1
-    for (int c = 0; c < D / 32; ++c) {
-        uint32_t o[32], o1[32];
-        ptx::tmem_ld32(o0_taddr + (uint32_t)(c * 32), o);
-        if (TWO) ptx::tmem_ld32(o1_taddr + (uint32_t)(c * 32), o1);
-        ptx::tmem_wait_ld();
         if (row_ok) {
+            if (partial) {
 #pragma unroll
-            for (int v = 0; v < 8; ++v) {
-                float f[4];
+                for (int v = 0; v < 8; ++v) po[(c * 8 + v) * PAIR] = make_float4(f[v * 4], f[v * 4 + 1], f[v * 4 + 2], f[v * 4 + 3]);
+            } else {
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    f[e] = __uint_as_float(o[v * 4 + e]) * w0;
-                    if (TWO) f[e] = fmaf(__uint_as_float(o1[v * 4 + e]), w1, f[e]);
+                for (int v = 0; v < 4; ++v) {
+                    uint4 w;
+                    w.x = ptx::pack_bf16(f[v * 8 + 0], f[v * 8 + 1]); w.y = ptx::pack_bf16(f[v * 8 + 2], f[v * 8 + 3]);
+                    w.z = ptx::pack_bf16(f[v * 8 + 4], f[v * 8 + 5]); w.w = ptx::pack_bf16(f[v * 8 + 6], f[v * 8 + 7]);
+                    dst[c * 4 + v] = w;
                 }
-                po[(c * 8 + v) * PAIR] = make_float4(f[0], f[1], f[2], f[3]);
             }
         }
     }
@@ -880,6 +870,9 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         const int prow = ((shared && s == 1) ? BM : 0) + row;                 // row inside the partial slot
         float4* po = reinterpret_cast<float4*>(p.part_o) + (int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * (D / 4) * PAIR + prow;
         float2* pml = reinterpret_cast<float2*>(p.part_ml) + (int64_t)(it.part_slot < 0 ? 0 : it.part_slot) * PAIR + prow;
+        const bool partial = it.part_slot >= 0;
+        bool do_store = false, two = false;
+        float w0 = 1.f, w1 = 0.f, m_out = m, l_out = l;
         if (n == 0) {
             // empty context: zeros (reading S13); never split
             if (row_ok && (shared || s == 0)) {
@@ -887,39 +880,36 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
                 for (int c = 0; c < D / 8; ++c) dst[c] = make_uint4(0, 0, 0, 0);
             }
         } else if (shared) {
-            if (warp_active) {
-                if (it.part_slot < 0) {
-                    store_final_row<D, false>(o_taddr, o_taddr, l > 0.f ? 1.f / l : 0.f, 0.f, row_ok, dst);
-                } else {
-                    store_partial_row<D, false>(o_taddr, o_taddr, 1.f, 0.f, row_ok, po);
-                    if (row_ok) *pml = make_float2(m, l);
-                }
-            }
+            do_store = warp_active;
         } else {
             // SPLIT: stream 1 hands (m, l) to stream 0, which merges O_0 and O_1
             if (s == 1) {
                 ml_x[row] = make_float2(m, l);
                 ptx::mbar_arrive(bar(L::B_EPI_A));
-                ptx::mbar_wait(bar(L::B_EPI_B), ecount & 1u, abort_flag);       // stream 0 is done reading O_1
             } else {
                 ptx::mbar_wait(bar(L::B_EPI_A), ecount & 1u, abort_flag);
                 TRACE_EV(37);
                 const float2 x = ml_x[row];
-                const float ms = fmaxf(m, x.x);
-                const bool two = n > 1;                                    // stream 1 had tiles
-                const float w0 = ptx::ex2(m - ms), w1 = two ? ptx::ex2(x.x - ms) : 0.f;
-                const float ls = l * w0 + x.y * w1;
-                if (warp_active) {
-                    if (it.part_slot < 0) {
-                        const float inv = ls > 0.f ? 1.f / ls : 0.f;
-                        if (two) store_final_row<D, true>(o_taddr, o_other, w0 * inv, w1 * inv, row_ok, dst);
-                        else store_final_row<D, false>(o_taddr, o_taddr, w0 * inv, 0.f, row_ok, dst);
-                    } else {
-                        if (two) store_partial_row<D, true>(o_taddr, o_other, w0, w1, row_ok, po);
-                        else store_partial_row<D, false>(o_taddr, o_taddr, w0, 0.f, row_ok, po);
-                        if (row_ok) *pml = make_float2(ms, ls);
-                    }
-                }
+                m_out = fmaxf(m, x.x);
+                two = n > 1;                                               // stream 1 had tiles
+                w0 = ptx::ex2(m - m_out);
+                w1 = two ? ptx::ex2(x.x - m_out) : 0.f;
+                l_out = l * w0 + x.y * w1;
+                do_store = warp_active;
+            }
+        }
+        if (do_store) {
+            if (!partial) {
+                const float inv = l_out > 0.f ? 1.f / l_out : 0.f;
+                w0 *= inv; w1 *= inv;
+            }
+            store_row<D>(o_taddr, o_other, two, w0, w1, row_ok, partial, dst, po);
+            if (partial && row_ok) *pml = make_float2(m_out, l_out);
+        }
+        if (n > 0 && !shared) {
+            if (s == 1) {
+                ptx::mbar_wait(bar(L::B_EPI_B), ecount & 1u, abort_flag);       // stream 0 is done reading O_1
+            } else {
                 ptx::tc_fence_before();
                 ptx::mbar_arrive(bar(L::B_EPI_B));
             }
