@@ -99,15 +99,11 @@ struct Smem {
 static_assert(sizeof(Item) == 64, "Item is 64 bytes");
 static_assert(Smem<128>::ALLOC <= 232448, "shared memory budget (227 KB)");
 
-// floor(a * b / d) for non-negative a, b and d > 0: 32-bit division whenever the product fits (64-bit division is slow)
-__device__ __forceinline__ int mul_div(int a, int b, int d) {
-    const uint64_t prod = (uint64_t)(uint32_t)a * (uint32_t)b;
-    return (prod >> 32) == 0 ? (int)((uint32_t)prod / (uint32_t)d) : (int)(prod / (uint32_t)d);
-}
-__device__ __forceinline__ int mul_div_ceil(int64_t a, int b, int d) {   // ceil(a * b / d), a < 2^31
-    const uint64_t prod = (uint64_t)a * (uint32_t)b + (uint32_t)d - 1u;
-    return (prod >> 32) == 0 ? (int)((uint32_t)prod / (uint32_t)d) : (int)(prod / (uint32_t)d);
-}
+// floor(a * b / d) and ceil(a * b / d) for the static partition.  32-bit arithmetic only (a 64-bit division is some
+// 150 instructions of cold code per call site): the static partition is used only while T * #CTAs < 2^31, larger
+// batches are handed out dynamically.
+__device__ __forceinline__ int mul_div(int a, int b, int d) { return (int)(((uint32_t)a * (uint32_t)b) / (uint32_t)d); }
+__device__ __forceinline__ int mul_div_ceil(int a, int b, int d) { return (int)(((uint32_t)a * (uint32_t)b + (uint32_t)d - 1u) / (uint32_t)d); }
 
 struct ReqInfo {
     int q0, qn, c, np, tiles_u, units;
@@ -194,7 +190,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
         U += __shfl_xor_sync(FULL, U, o);
         T += __shfl_xor_sync(FULL, T, o);
     }
-    const bool dynamic = U >= DYN_UNITS_PER_CTA * G_ctas;
+    const bool dynamic = U >= DYN_UNITS_PER_CTA * G_ctas || T >= (int)(0x7fffffffu / (uint32_t)(G_ctas + 1));
     TRACE_EV(51);
 
     // walking state
@@ -563,6 +559,9 @@ __device__ __forceinline__ void tile_steps(MmaState<D>& st, int s, int c, int ti
     if (pb > 0 || qb > 0) half_step<D>(st, s, 1, pb > 0 ? pb : 0, false, sv, rel, qb > 0 ? qb : 0, sk, qs, rel, q_rel);
 }
 
+struct SharedMode { static constexpr bool value = true; };
+struct SplitMode { static constexpr bool value = false; };
+
 template <int D>
 __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, uint32_t tmem, const Item* items,
                                          volatile uint32_t* abort_flag, uint32_t* kv_seq_smem, int s, int lane) {
@@ -589,56 +588,60 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
             //   SPLIT:  one q tile read by both issuers; stream x owns kv tiles kv0 + 2i + x and their stages; ring order
             //           K(0,0) [K(1,0)] | V(0,i) [K(0,i+1)] [V(1,i)] [K(1,i+1)] | ...
             // Round i = -1 is the prologue (first QK only); round i >= 0 issues PV of step i and QK of step i + 1.
-            const bool shared = it.rows1 > 0;
-            const int n0 = shared ? n : (n + 1) >> 1, n1 = shared ? n : n >> 1, ns = s ? n1 : n0;
-            const uint32_t qc = shared ? qcount + (uint32_t)s : qcount, qs = qc & 1u;
-            if (shared) {
-                // The other stream's q tile is only observed, and only for items so short that this issuer could
-                // finish them before that tile has landed (same parity-aliasing hazard as for the K/V ring).
-                const uint32_t qo = qcount + (uint32_t)(s ^ 1);
-                if (n <= NSTAGE) ptx::mbar_wait(st.bar(L::B_Q_FULL + (qo & 1u)), (qo >> 1) & 1u, abort_flag);
-            }
-            ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qc >> 1) & 1u, abort_flag);
-            TRACE_EV(3 + s);
-            if (!shared && ns == 0 && lane == 0) ptx::mbar_arrive(st.bar(L::B_Q_EMPTY + qs));   // nothing to read: release the q tile
-            uint32_t sk = 0, sv = 0;
-            for (int i = -1; i < n0; ++i) {
-                bool work = false;
-                int tile = -1, next = -1;
-#pragma unroll
-                for (int x = 0; x < 2; ++x) {                // SHARED: one pass (x = s); SPLIT: stream 0's stages, then stream 1's
-                    if (shared && x != s) continue;
-                    const int nx = x ? n1 : n0;
-                    const bool has_v = i >= 0 && i < nx, has_k = i + 1 < nx;
-                    if (x != s) {                            // the other issuer's stages (SPLIT)
-                        if (has_v) st.skip();
-                        if (has_k) st.skip();
-                        continue;
-                    }
-                    if (has_v) {
-                        sv = st.acquire();
-                        tile = shared ? kv0 + i : kv0 + 2 * i + x;
-                        const int nv = c - tile * BN;
-                        if (nv < BN && (nv & 15)) {          // tail tile: stale rows of the last page
-                            if (!shared || s == 0) zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
-                            if (shared) {                    // issuer 0 zero-fills, issuer 1 waits for it
-                                if (s == 0) { if (lane == 0) ptx::mbar_arrive(st.bar(L::B_ZFILL)); }
-                                else ptx::mbar_wait(st.bar(L::B_ZFILL), st.zf_par, abort_flag);
-                                st.zf_par ^= 1u;
+            // (instantiated once per mode: the mode tests fold away in the hot SHARED loop of prefill)
+            auto rounds = [&](auto shared_c) {
+                constexpr bool shared = decltype(shared_c)::value;
+                const int n0 = shared ? n : (n + 1) >> 1, n1 = shared ? n : n >> 1, ns = s ? n1 : n0;
+                const uint32_t qc = shared ? qcount + (uint32_t)s : qcount, qs = qc & 1u;
+                if (shared) {
+                    // The other stream's q tile is only observed, and only for items so short that this issuer could
+                    // finish them before that tile has landed (same parity-aliasing hazard as for the K/V ring).
+                    const uint32_t qo = qcount + (uint32_t)(s ^ 1);
+                    if (n <= NSTAGE) ptx::mbar_wait(st.bar(L::B_Q_FULL + (qo & 1u)), (qo >> 1) & 1u, abort_flag);
+                }
+                ptx::mbar_wait(st.bar(L::B_Q_FULL + qs), (qc >> 1) & 1u, abort_flag);
+                TRACE_EV(3 + s);
+                if (!shared && ns == 0 && lane == 0) ptx::mbar_arrive(st.bar(L::B_Q_EMPTY + qs));   // nothing to read: release the q tile
+                uint32_t sk = 0, sv = 0;
+                for (int i = -1; i < n0; ++i) {
+                    bool work = false;
+                    int tile = -1, next = -1;
+    #pragma unroll
+                    for (int x = 0; x < 2; ++x) {                // SHARED: one pass (x = s); SPLIT: stream 0's stages, then stream 1's
+                        if (shared && x != s) continue;
+                        const int nx = x ? n1 : n0;
+                        const bool has_v = i >= 0 && i < nx, has_k = i + 1 < nx;
+                        if (x != s) {                            // the other issuer's stages (SPLIT)
+                            if (has_v) st.skip();
+                            if (has_k) st.skip();
+                            continue;
+                        }
+                        if (has_v) {
+                            sv = st.acquire();
+                            tile = shared ? kv0 + i : kv0 + 2 * i + x;
+                            const int nv = c - tile * BN;
+                            if (nv < BN && (nv & 15)) {          // tail tile: stale rows of the last page
+                                if (!shared || s == 0) zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
+                                if (shared) {                    // issuer 0 zero-fills, issuer 1 waits for it
+                                    if (s == 0) { if (lane == 0) ptx::mbar_arrive(st.bar(L::B_ZFILL)); }
+                                    else ptx::mbar_wait(st.bar(L::B_ZFILL), st.zf_par, abort_flag);
+                                    st.zf_par ^= 1u;
+                                }
                             }
                         }
+                        if (has_k) {
+                            sk = st.acquire();
+                            next = shared ? kv0 + i + 1 : kv0 + 2 * (i + 1) + x;
+                        }
+                        work = has_v || has_k;
                     }
-                    if (has_k) {
-                        sk = st.acquire();
-                        next = shared ? kv0 + i + 1 : kv0 + 2 * (i + 1) + x;
-                    }
-                    work = has_v || has_k;
+                    if (work)
+                        tile_steps<D>(st, s, c, tile, i == 0, sv, next, sk, qs, shared ? 1 : 2,
+                                      (next >= 0 && i + 2 == ns) ? (shared ? 2 : 1) : 0);
                 }
-                if (work)
-                    tile_steps<D>(st, s, c, tile, i == 0, sv, next, sk, qs, shared ? 1 : 2,
-                                  (next >= 0 && i + 2 == ns) ? (shared ? 2 : 1) : 0);
-            }
-            qcount += shared ? 2u : 1u;
+                qcount += shared ? 2u : 1u;
+            };
+            if (it.rows1 > 0) rounds(SharedMode{}); else rounds(SplitMode{});
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(st.bar(L::B_ITEM_EMPTY + islot));

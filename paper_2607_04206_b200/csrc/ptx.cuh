@@ -68,44 +68,43 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
 #ifndef SANGAM_WAIT_TIMEOUT_NS
 #define SANGAM_WAIT_TIMEOUT_NS 2000000000ull
 #endif
-// Diagnostic of the first watchdog timeout since the library was loaded.  Every warp notes the barrier it is
-// blocked on in a small shared table that follows the abort word (abort_flag[3 + warp]); the warp whose watchdog
-// fires first dumps the whole table: [0] = its own barrier | 1<<31, [1] warp, [2] CTA, [3] parity, [4..19] the table.
+// Diagnostic of the first watchdog timeout (builds with -DSANGAM_WAIT_TABLE): [0] = barrier | 1<<31, [1] warp, [2] CTA,
+// [3] parity, [4..19] the barrier every warp of that CTA was blocked on.
 __device__ unsigned int g_timeout_info[20];
-__device__ __forceinline__ bool mbar_wait_slow(uint32_t bar, uint32_t parity, volatile uint32_t* abort_flag) {
-    if (*abort_flag) return false;
-    const uint32_t warp = threadIdx.x >> 5;
+
+// hot path: one try_wait; then suspending waits (the hardware resumes the thread when the phase completes) with a
+// watchdog every 16 expired 20-us suspensions.  The slow path is inlined at ~60 wait sites, so it is kept minimal (the
+// kernel's instruction footprint is a first-order performance factor; an out-of-line version costs spills around the
+// call in the hot loops); the diagnostics are compiled in only with -DSANGAM_WAIT_TABLE.
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile uint32_t* abort_flag) {
+    if (mbar_try_wait(bar, parity)) return true;
 #ifdef SANGAM_WAIT_TABLE
-    if ((threadIdx.x & 31) == 0) abort_flag[3 + warp] = bar | (parity << 31);
+    if ((threadIdx.x & 31) == 0) abort_flag[3 + (threadIdx.x >> 5)] = bar | (parity << 31);
 #endif
     uint64_t t0 = 0;
     uint32_t spins = 0;
-    bool ok = false;
-    while (true) {
-        if (mbar_try_wait_hint(bar, parity, 20000u)) { ok = true; break; }
+    bool ok = true;
+    while (!mbar_try_wait_hint(bar, parity, 20000u)) {
         if ((++spins & 0xFu) == 0) {
-            if (*abort_flag) break;
             const uint64_t now = globaltimer_ns();
             if (t0 == 0) t0 = now;
-            else if (now - t0 > SANGAM_WAIT_TIMEOUT_NS) {
-                if (atomicCAS(&g_timeout_info[0], 0u, bar | 0x80000000u) == 0u) {
-                    g_timeout_info[1] = warp; g_timeout_info[2] = blockIdx.x; g_timeout_info[3] = parity;
+            if (*abort_flag || now - t0 > SANGAM_WAIT_TIMEOUT_NS) {
+#ifdef SANGAM_WAIT_TABLE
+                if (!*abort_flag && atomicCAS(&g_timeout_info[0], 0u, bar | 0x80000000u) == 0u) {
+                    g_timeout_info[1] = threadIdx.x >> 5; g_timeout_info[2] = blockIdx.x; g_timeout_info[3] = parity;
                     for (int k = 0; k < 16; ++k) g_timeout_info[4 + k] = abort_flag[3 + k];
                 }
+#endif
                 *abort_flag = 1u;
+                ok = false;
                 break;
             }
         }
     }
 #ifdef SANGAM_WAIT_TABLE
-    if ((threadIdx.x & 31) == 0) abort_flag[3 + warp] = 0u;
+    if ((threadIdx.x & 31) == 0) abort_flag[3 + (threadIdx.x >> 5)] = 0u;
 #endif
     return ok;
-}
-// hot path: one try_wait; everything else (suspending wait, abort flag, timeout) is out of line
-__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile uint32_t* abort_flag) {
-    if (mbar_try_wait(bar, parity)) return true;
-    return mbar_wait_slow(bar, parity, abort_flag);
 }
 
 __device__ __forceinline__ void fence_proxy_async_smem() {
