@@ -48,7 +48,7 @@ constexpr int SLAB = 128 * 128;  // bytes of one 64-wide swizzled slab of a 128-
 #endif
 constexpr int DYN_UNITS_PER_CTA = SANGAM_DYN_UNITS;   // >= this many units per CTA: whole units, dynamic hand-out
 #ifndef SANGAM_UNIT_OV
-#define SANGAM_UNIT_OV 3
+#define SANGAM_UNIT_OV 1
 #endif
 constexpr int UNIT_OV = SANGAM_UNIT_OV;  // static partition: fixed cost of starting/finishing a unit, in kv-tile equivalents
 constexpr float LAZY_T = 8.f;    // the reference maximum moves only when a tile exceeds it by 2^8
