@@ -98,7 +98,7 @@ int sangam_kv_write(sangam_ctx* ctx, const void* k, const void* v, const int32_t
  *   s_j = scale * <q[t][h], K_r[j][g]>, j < c;   out[t][h] = sum_j softmax_j(s) V_r[j][g]
  * with K_r[j] = k_pages[block_table[r][j/16]][g][j%16].  No mask among j < c.  c = 0 writes zeros.
  * bf16 inputs, fp32 accumulation, P rounded to bf16 before PV, out = bf16(O / l).
- * Long contexts are split over CTAs and merged inside the same kernel in fixed order; results are bitwise
+ * Long contexts are split over CTAs and merged by a combine kernel in fixed order; results are bitwise
  * reproducible for fixed inputs.  `total_q` is the host-known number of rows of q/out
  * (an upper bound is fine: rows past cu_q_lens[batch] are not touched).
  */

@@ -88,7 +88,7 @@ struct Smem {
     static constexpr int B_KV_FULL = 0, B_KV_EMPTY = NSTAGE, B_ITEM_FULL = 2 * NSTAGE, B_ITEM_EMPTY = B_ITEM_FULL + 2,
                          B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 2, B_S_FULL = B_Q_EMPTY + 2,   // [stream][half]
                          B_P_FULL = B_S_FULL + 4, B_PV_DONE = B_P_FULL + 4, B_EPI_A = B_PV_DONE + 4,
-                         B_EPI_B = B_EPI_A + 1, B_EPI_C = B_EPI_B + 1, B_EPI_D = B_EPI_C + 1, B_ZFILL = B_EPI_D + 1, NBAR = B_ZFILL + 1;
+                         B_EPI_B = B_EPI_A + 1, B_ZFILL = B_EPI_B + 1, NBAR = B_ZFILL + 1;
     static constexpr int OFF_ITEMS = OFF_BAR + ((NBAR * 8 + 15) / 16) * 16;
     static constexpr int OFF_ML = OFF_ITEMS + 2 * (int)sizeof(Item);    // (m, l) of stream 1, 128 rows
     static constexpr int OFF_MISC = OFF_ML + BM * 8;
@@ -797,9 +797,6 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         const int rows_valid = (shared && s == 1) ? it.rows1 : it.rows0;
         const bool warp_active = wg_warp * 32 < rows_valid;
         float m = -INFINITY, l = 0.f;
-#ifdef SANGAM_DESYNC_NS
-        if (s == 1) __nanosleep(SANGAM_DESYNC_NS);           // experiment: start stream 1 out of phase with stream 0
-#endif
         uint32_t steps = 0;                                    // half tiles of this item handed to the issuer
         for (int i = 0; i < ns; ++i) {
             if (*abort_flag) break;
@@ -963,8 +960,6 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
         }
         ptx::mbar_init(bar(L::B_EPI_A), 128);
         ptx::mbar_init(bar(L::B_EPI_B), 128);
-        ptx::mbar_init(bar(L::B_EPI_C), 256);
-        ptx::mbar_init(bar(L::B_EPI_D), 1);
         ptx::mbar_init(bar(L::B_ZFILL), 1);
         *abort_flag = 0u;
         for (int k = 0; k < 16; ++k) abort_flag[3 + k] = 0u;
@@ -996,9 +991,6 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
         else if (warp == 8) qload_warp<D>(p, &mapQ, sbase, items, abort_flag, lane);
         else mma_warp<D>(p, sbase, tmem, items, abort_flag, kv_seq, warp - 10, lane);
     }
-#ifdef SANGAM_EXIT_DRAIN_NS
-    __nanosleep(SANGAM_EXIT_DRAIN_NS);                       // experiment: let stray asynchronous arrivals land
-#endif
     ptx::tc_fence_before();
     __syncthreads();
     TRACE_CTA(1);
