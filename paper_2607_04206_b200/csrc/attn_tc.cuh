@@ -198,6 +198,11 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
     ReqInfo cur = ReqCache::derive(p, 0, 0, 0);
     cur.units = 0;
     if (R > 0) cur = rc.get(p, 0);
+    if (dynamic && R > 0) {                            // dynamic tickets walk downwards from the last request
+        r_cur = R - 1;
+        cur = rc.get(p, r_cur);
+        ubase = U - cur.units;
+    }
     TRACE_EV(55);
     if (!dynamic && T > 0) {
         Geff = G_ctas < T ? G_ctas : T;
@@ -251,13 +256,17 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
             if (lane == 0) u = atomicAdd(p.sched, 1);
             u = __shfl_sync(FULL, u, 0);
             if (u < U) {
-                while (r_cur < R && u >= ubase + cur.units) {
-                    ubase += cur.units;
-                    ++r_cur;
-                    if (r_cur < R) cur = rc.get(p, r_cur);
+                // Tickets walk the unit list from the END: Alg. 1 batches seat decodes first and prefills last
+                // (PAPER.md:181-190), so the long prefill units start first and the short decode units fill the
+                // tail of the launch (longest-first balance).
+                const int uu = U - 1 - u;
+                while (r_cur > 0 && uu < ubase) {
+                    --r_cur;
+                    cur = rc.get(p, r_cur);
+                    ubase -= cur.units;
                 }
                 if (r_cur < R) {
-                    const int ul = u - ubase;
+                    const int ul = uu - ubase;
                     it.valid = 1; it.r = r_cur; it.g = ul / cur.np;
                     it.tok0 = (ul - it.g * cur.np) * 2 * p.tpt;
                     it.kv0 = 0; it.kv1 = cur.tiles_u;
