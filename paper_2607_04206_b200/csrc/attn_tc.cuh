@@ -129,7 +129,9 @@ struct ReqCache {
     __device__ __forceinline__ static ReqInfo derive(const AttnParams& p, int q0_, int qn_, int c_) {
         ReqInfo x;
         x.q0 = q0_; x.qn = qn_; x.c = c_;
-        x.np = (qn_ + 2 * p.tpt - 1) / (2 * p.tpt);      // a q tile holds tpt = 128 / G whole tokens (all G heads of each)
+        // a q tile holds tpt = 128 / G whole tokens (all G heads of each); ceil(qn / (2 tpt)) by the host's magic
+        // multiplier (exact for qn < 2^24): an integer division is ~25 instructions at each of this function's call sites
+        x.np = (int)__umulhi((uint32_t)(qn_ + 2 * p.tpt - 1), p.tpt2_magic);
         const int nkv = (c_ + BN - 1) / BN;
         x.tiles_u = nkv > 0 ? nkv : 1;
         x.units = p.Hkv * x.np;

@@ -25,6 +25,7 @@ struct AttnParams {
     int32_t batch, total_q;
     int32_t Hq, Hkv, G, W, P;
     int32_t tpt;                   // query tokens per 128-row q tile = 128 / G
+    uint32_t tpt2_magic;           // floor(2^32 / (2 tpt)) + 1: x / (2 tpt) = umulhi(x, magic) for x < 2^24
     float scale;                   // natural-base logit scale
     float scale_log2;              // scale * log2(e)
     // split-KV workspace (library owned)

@@ -65,40 +65,36 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
 }
 // Bounded wait: a protocol bug must end the kernel with a flag, never hang the GPU.
 // `abort_flag` is a CTA-shared word; once set every later wait returns at once.
-#ifndef SANGAM_WAIT_TIMEOUT_NS
-#define SANGAM_WAIT_TIMEOUT_NS 2000000000ull
+#ifndef SANGAM_WAIT_MAX_SPINS
+#define SANGAM_WAIT_MAX_SPINS (1u << 17)
 #endif
 // Diagnostic of the first watchdog timeout (builds with -DSANGAM_WAIT_TABLE): [0] = barrier | 1<<31, [1] warp, [2] CTA,
 // [3] parity, [4..19] the barrier every warp of that CTA was blocked on.
 __device__ unsigned int g_timeout_info[20];
 
-// hot path: one try_wait; then suspending waits (the hardware resumes the thread when the phase completes) with a
-// watchdog every 16 expired 20-us suspensions.  The slow path is inlined at ~60 wait sites, so it is kept minimal (the
-// kernel's instruction footprint is a first-order performance factor; an out-of-line version costs spills around the
-// call in the hot loops); the diagnostics are compiled in only with -DSANGAM_WAIT_TABLE.
+// hot path: one try_wait; then suspending waits (the hardware resumes the thread when the phase completes or after
+// the 20-us hint).  The slow path is inlined at ~60 wait sites, so it is kept minimal -- the kernel's instruction
+// footprint is a first-order performance factor, and an out-of-line version costs spills around the call in the hot
+// loops.  Watchdog = a count of expired suspensions: 2^17 of them are at least a second of a barrier that makes no
+// progress (a legitimate wait sees a handful of wake-ups).  Diagnostics only with -DSANGAM_WAIT_TABLE.
 __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatile uint32_t* abort_flag) {
     if (mbar_try_wait(bar, parity)) return true;
 #ifdef SANGAM_WAIT_TABLE
     if ((threadIdx.x & 31) == 0) abort_flag[3 + (threadIdx.x >> 5)] = bar | (parity << 31);
 #endif
-    uint64_t t0 = 0;
     uint32_t spins = 0;
     bool ok = true;
     while (!mbar_try_wait_hint(bar, parity, 20000u)) {
-        if ((++spins & 0xFu) == 0) {
-            const uint64_t now = globaltimer_ns();
-            if (t0 == 0) t0 = now;
-            if (*abort_flag || now - t0 > SANGAM_WAIT_TIMEOUT_NS) {
+        if ((++spins & 0xFu) == 0 && (*abort_flag || spins > SANGAM_WAIT_MAX_SPINS)) {
 #ifdef SANGAM_WAIT_TABLE
-                if (!*abort_flag && atomicCAS(&g_timeout_info[0], 0u, bar | 0x80000000u) == 0u) {
-                    g_timeout_info[1] = threadIdx.x >> 5; g_timeout_info[2] = blockIdx.x; g_timeout_info[3] = parity;
-                    for (int k = 0; k < 16; ++k) g_timeout_info[4 + k] = abort_flag[3 + k];
-                }
-#endif
-                *abort_flag = 1u;
-                ok = false;
-                break;
+            if (!*abort_flag && atomicCAS(&g_timeout_info[0], 0u, bar | 0x80000000u) == 0u) {
+                g_timeout_info[1] = threadIdx.x >> 5; g_timeout_info[2] = blockIdx.x; g_timeout_info[3] = parity;
+                for (int k = 0; k < 16; ++k) g_timeout_info[4 + k] = abort_flag[3 + k];
             }
+#endif
+            *abort_flag = 1u;
+            ok = false;
+            break;
         }
     }
 #ifdef SANGAM_WAIT_TABLE

@@ -167,6 +167,7 @@ static AttnParams make_params(sangam_ctx* ctx, const void* q, const void* k_page
     p.Hq = ctx->cfg.num_q_heads; p.Hkv = ctx->cfg.num_kv_heads; p.G = ctx->G;
     p.W = ctx->cfg.max_pages_per_req; p.P = ctx->cfg.num_pages;
     p.tpt = 128 / ctx->G;
+    p.tpt2_magic = (uint32_t)(0x100000000ull / (uint64_t)(2 * p.tpt)) + 1u;
     p.scale = scale;
     p.scale_log2 = scale * 1.4426950408889634f;
     p.part_o = ctx->d_part_o; p.part_ml = ctx->d_part_ml; p.num_slots = ctx->num_slots; p.slot_meta = ctx->d_slot_meta;
