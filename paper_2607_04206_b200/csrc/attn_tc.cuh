@@ -1016,7 +1016,7 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
 // A column group's consecutive rows are contiguous in a slot, so every load coalesces.
 // ------------------------------------------------------------------------------------------------
 template <int D>
-__global__ void __launch_bounds__(PAIR)
+__global__ void __launch_bounds__(2 * PAIR)
 combine_kernel(const AttnParams p) {
     const int b = blockIdx.x;
     const SlotMeta h = reinterpret_cast<const SlotMeta*>(p.slot_meta)[b];
@@ -1025,23 +1025,24 @@ combine_kernel(const AttnParams p) {
     if (np < 1 || 2 * (b + np - 1) >= p.num_slots || (unsigned)h.g >= (unsigned)p.Hkv) { raise_flag(p.flags, DEV_INTERNAL | 0x100u); return; }
     const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
     if (R > 64) {
-        // many rows (GQA decode): one thread per row, 32 independent 16-byte loads per piece in flight
-        const int s = threadIdx.x >> 7, row = threadIdx.x & 127, rr = threadIdx.x;
+        // many rows (GQA decode): one thread per (row, half of the columns), D/8 independent 16-byte loads per piece in flight
+        const int half = threadIdx.x >> 8, rr = threadIdx.x & (PAIR - 1), s = rr >> 7, row = rr & 127;
         if (row >= (s ? h.rows1 : h.rows0)) return;
+        constexpr int HC = D / 2;                            // columns per thread
         float ms = -INFINITY;
         for (int pi = 0; pi < np; ++pi) ms = fmaxf(ms, ml[(int64_t)(pi == 0 ? 2 * b + 1 : 2 * (b + pi)) * PAIR + rr].x);
-        float acc[D];
+        float acc[HC];
 #pragma unroll
-        for (int e = 0; e < D; ++e) acc[e] = 0.f;
+        for (int e = 0; e < HC; ++e) acc[e] = 0.f;
         float ls = 0.f;
         for (int pi = 0; pi < np; ++pi) {
             const int64_t slot = pi == 0 ? 2 * b + 1 : 2 * (b + pi);
             const float2 x = ml[slot * PAIR + rr];
             const float w = ptx::ex2(x.x - ms);
             ls = fmaf(x.y, w, ls);
-            const float4* src = reinterpret_cast<const float4*>(p.part_o) + slot * (D / 4) * PAIR + rr;
+            const float4* src = reinterpret_cast<const float4*>(p.part_o) + (slot * (D / 4) + half * (HC / 4)) * PAIR + rr;
 #pragma unroll
-            for (int c4 = 0; c4 < D / 4; ++c4) {
+            for (int c4 = 0; c4 < HC / 4; ++c4) {
                 const float4 o = __ldcs(src + c4 * PAIR);
                 acc[c4 * 4 + 0] = fmaf(o.x, w, acc[c4 * 4 + 0]); acc[c4 * 4 + 1] = fmaf(o.y, w, acc[c4 * 4 + 1]);
                 acc[c4 * 4 + 2] = fmaf(o.z, w, acc[c4 * 4 + 2]); acc[c4 * 4 + 3] = fmaf(o.w, w, acc[c4 * 4 + 3]);
@@ -1051,9 +1052,9 @@ combine_kernel(const AttnParams p) {
         const int tl = row / p.G, hh = row - tl * p.G;
         const int tok = h.q_start + h.tok0 + s * p.tpt + tl;
         if ((unsigned)tok >= (unsigned)p.total_q) { raise_flag(p.flags, DEV_INTERNAL | 0x200u); return; }
-        uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + h.g * p.G + hh) * D);
+        uint4* dst = reinterpret_cast<uint4*>(p.out + ((int64_t)tok * p.Hq + h.g * p.G + hh) * D + half * HC);
 #pragma unroll
-        for (int c8 = 0; c8 < D / 8; ++c8) {
+        for (int c8 = 0; c8 < HC / 8; ++c8) {
             uint4 w4;
             w4.x = ptx::pack_bf16(acc[c8 * 8 + 0] * inv, acc[c8 * 8 + 1] * inv);
             w4.y = ptx::pack_bf16(acc[c8 * 8 + 2] * inv, acc[c8 * 8 + 3] * inv);
@@ -1065,7 +1066,7 @@ combine_kernel(const AttnParams p) {
     }
     // few rows (MHA decode): work item = (8-column group cg, row), consecutive threads take consecutive rows of one
     // column group, so a 32-row unit still spreads over all 256 threads
-    for (int item = threadIdx.x; item < R * (D / 8); item += PAIR) {
+    for (int item = threadIdx.x; item < R * (D / 8); item += 2 * PAIR) {
         const int cg = item / R, ri = item - cg * R;
         const int s = ri >= h.rows0, row = ri - (s ? h.rows0 : 0), rr = s * BM + row;      // rr = row inside the slot
         float ms = -INFINITY;
@@ -1159,10 +1160,10 @@ static inline cudaError_t tc_launch(const AttnParams& p, const TcMaps& maps, int
                                     cudaStream_t stream, int* launched) {
     if (head_dim == 128) {
         tc::attn_kernel<128><<<sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
-        tc::combine_kernel<128><<<sm_count, tc::PAIR, 0, stream>>>(p);
+        tc::combine_kernel<128><<<sm_count, 2 * tc::PAIR, 0, stream>>>(p);
     } else {
         tc::attn_kernel<64><<<sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
-        tc::combine_kernel<64><<<sm_count, tc::PAIR, 0, stream>>>(p);
+        tc::combine_kernel<64><<<sm_count, 2 * tc::PAIR, 0, stream>>>(p);
     }
     *launched = 2;
     return cudaGetLastError();

@@ -21,24 +21,33 @@ kv_write_kernel(const uint4* __restrict__ k, const uint4* __restrict__ v,
     for (; idx < total; idx += stride * UNROLL) {
         uint4 kk[UNROLL], vv[UNROLL];
         int64_t dst[UNROLL];
+        // the row data and the slot ids are fetched together (the data address does not depend on the slot): one
+        // memory latency per pass instead of two.  Rows that turn out to be skipped (slot < 0) were read for nothing.
+        int32_t sl[UNROLL];
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u) {
+            const int64_t e = idx + u * stride;
+            sl[u] = -1;
+            if (e < total) {
+                sl[u] = __ldg(slot_mapping + (int32_t)(e / chunks_per_token));
+                kk[u] = __ldcs(k + e);   // streamed once
+                vv[u] = __ldcs(v + e);
+            }
+        }
 #pragma unroll
         for (int u = 0; u < UNROLL; ++u) {
             const int64_t e = idx + u * stride;
             dst[u] = -1;
-            if (e < total) {
-                const int32_t i = (int32_t)(e / chunks_per_token);
-                const int32_t rem = (int32_t)(e - (int64_t)i * chunks_per_token);
-                const int32_t s = __ldg(slot_mapping + i);
-                if (s >= 0) {
-                    if (s < num_slots_total) {
-                        const int32_t h = rem / chunks_per_row, c = rem - h * chunks_per_row;
-                        const int32_t page = s >> 4, off = s & 15;
-                        dst[u] = (((int64_t)page * Hkv + h) * SANGAM_PAGE + off) * chunks_per_row + c;
-                        kk[u] = __ldcs(k + e);   // streamed once
-                        vv[u] = __ldcs(v + e);
-                    } else {
-                        raise_flag(flags, DEV_BAD_SLOT);
-                    }
+            const int32_t s = sl[u];
+            if (e < total && s >= 0) {
+                if (s < num_slots_total) {
+                    const int32_t i = (int32_t)(e / chunks_per_token);
+                    const int32_t rem = (int32_t)(e - (int64_t)i * chunks_per_token);
+                    const int32_t h = rem / chunks_per_row, c = rem - h * chunks_per_row;
+                    const int32_t page = s >> 4, off = s & 15;
+                    dst[u] = (((int64_t)page * Hkv + h) * SANGAM_PAGE + off) * chunks_per_row + c;
+                } else {
+                    raise_flag(flags, DEV_BAD_SLOT);
                 }
             }
         }
