@@ -476,9 +476,10 @@ struct MmaState {
     // the skipped use may still be in flight when the next-but-one is awaited).  So the producer publishes the
     // position it is loading into each stage (kv_seq) and the issuer first waits for ITS position to be the one
     // in flight; from then on the barrier's current phase is exactly that load's.
-    __device__ __forceinline__ uint32_t acquire() {
+    // (SHARED mode: both issuers consume every use of every stage, so the check is skipped there)
+    __device__ __forceinline__ uint32_t acquire(bool check = true) {
         const uint32_t s0 = stage;
-        if (kv_seq[s0] != pos) {                       // the issuer is ahead of the producer
+        if (check && kv_seq[s0] != pos) {              // the issuer is ahead of the producer
             uint32_t spins = 0;
             while (kv_seq[s0] != pos)
                 if ((++spins & 0x3ffu) == 0 && *abort_flag) break;
@@ -628,7 +629,7 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
                             continue;
                         }
                         if (has_v) {
-                            sv = st.acquire();
+                            sv = st.acquire(!shared);
                             tile = shared ? kv0 + i : kv0 + 2 * i + x;
                             const int nv = c - tile * BN;
                             if (nv < BN && (nv & 15)) {          // tail tile: stale rows of the last page
@@ -641,7 +642,7 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
                             }
                         }
                         if (has_k) {
-                            sk = st.acquire();
+                            sk = st.acquire(!shared);
                             next = shared ? kv0 + i + 1 : kv0 + 2 * (i + 1) + x;
                         }
                         work = has_v || has_k;
