@@ -176,3 +176,36 @@ def test_graph_replay_with_changed_lengths(oracle):
         graph.replay(); torch.cuda.synchronize()
         assert np.array_equal(first, bits_of(out[:b.total_q]))
     assert eng.device_status() == 0
+
+
+@pytest.mark.parametrize("scale", [-0.0883883461356163, 0.0, 0.35])
+def test_scale_sign_and_magnitude(oracle, scale):
+    """The logit scale is a caller-supplied float (reading S5): negative (the kernel flips the sign of S and works
+    with |scale|), zero (uniform weights: out = mean of V, oracle pin 7) and large (exercises the lazy rescale:
+    logits of up to +-40 in log2 units move the reference maximum many times)."""
+    b = si.custom(47, [40, 150, 7], [300, 420, 129], num_q_heads=8, num_kv_heads=2, head_dim=128)
+    b.scale = np.float32(scale)
+    ref, kp, vp = oracle.iteration(b)
+    db = DeviceBatch(b)
+    out = db.iteration()
+    mx, mean = compare(out, ref)
+    print(f"scale {scale}: max-abs {mx:.3e} mean-abs {mean:.3e}")
+    assert mx <= MAX_ABS and mean <= MEAN_ABS
+    assert db.eng.device_status() == 0
+
+
+def test_more_than_32_requests(oracle):
+    """The planner keeps the first 32 requests' metadata in registers and reads the rest from global memory."""
+    rng = np.random.default_rng(5)
+    R = 45
+    q_lens = rng.integers(0, 40, R).tolist()
+    ctx = rng.integers(1, 300, R).tolist()
+    b = si.custom(48, q_lens, ctx, num_q_heads=4, num_kv_heads=4, head_dim=64)
+    ref, kp, vp = oracle.iteration(b)
+    db = DeviceBatch(b)
+    out = db.iteration()
+    assert np.array_equal(bits_of(db.k_pages), kp) and np.array_equal(bits_of(db.v_pages), vp)
+    mx, mean = compare(out, ref)
+    print(f"45 requests: max-abs {mx:.3e} mean-abs {mean:.3e}")
+    assert mx <= MAX_ABS and mean <= MEAN_ABS
+    assert db.eng.device_status() == 0
