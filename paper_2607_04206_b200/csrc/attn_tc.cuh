@@ -985,6 +985,11 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
         ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
         ptx::tmem_relinquish();
     }
+    // Everything above touches only this CTA's shared memory, TMEM and the kernel parameters: under a programmatic
+    // dependent launch it overlaps the tail of the previous kernel in the stream.  Global memory is read or written
+    // only after pdl_wait; the combine kernel behind this one may be scheduled onto SMs as they drain.
+    ptx::pdl_wait();
+    ptx::pdl_trigger();
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
@@ -1019,6 +1024,8 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
 template <int D>
 __global__ void __launch_bounds__(2 * PAIR)
 combine_kernel(const AttnParams p) {
+    ptx::pdl_wait();       // before any global read, in every block: this grid's completion then implies attn_kernel's
+    ptx::pdl_trigger();
     const int b = blockIdx.x;
     const SlotMeta h = reinterpret_cast<const SlotMeta*>(p.slot_meta)[b];
     if (!h.valid) return;
@@ -1157,15 +1164,36 @@ static inline int tc_encode_q(TcMaps* maps, const void* q, int total_q, int Hq, 
     return r == CUDA_SUCCESS ? 0 : -1;
 }
 
+// Both kernels are launched with programmatic stream serialization (they call griddepcontrol.wait before touching
+// global memory), also under stream capture: the graph keeps the programmatic edges.
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t stream,
+                                     Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
 static inline cudaError_t tc_launch(const AttnParams& p, const TcMaps& maps, int head_dim, int sm_count,
                                     cudaStream_t stream, int* launched) {
+    cudaError_t e;
+    *launched = 0;
     if (head_dim == 128) {
-        tc::attn_kernel<128><<<sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
-        tc::combine_kernel<128><<<sm_count, 2 * tc::PAIR, 0, stream>>>(p);
+        e = launch_pdl(tc::attn_kernel<128>, sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream, maps.k, maps.v, maps.q, p);
+        if (e != cudaSuccess) return e;
+        *launched = 1;
+        e = launch_pdl(tc::combine_kernel<128>, sm_count, 2 * tc::PAIR, 0, stream, p);
     } else {
-        tc::attn_kernel<64><<<sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream>>>(maps.k, maps.v, maps.q, p);
-        tc::combine_kernel<64><<<sm_count, 2 * tc::PAIR, 0, stream>>>(p);
+        e = launch_pdl(tc::attn_kernel<64>, sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream, maps.k, maps.v, maps.q, p);
+        if (e != cudaSuccess) return e;
+        *launched = 1;
+        e = launch_pdl(tc::combine_kernel<64>, sm_count, 2 * tc::PAIR, 0, stream, p);
     }
+    if (e != cudaSuccess) return e;
     *launched = 2;
     return cudaGetLastError();
 }

@@ -14,6 +14,10 @@ kv_write_kernel(const uint4* __restrict__ k, const uint4* __restrict__ v,
                 uint4* __restrict__ k_pages, uint4* __restrict__ v_pages,
                 int32_t Hkv, int32_t chunks_per_row /* D/8 */, int32_t num_slots_total,
                 uint32_t* flags) {
+    // programmatic dependent launch: wait for the previous kernel in the stream (it may still read the pages), then let
+    // the attention kernel behind this one run its shared-memory / TMEM prologue while the rows are copied
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const int64_t chunks_per_token = (int64_t)Hkv * chunks_per_row;
     const int64_t total = (int64_t)num_tokens * chunks_per_token;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;

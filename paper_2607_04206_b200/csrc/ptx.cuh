@@ -103,6 +103,11 @@ __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatil
     return ok;
 }
 
+// Programmatic dependent launch: `pdl_wait` returns once every grid this one depends on has completed and its
+// memory is visible (a no-op for a launch without the attribute); `pdl_trigger` lets the next grid in the
+// stream start its own prologue as soon as every CTA of this grid has called it or exited.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
