@@ -42,7 +42,11 @@ constexpr int BN = 128;          // kv positions per tile (8 pages)
 constexpr int PAIR = 2 * BM;     // packed rows per work unit
 constexpr int NSTAGE = 5;        // K/V tile ring depth
 constexpr int NTHREADS = 384;
-constexpr int SLAB = 128 * 128;  // bytes of one 64-wide swizzled slab of a 128-row tile
+constexpr int SLAB = 128 * 128;  // bytes of one 64-wide swizzled slab of a 128-row q tile
+// K/V stages are PAGE-major: one TMA box = one whole (page, head) = 16 rows x D, landing as 2 row groups x D/64
+// slabs of 8-row x 128-byte swizzle atoms.  Atom (8-row group j, slab t) of a stage sits at j * KV_ATOM_STRIDE + t * 1024,
+// so the 8-row groups of one slab are KV_ATOM_STRIDE apart (the descriptors' SBO) and the slabs 1024 bytes (V's LBO).
+template <int D> constexpr int KV_ATOM_STRIDE = 1024 * (D / 64);
 #ifndef SANGAM_DYN_UNITS
 #define SANGAM_DYN_UNITS 4
 #endif
@@ -347,8 +351,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
         if (n > 0) {
             const int pages_total = (it.c + SANGAM_PAGE - 1) / SANGAM_PAGE;
             const int32_t* bt = p.block_table + (int64_t)it.r * p.W;
-            constexpr int BOX_PER_PAGE = D / 64;
-            const int pg = lane / BOX_PER_PAGE, slab = lane % BOX_PER_PAGE;
+            const int pg = lane;                         // one box per page: lanes 0..7 issue
             const int lead = it.rows1 > 0 ? 1 : 2;
             auto ld_page = [&](int j) {                  // page pg of the item's j-th tile (0 if it does not exist)
                 const int tile = it.kv0 + j;
@@ -376,9 +379,8 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                 __syncwarp();
                 if (pg < np) {
                     if ((unsigned)page >= (unsigned)p.P) raise_flag(p.flags, DEV_BAD_PAGE);   // TMA zero-fills out of range
-                    ptx::tma_load_2d(sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES + slab * SLAB + pg * 2048),
-                                     is_v ? mapV : mapK, bar(L::B_KV_FULL + stage), slab * 64,
-                                     (page * p.Hkv + it.g) * SANGAM_PAGE);
+                    ptx::tma_load_4d(sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES + pg * (2 * KV_ATOM_STRIDE<D>)),
+                                     is_v ? mapV : mapK, bar(L::B_KV_FULL + stage), 0, 0, 0, (page * p.Hkv + it.g) * 2);
                 }
                 TRACE_EV(54);
                 if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
@@ -501,7 +503,8 @@ __device__ __forceinline__ void zero_v_tail(uint32_t v_addr, int nv, int ncols, 
     const int nrows = ncols - nv;
     for (int e = lane; e < nrows * 8 * (D / 64); e += 32) {
         const int chunk = e & 7, rr = (e >> 3) % nrows, slab = (e >> 3) / nrows;
-        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(v_addr + (uint32_t)(slab * SLAB + (nv + rr) * 128 + chunk * 16)), "r"(0)
+        const int row = nv + rr;
+        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(v_addr + (uint32_t)((row >> 3) * KV_ATOM_STRIDE<D> + slab * 1024 + (row & 7) * 128 + chunk * 16)), "r"(0)
                      : "memory");
     }
     ptx::fence_proxy_async_smem();
@@ -532,26 +535,28 @@ __device__ __forceinline__ void half_step(MmaState<D>& st, int s, int h, int pv_
     if (ptx::elect_one()) {
         const uint32_t sh_tmem = st.tmem + (uint32_t)(s * 128 + h * 64);          // S_s,h / P_s,h
         if (pv_cols > 0) {
-            // K-steps of 16 kv rows = 2048 bytes of V; half h starts 64 rows in
-            const uint64_t b_desc = st.v_desc0 + (uint64_t)(stage_v * (L::KV_BYTES >> 4) + h * 512);
+            // K-steps of 16 kv rows = one page = two 8-row groups of V; half h starts 64 rows (8 groups) in
+            constexpr uint32_t VSTEP = (uint32_t)(2 * KV_ATOM_STRIDE<D>) >> 4;
+            const uint64_t b_desc = st.v_desc0 + (uint64_t)(stage_v * (L::KV_BYTES >> 4) + h * (4 * VSTEP));
             const uint32_t idesc = ptx::idesc_bf16(BM, D, 0, 1);
             const uint32_t d_tmem = st.tmem + 256u + (uint32_t)s * 128u;
             if (pv_cols == 64) {
-                ptx::mma_ts_x4(d_tmem, sh_tmem, b_desc, idesc, first_pv ? 0u : 1u, 128u);
+                ptx::mma_ts_x4(d_tmem, sh_tmem, b_desc, idesc, first_pv ? 0u : 1u, VSTEP);
             } else {
                 for (int ks = 0; ks < pv_cols / 16; ++ks)
-                    ptx::mma_ts(d_tmem, sh_tmem + (uint32_t)(ks * 8), b_desc + (uint64_t)(ks * 128), idesc, (!first_pv || ks > 0) ? 1u : 0u);
+                    ptx::mma_ts(d_tmem, sh_tmem + (uint32_t)(ks * 8), b_desc + (uint64_t)(ks * VSTEP), idesc, (!first_pv || ks > 0) ? 1u : 0u);
             }
             for (int i = 0; i < rel_v; ++i) ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_v));
             ptx::mma_commit(st.bar(L::B_PV_DONE + 2 * s + h));
         }
         if (qk_cols > 0) {
-            // K-steps of 16 elements = 32 bytes inside a 64-wide slab, second slab SLAB bytes further; half h of K = rows 64 h ..
+            // K-steps of 16 elements = 32 bytes inside a 64-wide slab; second slab SLAB bytes further in the q tile and
+            // 1024 bytes further in the page-major K stage; half h of K = rows 64 h .. = 8 row groups in
             const uint64_t a_desc = st.q_desc0 + (uint64_t)(qs * (L::Q_BYTES >> 4));
-            const uint64_t b_desc = st.k_desc0 + (uint64_t)(stage_k * (L::KV_BYTES >> 4) + h * 512);
+            const uint64_t b_desc = st.k_desc0 + (uint64_t)(stage_k * (L::KV_BYTES >> 4) + h * ((8 * KV_ATOM_STRIDE<D>) >> 4));
             const uint32_t idesc = ptx::idesc_bf16(BM, (uint32_t)qk_cols, 0, 0);
             ptx::mma_ss_x4(sh_tmem, a_desc, b_desc, idesc, 0u, 2u);
-            if (D == 128) ptx::mma_ss_x4(sh_tmem, a_desc + (SLAB >> 4), b_desc + (SLAB >> 4), idesc, 1u, 2u);
+            if (D == 128) ptx::mma_ss_x4(sh_tmem, a_desc + (SLAB >> 4), b_desc + (1024 >> 4), idesc, 1u, 2u);
             for (int i = 0; i < rel_k; ++i) ptx::mma_commit(st.bar(L::B_KV_EMPTY + stage_k));
             ptx::mma_commit(st.bar(L::B_S_FULL + 2 * s + h));
             for (int i = 0; i < q_rel; ++i) ptx::mma_commit(st.bar(L::B_Q_EMPTY + qs));
@@ -581,8 +586,8 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
     MmaState<D> st;
     st.sbase = sbase; st.tmem = tmem; st.abort_flag = abort_flag;
     st.q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);        // K-major operands (Q, K)
-    st.k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, 1024);
-    st.v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, SLAB, 1024);     // MN-major operand (V)
+    st.k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, KV_ATOM_STRIDE<D>);
+    st.v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 1024, KV_ATOM_STRIDE<D>);     // MN-major operand (V)
     st.stage = 0; st.phase = 0; st.pos = 0; st.kv_seq = reinterpret_cast<volatile uint32_t*>(kv_seq_smem);
     st.p_par0 = 0; st.p_par1 = 0; st.zf_par = 0;
     uint32_t icount = 0, qcount = 0;
@@ -1122,8 +1127,9 @@ typedef CUresult (*sangam_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32
                                      const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// Pool viewed as a 2-D tensor [P*Hkv*16 rows][D] bf16; one box = 16 rows (a page of one head) x 64 columns,
-// 128-byte swizzled: exactly one UMMA swizzle slab of a page.
+// Pool viewed as a 4-D tensor (64 columns, 8 rows of a row group, D/64 slabs, P*Hkv*2 row groups) of bf16; one box =
+// (64, 8, D/64, 2) = a whole page of one head (16 rows x D), 128-byte swizzled: it lands as 2 x D/64 UMMA swizzle atoms.
+// One TMA instruction per page instead of one per (page, slab): the gather is bound by TMA instructions, not bytes.
 static inline int tc_encode_maps(TcMaps* maps, const void* k_pages, const void* v_pages, int num_pages, int Hkv, int D) {
     static sangam_encode_fn enc = nullptr;
     if (!enc) {
@@ -1132,13 +1138,13 @@ static inline int tc_encode_maps(TcMaps* maps, const void* k_pages, const void* 
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return -1;
         enc = reinterpret_cast<sangam_encode_fn>(fn);
     }
-    const cuuint64_t gdim[2] = {(cuuint64_t)D, (cuuint64_t)num_pages * Hkv * SANGAM_PAGE};
-    const cuuint64_t gstr[1] = {(cuuint64_t)D * 2};
-    const cuuint32_t box[2] = {64, SANGAM_PAGE}, estr[2] = {1, 1};
+    const cuuint64_t gdim[4] = {64, 8, (cuuint64_t)(D / 64), (cuuint64_t)num_pages * Hkv * (SANGAM_PAGE / 8)};
+    const cuuint64_t gstr[3] = {(cuuint64_t)D * 2, 128, (cuuint64_t)D * 2 * 8};
+    const cuuint32_t box[4] = {64, 8, (cuuint32_t)(D / 64), SANGAM_PAGE / 8}, estr[4] = {1, 1, 1, 1};
     const void* ptrs[2] = {k_pages, v_pages};
     CUtensorMap* out[2] = {&maps->k, &maps->v};
     for (int i = 0; i < 2; ++i) {
-        CUresult r = enc(out[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptrs[i]), gdim, gstr, box, estr,
+        CUresult r = enc(out[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(ptrs[i]), gdim, gstr, box, estr,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return -1;
