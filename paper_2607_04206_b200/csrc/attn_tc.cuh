@@ -346,7 +346,7 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
         if (!it.valid) break;
 
         // K/V tile loads in ring order (see above).  The block-table entries of a tile serve its K and its V load
-        // and are fetched three tiles ahead: lane (2 pg + slab) keeps page pg of tiles j, j+1, j+2 in w0, w1, w2.
+        // and are fetched ahead: lane pg (< 8) keeps page pg of the tiles in flight in the window w0 .. w3.
         const int n = it.kv1 - it.kv0;
         if (n > 0) {
             const int pages_total = (it.c + SANGAM_PAGE - 1) / SANGAM_PAGE;
@@ -1026,7 +1026,9 @@ attn_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CU
 //   m* = max m_i;  l* = sum l_i 2^(m_i-m*);  O* = sum O_i 2^(m_i-m*);  out = bf16(O*/l*)
 // A column group's consecutive rows are contiguous in a slot, so every load coalesces.
 // ------------------------------------------------------------------------------------------------
-template <int D>
+// CS = blocks per unit (grid.y): 4 for GQA models (units of up to 256 rows: the 64 units of a Dream-like decode batch
+// keep 256 blocks busy instead of 64), 1 for MHA models (32-row decode units: extra blocks would only add launch cost)
+template <int D, int CS>
 __global__ void __launch_bounds__(2 * PAIR)
 combine_kernel(const AttnParams p) {
     ptx::pdl_wait();       // before any global read, in every block: this grid's completion then implies attn_kernel's
@@ -1038,10 +1040,11 @@ combine_kernel(const AttnParams p) {
     if (np < 1 || 2 * (b + np - 1) >= p.num_slots || (unsigned)h.g >= (unsigned)p.Hkv) { raise_flag(p.flags, DEV_INTERNAL | 0x100u); return; }
     const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
     if (R > 64) {
-        // many rows (GQA decode): one thread per (row, half of the columns), D/8 independent 16-byte loads per piece in flight
-        const int half = threadIdx.x >> 8, rr = threadIdx.x & (PAIR - 1), s = rr >> 7, row = rr & 127;
+        // many rows (GQA decode): one thread per (row, 1/(2 CS) of the columns), D/(8 CS) independent 16-byte loads per
+        // piece in flight; the CS blocks (blockIdx.y) of a unit take interleaved column slices
+        const int half = (threadIdx.x >> 8) * CS + blockIdx.y, rr = threadIdx.x & (PAIR - 1), s = rr >> 7, row = rr & 127;
         if (row >= (s ? h.rows1 : h.rows0)) return;
-        constexpr int HC = D / 2;                            // columns per thread
+        constexpr int HC = D / (2 * CS);                     // columns per thread
         float ms = -INFINITY;
         for (int pi = 0; pi < np; ++pi) ms = fmaxf(ms, ml[(int64_t)(pi == 0 ? 2 * b + 1 : 2 * (b + pi)) * PAIR + rr].x);
         float acc[HC];
@@ -1079,7 +1082,7 @@ combine_kernel(const AttnParams p) {
     }
     // few rows (MHA decode): work item = (8-column group cg, row), consecutive threads take consecutive rows of one
     // column group, so a 32-row unit still spreads over all 256 threads
-    for (int item = threadIdx.x; item < R * (D / 8); item += 2 * PAIR) {
+    for (int item = threadIdx.x + blockIdx.y * 2 * PAIR; item < R * (D / 8); item += 2 * PAIR * CS) {
         const int cg = item / R, ri = item - cg * R;
         const int s = ri >= h.rows0, row = ri - (s ? h.rows0 : 0), rr = s * BM + row;      // rr = row inside the slot
         float ms = -INFINITY;
@@ -1173,10 +1176,10 @@ static inline int tc_encode_q(TcMaps* maps, const void* q, int total_q, int Hq, 
 // Both kernels are launched with programmatic stream serialization (they call griddepcontrol.wait before touching
 // global memory), also under stream capture: the graph keeps the programmatic edges.
 template <typename... KArgs, typename... Args>
-static inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t stream,
+static inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, unsigned block, size_t smem, cudaStream_t stream,
                                      Args... args) {
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cfg.gridDim = grid; cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
@@ -1189,15 +1192,17 @@ static inline cudaError_t tc_launch(const AttnParams& p, const TcMaps& maps, int
     cudaError_t e;
     *launched = 0;
     if (head_dim == 128) {
-        e = launch_pdl(tc::attn_kernel<128>, sm_count, tc::NTHREADS, tc::Smem<128>::ALLOC, stream, maps.k, maps.v, maps.q, p);
+        e = launch_pdl(tc::attn_kernel<128>, dim3(sm_count), tc::NTHREADS, tc::Smem<128>::ALLOC, stream, maps.k, maps.v, maps.q, p);
         if (e != cudaSuccess) return e;
         *launched = 1;
-        e = launch_pdl(tc::combine_kernel<128>, sm_count, 2 * tc::PAIR, 0, stream, p);
+        e = p.G > 1 ? launch_pdl(tc::combine_kernel<128, 4>, dim3(sm_count, 4), 2 * tc::PAIR, 0, stream, p)
+                    : launch_pdl(tc::combine_kernel<128, 1>, dim3(sm_count, 1), 2 * tc::PAIR, 0, stream, p);
     } else {
-        e = launch_pdl(tc::attn_kernel<64>, sm_count, tc::NTHREADS, tc::Smem<64>::ALLOC, stream, maps.k, maps.v, maps.q, p);
+        e = launch_pdl(tc::attn_kernel<64>, dim3(sm_count), tc::NTHREADS, tc::Smem<64>::ALLOC, stream, maps.k, maps.v, maps.q, p);
         if (e != cudaSuccess) return e;
         *launched = 1;
-        e = launch_pdl(tc::combine_kernel<64>, sm_count, 2 * tc::PAIR, 0, stream, p);
+        e = p.G > 1 ? launch_pdl(tc::combine_kernel<64, 4>, dim3(sm_count, 4), 2 * tc::PAIR, 0, stream, p)
+                    : launch_pdl(tc::combine_kernel<64, 1>, dim3(sm_count, 1), 2 * tc::PAIR, 0, stream, p);
     }
     if (e != cudaSuccess) return e;
     *launched = 2;

@@ -131,7 +131,7 @@ extern "C" int sangam_kv_write(sangam_ctx* ctx, const void* k, const void* v, co
     int64_t blocks = (total + 256 * UNROLL - 1) / (256 * UNROLL);
     const int64_t cap = (int64_t)ctx->sm_count * 16;
     if (blocks > cap) blocks = cap;
-    CK(launch_pdl(kv_write_kernel<UNROLL>, (unsigned)blocks, 256u, 0, (cudaStream_t)stream,
+    CK(launch_pdl(kv_write_kernel<UNROLL>, dim3((unsigned)blocks), 256u, 0, (cudaStream_t)stream,
                   (const uint4*)k, (const uint4*)v, slot_mapping, num_tokens, (uint4*)k_pages, (uint4*)v_pages,
                   (int32_t)ctx->cfg.num_kv_heads, (int32_t)cpr, (int32_t)(ctx->cfg.num_pages * SANGAM_PAGE), ctx->d_flags));
     ctx->launches += 1;
