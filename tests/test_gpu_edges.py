@@ -209,3 +209,24 @@ def test_more_than_32_requests(oracle):
     print(f"45 requests: max-abs {mx:.3e} mean-abs {mean:.3e}")
     assert mx <= MAX_ABS and mean <= MEAN_ABS
     assert db.eng.device_status() == 0
+
+
+@pytest.mark.parametrize("hq,hkv,d", [(8, 2, 64), (14, 2, 128), (4, 4, 128)])
+def test_decode_units_split_into_many_pieces(oracle, hq, hkv, d):
+    """Few (request, kv head) units with long contexts: the stream-K cut gives every CTA about one kv tile, so a unit is
+    merged from tens of partial pieces by combine_kernel (both its row paths, every column slice of the GQA grid)."""
+    b = si.custom(49, [32, 32, 5], [3000, 5003, 2049], num_q_heads=hq, num_kv_heads=hkv, head_dim=d)
+    ref, kp, vp = oracle.iteration(b)
+    db = DeviceBatch(b)
+    out = db.iteration()
+    assert np.array_equal(bits_of(db.k_pages), kp) and np.array_equal(bits_of(db.v_pages), vp)
+    mx, mean = compare(out, ref)
+    print(f"many pieces Hq={hq} Hkv={hkv} D={d}: max-abs {mx:.3e} mean-abs {mean:.3e}")
+    assert mx <= MAX_ABS and mean <= MEAN_ABS
+    first = bits_of(out).copy()
+    db.out.fill_(float("nan"))
+    db.attend()
+    import torch
+    torch.cuda.synchronize()
+    assert np.array_equal(bits_of(db.out), first), "split-KV merge is not bitwise reproducible"
+    assert db.eng.device_status() == 0
