@@ -77,7 +77,8 @@ __device__ __forceinline__ void trace_ns(unsigned ev) {
 }
 #define TRACE_EV(ev) trace_ev(ev)
 #define TRACE_NS(ev) trace_ns(ev)
-#define TRACE_CTA(which) do { if (threadIdx.x == 0 && blockIdx.x < 256) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_cta_times[2 * blockIdx.x + (which)] = t_; } } while (0)
+// bits 63..54 of the entry stamp carry %smid (the timer's high bits are constant over a launch: the host masks them off)
+#define TRACE_CTA(which) do { if (threadIdx.x == 0 && blockIdx.x < 256) { unsigned long long t_; unsigned sm_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm_)); g_cta_times[2 * blockIdx.x + (which)] = (which) ? t_ : ((t_ & 0x003fffffffffffffull) | ((unsigned long long)sm_ << 54)); } } while (0)
 #define TRACE_INIT() do { if (threadIdx.x < 16) trace_cnt()[threadIdx.x] = 0; if (threadIdx.x == 16) trace_cnt()[16] = blockIdx.x == g_trace_cta; __syncthreads(); } while (0)
 #else
 #define TRACE_EV(ev) ((void)0)
