@@ -35,7 +35,9 @@ struct AttnParams {
     void* slot_meta;               // [num_ctas] tc::SlotMeta, rewritten by every launch
     uint32_t* flags;               // sticky device flags
     int32_t* sched;                // [0] dynamic work counter (self-resetting), [1] finished-CTA count
+    int32_t* plan_cache;           // [num_ctas][PLAN_CACHE_INTS]: each CTA's last plan, keyed by the batch's lengths
 };
+constexpr int PLAN_CACHE_INTS = 32 * 3 + 16;   // (q0, qn, c) of up to 32 requests + header
 
 __device__ __forceinline__ void raise_flag(uint32_t* flags, uint32_t f) {
     if (flags) atomicOr(flags, f);

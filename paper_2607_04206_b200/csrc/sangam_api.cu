@@ -23,6 +23,7 @@ struct sangam_ctx {
     float* d_part_o;
     float* d_part_ml;
     void* d_slot_meta;
+    int32_t* d_plan_cache;
     int32_t num_slots;
     // tensor maps for the K / V pools, re-encoded when the pool pointer changes
     TcMaps maps;
@@ -85,6 +86,9 @@ extern "C" int sangam_create(const sangam_config* cfg, sangam_ctx** out) {
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_part_ml, (size_t)ctx->num_slots * 256 * 2 * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_slot_meta, (size_t)ctx->num_slots * 32);
     if (e == cudaSuccess) e = cudaMemset(ctx->d_slot_meta, 0, (size_t)ctx->num_slots * 32);
+    const size_t plan_bytes = (size_t)(ctx->sm_count > 0 ? ctx->sm_count : 148) * PLAN_CACHE_INTS * sizeof(int32_t);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_plan_cache, plan_bytes);
+    if (e == cudaSuccess) e = cudaMemset(ctx->d_plan_cache, 0, plan_bytes);
     if (e == cudaSuccess) e = tc_configure(cfg->head_dim);
     if (e != cudaSuccess) {
         sangam_destroy(ctx);
@@ -96,7 +100,7 @@ extern "C" int sangam_create(const sangam_config* cfg, sangam_ctx** out) {
 
 extern "C" int sangam_destroy(sangam_ctx* ctx) {
     if (!ctx) return SANGAM_ERR_INVALID_ARG;
-    cudaFree(ctx->d_flags); cudaFree(ctx->d_sched); cudaFree(ctx->d_part_o); cudaFree(ctx->d_part_ml); cudaFree(ctx->d_slot_meta);
+    cudaFree(ctx->d_flags); cudaFree(ctx->d_sched); cudaFree(ctx->d_part_o); cudaFree(ctx->d_part_ml); cudaFree(ctx->d_slot_meta); cudaFree(ctx->d_plan_cache);
     cudaFree(ctx->s_q); cudaFree(ctx->s_k); cudaFree(ctx->s_v); cudaFree(ctx->s_out);
     cudaFree(ctx->s_slot); cudaFree(ctx->s_bt); cudaFree(ctx->s_cu); cudaFree(ctx->s_ctx);
     delete ctx;
@@ -171,7 +175,7 @@ static AttnParams make_params(sangam_ctx* ctx, const void* q, const void* k_page
     p.scale = scale;
     p.scale_log2 = scale * 1.4426950408889634f;
     p.part_o = ctx->d_part_o; p.part_ml = ctx->d_part_ml; p.num_slots = ctx->num_slots; p.slot_meta = ctx->d_slot_meta;
-    p.flags = ctx->d_flags; p.sched = ctx->d_sched;
+    p.flags = ctx->d_flags; p.sched = ctx->d_sched; p.plan_cache = ctx->d_plan_cache;
     return p;
 }
 
