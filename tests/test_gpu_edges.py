@@ -152,7 +152,11 @@ def test_graph_replay_with_changed_lengths(oracle):
         return b, ref, kpf
 
     cases = [(51, [32] * 6, [600, 300, 129, 640, 77, 500]), (52, [64, 0, 32, 5], [200, 100, 640, 33]),
-             (53, [10, 20, 30, 40, 50, 60], [16, 32, 48, 64, 80, 96])]
+             (53, [10, 20, 30, 40, 50, 60], [16, 32, 48, 64, 80, 96]),
+             # the per-CTA plan cache is keyed by the lengths: one context longer by one position (a new tile), one
+             # query row fewer, the first batch again (each case runs as a miss, then as a hit, bit-identically)
+             (54, [32] * 6, [600, 300, 129, 640, 77, 513]), (55, [32] * 5 + [31], [600, 300, 129, 640, 77, 513]),
+             (51, [32] * 6, [600, 300, 129, 640, 77, 500])]
     b, ref, _ = fill(*cases[0])
     torch.cuda.synchronize()
     with torch.cuda.stream(stream):
