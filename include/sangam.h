@@ -107,6 +107,18 @@ int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_pages, const
                       int32_t batch, int32_t total_q, float scale, void* out, void* stream);
 
 /*
+ * Kernel choice of sangam_block_attn.  AUTO (default): decode-shaped batches (total_q * G <= 32 * batch, i.e. on
+ * average at most one 32-row unit per request and kv head -- block decodes, block 32) run
+ * the swapped-operand decode kernel, everything else the two-stream prefill / hybrid kernel.  Both kernels compute
+ * the same function for every batch; PREFILL / DECODE force one of them (tests, measurements).  DECODE returns
+ * SANGAM_ERR_UNSUPPORTED for geometries the decode kernel is not built for (num_q_heads / num_kv_heads > 32).
+ */
+#define SANGAM_DISPATCH_AUTO    0
+#define SANGAM_DISPATCH_PREFILL 1
+#define SANGAM_DISPATCH_DECODE  2
+int sangam_set_dispatch(sangam_ctx* ctx, int32_t mode);
+
+/*
  * Same contract as sangam_block_attn, computed by a plain CUDA-core (no tensor core) kernel with
  * fp32 arithmetic.  A cross-check for the tcgen05 path on workloads too large for the CPU oracle;
  * never dispatched by sangam_block_attn.

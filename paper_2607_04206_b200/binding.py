@@ -11,8 +11,10 @@ LIB_PATH = os.path.join(HERE, "libsangam.so")
 DECLARED_SYMBOLS = [
     "sangam_create", "sangam_destroy", "sangam_kv_write", "sangam_block_attn", "sangam_block_attn_simt",
     "sangam_iteration_host", "sangam_device_status", "sangam_clear_device_status", "sangam_launch_count",
-    "sangam_last_error", "sangam_version",
+    "sangam_last_error", "sangam_version", "sangam_set_dispatch",
 ]
+
+DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE = 0, 1, 2
 
 
 class SangamError(RuntimeError):
@@ -54,6 +56,7 @@ def load_library(build_if_missing: bool = False):
     lib.sangam_last_error.argtypes = [vp]
     lib.sangam_last_error.restype = ctypes.c_char_p
     lib.sangam_version.restype = ctypes.c_char_p
+    lib.sangam_set_dispatch.argtypes = [vp, i32]
     _lib = lib
     return lib
 
@@ -120,6 +123,10 @@ class Sangam:
             self.ctx, _ptr(q), _ptr(k), _ptr(v), _ptr(slot_mapping), int(slot_mapping.numel()), _ptr(k_pages),
             _ptr(v_pages), _ptr(block_table), _ptr(cu_q_lens), _ptr(ctx_lens), int(ctx_lens.numel()), int(q.shape[0]),
             float(scale), _ptr(out), _stream(stream)))
+
+    def set_dispatch(self, mode: int):
+        """DISPATCH_AUTO / DISPATCH_PREFILL / DISPATCH_DECODE: which attention kernel sangam_block_attn launches."""
+        self._check(self.lib.sangam_set_dispatch(self.ctx, int(mode)))
 
     def device_status(self) -> int:
         f = ctypes.c_uint32(0)

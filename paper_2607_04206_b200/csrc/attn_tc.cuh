@@ -27,10 +27,6 @@
 #include "common.cuh"
 #include "ptx.cuh"
 
-struct TcMaps {
-    CUtensorMap k, v, q;
-};
-
 #ifdef SANGAM_DEBUG_ITEM
 __device__ int g_bad_item[16];
 #endif
@@ -1166,75 +1162,59 @@ typedef CUresult (*sangam_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32
                                      const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// Pool viewed as a 4-D tensor (64 columns, 8 rows of a row group, D/64 slabs, P*Hkv*2 row groups) of bf16; one box =
-// (64, 8, D/64, 2) = a whole page of one head (16 rows x D), 128-byte swizzled: it lands as 2 x D/64 UMMA swizzle atoms.
-// One TMA instruction per page instead of one per (page, slab): the gather is bound by TMA instructions, not bytes.
-static inline int tc_encode_maps(TcMaps* maps, const void* k_pages, const void* v_pages, int num_pages, int Hkv, int D) {
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no -lcuda); looked up once
+static inline sangam_encode_fn tmap_encode_fn() {
     static sangam_encode_fn enc = nullptr;
     if (!enc) {
         cudaDriverEntryPointQueryResult q;
         void* fn = nullptr;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return -1;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return nullptr;
         enc = reinterpret_cast<sangam_encode_fn>(fn);
     }
+    return enc;
+}
+
+// Pool viewed as a 4-D tensor (64 columns, 8 rows of a row group, D/64 slabs, P*Hkv*2 row groups) of bf16; one box =
+// (64, 8, D/64, 2) = a whole page of one head (16 rows x D), 128-byte swizzled: it lands as 2 x D/64 UMMA swizzle atoms.
+// One TMA instruction per page instead of one per (page, slab): the gather is bound by TMA instructions, not bytes.
+// A box whose last coordinate is >= P*Hkv*2 lies outside the tensor and is filled with zeros (bad page ids).
+static inline int tmap_encode_pool(CUtensorMap* out, const void* pages, int num_pages, int Hkv, int D) {
+    sangam_encode_fn enc = tmap_encode_fn();
+    if (!enc) return -1;
     const cuuint64_t gdim[4] = {64, 8, (cuuint64_t)(D / 64), (cuuint64_t)num_pages * Hkv * (SANGAM_PAGE / 8)};
     const cuuint64_t gstr[3] = {(cuuint64_t)D * 2, 128, (cuuint64_t)D * 2 * 8};
     const cuuint32_t box[4] = {64, 8, (cuuint32_t)(D / 64), SANGAM_PAGE / 8}, estr[4] = {1, 1, 1, 1};
-    const void* ptrs[2] = {k_pages, v_pages};
-    CUtensorMap* out[2] = {&maps->k, &maps->v};
-    for (int i = 0; i < 2; ++i) {
-        CUresult r = enc(out[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(ptrs[i]), gdim, gstr, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) return -1;
-    }
-    return 0;
-}
-
-// q viewed as [total_q][Hq][D] bf16; one box = tpt tokens x G heads x 64 columns, 128-byte swizzled
-static inline int tc_encode_q(TcMaps* maps, const void* q, int total_q, int Hq, int D, int G, int tpt) {
-    sangam_encode_fn enc = nullptr;
-    {
-        cudaDriverEntryPointQueryResult qr;
-        void* fn = nullptr;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn) return -1;
-        enc = reinterpret_cast<sangam_encode_fn>(fn);
-    }
-    const cuuint64_t gdim[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)total_q};
-    const cuuint64_t gstr[2] = {(cuuint64_t)D * 2, (cuuint64_t)Hq * D * 2};
-    const cuuint32_t box[3] = {64, (cuuint32_t)G, (cuuint32_t)tpt}, estr[3] = {1, 1, 1};
-    CUresult r = enc(&maps->q, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), gdim, gstr, box, estr,
+    CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(pages), gdim, gstr, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? 0 : -1;
 }
 
-// Both kernels are launched with programmatic stream serialization (they call griddepcontrol.wait before touching
-// global memory), also under stream capture: the graph keeps the programmatic edges.
-template <typename... KArgs, typename... Args>
-static inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, unsigned block, size_t smem, cudaStream_t stream,
-                                     Args... args) {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = grid; cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kern, args...);
+// q viewed as [total_q][Hq][D] bf16; one box = `tokens` tokens x G heads x 64 columns, 128-byte swizzled
+static inline int tmap_encode_q(CUtensorMap* out, const void* q, int total_q, int Hq, int D, int G, int tokens) {
+    sangam_encode_fn enc = tmap_encode_fn();
+    if (!enc) return -1;
+    const cuuint64_t gdim[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)total_q};
+    const cuuint64_t gstr[2] = {(cuuint64_t)D * 2, (cuuint64_t)Hq * D * 2};
+    const cuuint32_t box[3] = {64, (cuuint32_t)G, (cuuint32_t)tokens}, estr[3] = {1, 1, 1};
+    CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), gdim, gstr, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? 0 : -1;
 }
 
-static inline cudaError_t tc_launch(const AttnParams& p, const TcMaps& maps, int head_dim, int sm_count,
-                                    cudaStream_t stream, int* launched) {
+static inline cudaError_t tc_launch(const AttnParams& p, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mq,
+                                    int head_dim, int sm_count, cudaStream_t stream, int* launched) {
     cudaError_t e;
     *launched = 0;
     if (head_dim == 128) {
-        e = launch_pdl(tc::attn_kernel<128>, dim3(sm_count), tc::NTHREADS, tc::Smem<128>::ALLOC, stream, maps.k, maps.v, maps.q, p);
+        e = launch_pdl(tc::attn_kernel<128>, dim3(sm_count), tc::NTHREADS, tc::Smem<128>::ALLOC, stream, mk, mv, mq, p);
         if (e != cudaSuccess) return e;
         *launched = 1;
         e = p.G > 1 ? launch_pdl(tc::combine_kernel<128, 4>, dim3(sm_count, 4), 2 * tc::PAIR, 0, stream, p)
                     : launch_pdl(tc::combine_kernel<128, 1>, dim3(sm_count, 1), 2 * tc::PAIR, 0, stream, p);
     } else {
-        e = launch_pdl(tc::attn_kernel<64>, dim3(sm_count), tc::NTHREADS, tc::Smem<64>::ALLOC, stream, maps.k, maps.v, maps.q, p);
+        e = launch_pdl(tc::attn_kernel<64>, dim3(sm_count), tc::NTHREADS, tc::Smem<64>::ALLOC, stream, mk, mv, mq, p);
         if (e != cudaSuccess) return e;
         *launched = 1;
         e = p.G > 1 ? launch_pdl(tc::combine_kernel<64, 4>, dim3(sm_count, 4), 2 * tc::PAIR, 0, stream, p)

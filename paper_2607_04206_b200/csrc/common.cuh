@@ -43,6 +43,20 @@ __device__ __forceinline__ void raise_flag(uint32_t* flags, uint32_t f) {
     if (flags) atomicOr(flags, f);
 }
 
+// All kernels are launched with programmatic stream serialization (they call griddepcontrol.wait before touching
+// global memory), also under stream capture: the graph keeps the programmatic edges.
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, unsigned block, size_t smem, cudaStream_t stream,
+                                     Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
 // Optional event trace of CTA 0 (debug builds with -DSANGAM_TRACE only; compiled out otherwise).
 #ifdef SANGAM_TRACE
 #define SANGAM_TRACE_CAP 8192            // events per warp

@@ -116,13 +116,6 @@ __device__ __forceinline__ void fence_proxy_async_smem() {
 __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap* m) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(m)) : "memory");
 }
-__device__ __forceinline__ void tma_load_2d(uint32_t dst_smem, const CUtensorMap* m, uint32_t bar, int32_t c0, int32_t c1) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-        ::"r"(dst_smem), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1)
-        : "memory");
-}
-
 __device__ __forceinline__ void tma_load_3d(uint32_t dst_smem, const CUtensorMap* m, uint32_t bar, int32_t c0, int32_t c1, int32_t c2) {
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
@@ -185,6 +178,24 @@ __device__ __forceinline__ void mma_ss_x4(uint32_t d_tmem, uint64_t a_desc, uint
         "add.u64 a, a, st;\n\tadd.u64 b, b, st;\n\t"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p;\n\t}"
         ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(step)
+        : "memory");
+}
+// Four K-steps of D (+)= A B, both operands in smem, with separate descriptor steps for A and B (16-byte units)
+__device__ __forceinline__ void mma_ss_x4_ab(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate,
+                                             uint32_t a_step, uint32_t b_step) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b64 a, b, sa, sb;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "mov.b64 a, %1;\n\tmov.b64 b, %2;\n\tcvt.u64.u32 sa, %5;\n\tcvt.u64.u32 sb, %6;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p;\n\t"
+        "setp.ne.b32 p, 1, 0;\n\t"
+        "add.u64 a, a, sa;\n\tadd.u64 b, b, sb;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p;\n\t"
+        "add.u64 a, a, sa;\n\tadd.u64 b, b, sb;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p;\n\t"
+        "add.u64 a, a, sa;\n\tadd.u64 b, b, sb;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(a_step), "r"(b_step)
         : "memory");
 }
 // Four K-steps of D (+)= A B with A in TMEM (8 packed bf16 columns per step) and B in smem
@@ -267,6 +278,19 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
+// warp-wide maximum of an fp32 value (CREDUX.MAX.F32, sm_100a): every lane gets the result
+__device__ __forceinline__ float redux_max(float v) {
+    float r;
+    asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+    return r;
+}
+// named barrier for a subset of the CTA's warps
+__device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+// store the low / high bf16 of a packed pair to two shared-memory addresses
+__device__ __forceinline__ void sts_bf16_pair(uint32_t addr_lo, uint32_t addr_hi, uint32_t packed) {
+    asm volatile("{\n\t.reg .b16 lo, hi;\n\tmov.b32 {lo, hi}, %2;\n\tst.shared.b16 [%0], lo;\n\tst.shared.b16 [%1], hi;\n\t}"
+                 ::"r"(addr_lo), "r"(addr_hi), "r"(packed) : "memory");
+}
 __device__ __forceinline__ float ex2(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));

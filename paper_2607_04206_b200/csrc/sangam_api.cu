@@ -9,10 +9,15 @@
 
 #include <new>
 
+#include "attn_dec.cuh"
 #include "attn_simt.cuh"
 #include "attn_tc.cuh"
 #include "common.cuh"
 #include "kv_write.cuh"
+
+constexpr int MAP_CACHE = 64;
+struct MapCacheKV { const void *k, *v; uint64_t tick; CUtensorMap mk, mv; };
+struct MapCacheQ { const void* q; int32_t rows; uint64_t tick; CUtensorMap main, dec; };
 
 struct sangam_ctx {
     sangam_config cfg;
@@ -25,12 +30,17 @@ struct sangam_ctx {
     void* d_slot_meta;
     int32_t* d_plan_cache;
     int32_t num_slots;
-    // tensor maps for the K / V pools, re-encoded when the pool pointer changes
-    TcMaps maps;
-    const void* maps_k;
-    const void* maps_v;
-    const void* maps_q;
-    int32_t maps_q_rows;
+    // decode kernel (attn_dec.cuh): resident CTAs per SM (0: unavailable), its split-KV workspace
+    int dec_occ;
+    int dispatch;                 // SANGAM_DISPATCH_*
+    float* d_dec_part_o;
+    float* d_dec_part_ml;
+    int32_t* d_dec_cnt;
+    // tensor-map caches: a model passes per-layer pools and per-layer q buffers, so the encoded maps are kept per
+    // (k_pages, v_pages) and per (q, total_q) -- cuTensorMapEncodeTiled costs microseconds of host time per call
+    MapCacheKV kv_cache[MAP_CACHE];
+    MapCacheQ q_cache[MAP_CACHE];
+    uint64_t map_tick;
     // staging for sangam_iteration_host (allocated on first use)
     void *s_q, *s_k, *s_v, *s_out;
     int32_t *s_slot, *s_bt, *s_cu, *s_ctx;
@@ -52,6 +62,27 @@ static int cuda_fail(sangam_ctx* c, cudaError_t e, const char* where) {
         if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);  \
     } while (0)
 
+// Every entry point runs on the ctx's device whatever device the calling thread has current, and leaves the
+// caller's current device as it found it.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int dev) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != dev) {
+            err = cudaSetDevice(dev);
+            switched = err == cudaSuccess;
+        }
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+#define ON_CTX_DEVICE(ctx)                                                          \
+    DeviceGuard guard_((ctx)->cfg.device);                                         \
+    if (guard_.err != cudaSuccess) return cuda_fail((ctx), guard_.err, "cudaSetDevice")
+
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 extern "C" const char* sangam_version(void) { return "sangam-b200 0.1 (sm_100a)"; }
@@ -70,12 +101,17 @@ extern "C" int sangam_create(const sangam_config* cfg, sangam_ctx** out) {
     if (cfg->num_pages <= 0 || cfg->max_batch <= 0 || cfg->max_total_q <= 0 || cfg->max_pages_per_req <= 0)
         return SANGAM_ERR_INVALID_ARG;
     if ((int64_t)cfg->num_pages * SANGAM_PAGE > 0x7fffffffLL) return SANGAM_ERR_INVALID_ARG;
+    // TMA page coordinate (page * Hkv + g) * 2 (and the out-of-range coordinate of a bad page id) must fit an int32
+    if (((int64_t)cfg->num_pages + 1) * cfg->num_kv_heads * 2 > 0x7fffffffLL) return SANGAM_ERR_INVALID_ARG;
+    // the planners divide row counts by a magic multiplier that is exact below 2^24
+    if (cfg->max_total_q >= (1 << 24)) return SANGAM_ERR_INVALID_ARG;
     sangam_ctx* ctx = new (std::nothrow) sangam_ctx();
     if (!ctx) return SANGAM_ERR_WORKSPACE;
     memset(ctx, 0, sizeof *ctx);
     ctx->cfg = *cfg;
     ctx->G = cfg->num_q_heads / cfg->num_kv_heads;
-    cudaError_t e = cudaSetDevice(cfg->device);
+    DeviceGuard guard(cfg->device);                     // the caller's current device is restored on return
+    cudaError_t e = guard.err;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, cfg->device);
     ctx->num_slots = 2 * (ctx->sm_count > 0 ? ctx->sm_count : 148);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_flags, sizeof(uint32_t));
@@ -90,6 +126,18 @@ extern "C" int sangam_create(const sangam_config* cfg, sangam_ctx** out) {
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_plan_cache, plan_bytes);
     if (e == cudaSuccess) e = cudaMemset(ctx->d_plan_cache, 0, plan_bytes);
     if (e == cudaSuccess) e = tc_configure(cfg->head_dim);
+    if (e == cudaSuccess && ctx->G <= dec::NQ) {
+        // decode kernel: dec_occ CTAs per SM; the flattened weighted unit list must stay below 2^31 coordinates
+        const int64_t worst = (int64_t)cfg->max_total_q * cfg->num_kv_heads * ((int64_t)cfg->max_pages_per_req + dec::OV);
+        ctx->dec_occ = worst < 0x7fffffffLL ? dec_configure(cfg->head_dim) : 0;
+        if (ctx->dec_occ > 0) {
+            const size_t nslots = (size_t)2 * ctx->dec_occ * ctx->sm_count;
+            e = cudaMalloc(&ctx->d_dec_part_o, nslots * dec::NQ * cfg->head_dim * sizeof(float));
+            if (e == cudaSuccess) e = cudaMalloc(&ctx->d_dec_part_ml, nslots * dec::NQ * 2 * sizeof(float));
+            if (e == cudaSuccess) e = cudaMalloc(&ctx->d_dec_cnt, (size_t)ctx->dec_occ * ctx->sm_count * sizeof(int32_t));
+            if (e == cudaSuccess) e = cudaMemset(ctx->d_dec_cnt, 0, (size_t)ctx->dec_occ * ctx->sm_count * sizeof(int32_t));
+        }
+    }
     if (e != cudaSuccess) {
         sangam_destroy(ctx);
         return SANGAM_ERR_CUDA;
@@ -100,6 +148,8 @@ extern "C" int sangam_create(const sangam_config* cfg, sangam_ctx** out) {
 
 extern "C" int sangam_destroy(sangam_ctx* ctx) {
     if (!ctx) return SANGAM_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->cfg.device);
+    cudaFree(ctx->d_dec_part_o); cudaFree(ctx->d_dec_part_ml); cudaFree(ctx->d_dec_cnt);
     cudaFree(ctx->d_flags); cudaFree(ctx->d_sched); cudaFree(ctx->d_part_o); cudaFree(ctx->d_part_ml); cudaFree(ctx->d_slot_meta); cudaFree(ctx->d_plan_cache);
     cudaFree(ctx->s_q); cudaFree(ctx->s_k); cudaFree(ctx->s_v); cudaFree(ctx->s_out);
     cudaFree(ctx->s_slot); cudaFree(ctx->s_bt); cudaFree(ctx->s_cu); cudaFree(ctx->s_ctx);
@@ -109,6 +159,7 @@ extern "C" int sangam_destroy(sangam_ctx* ctx) {
 
 extern "C" int sangam_device_status(sangam_ctx* ctx, uint32_t* flags) {
     if (!ctx || !flags) return SANGAM_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(ctx);
     CK(cudaDeviceSynchronize());
     CK(cudaMemcpy(flags, ctx->d_flags, sizeof(uint32_t), cudaMemcpyDeviceToHost));
     return SANGAM_OK;
@@ -116,6 +167,7 @@ extern "C" int sangam_device_status(sangam_ctx* ctx, uint32_t* flags) {
 
 extern "C" int sangam_clear_device_status(sangam_ctx* ctx) {
     if (!ctx) return SANGAM_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(ctx);
     CK(cudaDeviceSynchronize());
     CK(cudaMemset(ctx->d_flags, 0, sizeof(uint32_t)));
     return SANGAM_OK;
@@ -129,6 +181,7 @@ extern "C" int sangam_kv_write(sangam_ctx* ctx, const void* k, const void* v, co
     if (!k || !v || !slot_mapping || !k_pages || !v_pages) return fail(ctx, SANGAM_ERR_INVALID_ARG, "kv_write: null pointer");
     if (!aligned16(k) || !aligned16(v) || !aligned16(k_pages) || !aligned16(v_pages))
         return fail(ctx, SANGAM_ERR_INVALID_ARG, "kv_write: pointer not 16-byte aligned");
+    ON_CTX_DEVICE(ctx);
     const int cpr = ctx->cfg.head_dim / 8;
     const int64_t total = (int64_t)num_tokens * ctx->cfg.num_kv_heads * cpr;
     constexpr int UNROLL = 4;
@@ -184,6 +237,7 @@ extern "C" int sangam_block_attn_simt(sangam_ctx* ctx, const void* q, const void
                                       int32_t batch, int32_t total_q, float scale, void* out, void* stream) {
     int rc = check_attn_args(ctx, q, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, batch, total_q, out);
     if (rc != SANGAM_OK) return rc > 0 ? SANGAM_OK : rc;
+    ON_CTX_DEVICE(ctx);
     AttnParams p = make_params(ctx, q, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, batch, total_q, scale, out);
     const int64_t warps = (int64_t)total_q * p.Hq;
     const unsigned blocks = (unsigned)((warps + 7) / 8);
@@ -199,21 +253,77 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
                                  int32_t batch, int32_t total_q, float scale, void* out, void* stream) {
     int rc = check_attn_args(ctx, q, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, batch, total_q, out);
     if (rc != SANGAM_OK) return rc > 0 ? SANGAM_OK : rc;
-    if (ctx->maps_k != k_pages || ctx->maps_v != v_pages) {   // per-layer pools: re-encode on pointer change (host only)
-        if (tc_encode_maps(&ctx->maps, k_pages, v_pages, ctx->cfg.num_pages, ctx->cfg.num_kv_heads, ctx->cfg.head_dim) != 0)
-            return fail(ctx, SANGAM_ERR_CUDA, "block_attn: cuTensorMapEncodeTiled failed");
-        ctx->maps_k = k_pages; ctx->maps_v = v_pages;
+    ON_CTX_DEVICE(ctx);
+    const sangam_config& c = ctx->cfg;
+    // tensor maps of this call's pools and q buffer (host-side cache, least recently used entry replaced)
+    MapCacheKV* kv = nullptr;
+    MapCacheQ* qm = nullptr;
+    ++ctx->map_tick;
+    for (int i = 0; i < MAP_CACHE; ++i) {
+        if (ctx->kv_cache[i].tick && ctx->kv_cache[i].k == k_pages && ctx->kv_cache[i].v == v_pages) kv = &ctx->kv_cache[i];
+        if (ctx->q_cache[i].tick && ctx->q_cache[i].q == q && ctx->q_cache[i].rows == total_q) qm = &ctx->q_cache[i];
     }
-    if (ctx->maps_q != q || ctx->maps_q_rows != total_q) {
-        if (tc_encode_q(&ctx->maps, q, total_q, ctx->cfg.num_q_heads, ctx->cfg.head_dim, ctx->G, 128 / ctx->G) != 0)
+    if (!kv) {
+        kv = &ctx->kv_cache[0];
+        for (int i = 1; i < MAP_CACHE; ++i) if (ctx->kv_cache[i].tick < kv->tick) kv = &ctx->kv_cache[i];
+        kv->tick = 0;
+        if (tmap_encode_pool(&kv->mk, k_pages, c.num_pages, c.num_kv_heads, c.head_dim) != 0 ||
+            tmap_encode_pool(&kv->mv, v_pages, c.num_pages, c.num_kv_heads, c.head_dim) != 0)
+            return fail(ctx, SANGAM_ERR_CUDA, "block_attn: cuTensorMapEncodeTiled failed");
+        kv->k = k_pages; kv->v = v_pages;
+    }
+    kv->tick = ctx->map_tick;
+    if (!qm) {
+        qm = &ctx->q_cache[0];
+        for (int i = 1; i < MAP_CACHE; ++i) if (ctx->q_cache[i].tick < qm->tick) qm = &ctx->q_cache[i];
+        qm->tick = 0;
+        if (tmap_encode_q(&qm->main, q, total_q, c.num_q_heads, c.head_dim, ctx->G, 128 / ctx->G) != 0 ||
+            (ctx->dec_occ > 0 && tmap_encode_q(&qm->dec, q, total_q, c.num_q_heads, c.head_dim, ctx->G, dec::NQ / ctx->G) != 0))
             return fail(ctx, SANGAM_ERR_CUDA, "block_attn: cuTensorMapEncodeTiled (q) failed");
-        ctx->maps_q = q; ctx->maps_q_rows = total_q;
+        qm->q = q; qm->rows = total_q;
+    }
+    qm->tick = ctx->map_tick;
+
+    // Decode-shaped batches (on average at most one 32-row unit per request and kv head: block decodes)
+    // go to the swapped-operand decode kernel; prefill / refresh / hybrid batches to the two-stream kernel.  Both
+    // compute the same function for any batch; the choice only affects speed.  Lengths live on the device, so the
+    // host decides on the counts it knows: total_q and batch.
+    bool use_dec = ctx->dec_occ > 0 && (int64_t)total_q * ctx->G <= (int64_t)dec::NQ * batch;
+    if (ctx->dispatch == SANGAM_DISPATCH_PREFILL) use_dec = false;
+    if (ctx->dispatch == SANGAM_DISPATCH_DECODE) {
+        if (ctx->dec_occ <= 0) return fail(ctx, SANGAM_ERR_UNSUPPORTED, "block_attn: the decode kernel is not available for this geometry");
+        use_dec = true;
+    }
+    if (use_dec) {
+        DecParams d;
+        d.block_table = block_table; d.cu_q_lens = cu_q_lens; d.ctx_lens = ctx_lens;
+        d.out = (__nv_bfloat16*)out;
+        d.batch = batch; d.total_q = total_q;
+        d.Hq = c.num_q_heads; d.Hkv = c.num_kv_heads; d.G = ctx->G; d.W = c.max_pages_per_req; d.P = c.num_pages;
+        d.tq = dec::NQ / ctx->G;
+        d.tq_magic = (uint32_t)(0x100000000ull / (uint64_t)d.tq) + 1u;
+        d.scale_log2 = scale * 1.4426950408889634f;
+        d.part_o = ctx->d_dec_part_o; d.part_ml = ctx->d_dec_part_ml; d.piece_cnt = ctx->d_dec_cnt; d.flags = ctx->d_flags;
+        cudaError_t e = dec_launch(d, kv->mk, kv->mv, qm->dec, c.head_dim, ctx->dec_occ * ctx->sm_count, (cudaStream_t)stream);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "block_attn launch (decode kernel)");
+        ctx->launches += 1;
+        return SANGAM_OK;
     }
     AttnParams p = make_params(ctx, q, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, batch, total_q, scale, out);
     int launched = 0;
-    cudaError_t e = tc_launch(p, ctx->maps, ctx->cfg.head_dim, ctx->sm_count, (cudaStream_t)stream, &launched);
+    cudaError_t e = tc_launch(p, kv->mk, kv->mv, qm->main, c.head_dim, ctx->sm_count, (cudaStream_t)stream, &launched);
     ctx->launches += launched;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "block_attn launch");
+    return SANGAM_OK;
+}
+
+extern "C" int sangam_set_dispatch(sangam_ctx* ctx, int32_t mode) {
+    if (!ctx) return SANGAM_ERR_INVALID_ARG;
+    if (mode != SANGAM_DISPATCH_AUTO && mode != SANGAM_DISPATCH_PREFILL && mode != SANGAM_DISPATCH_DECODE)
+        return fail(ctx, SANGAM_ERR_INVALID_ARG, "set_dispatch: unknown mode");
+    if (mode == SANGAM_DISPATCH_DECODE && ctx->dec_occ <= 0)
+        return fail(ctx, SANGAM_ERR_UNSUPPORTED, "set_dispatch: the decode kernel is not available for this geometry");
+    ctx->dispatch = mode;
     return SANGAM_OK;
 }
 
@@ -243,6 +353,7 @@ extern "C" int sangam_iteration_host(sangam_ctx* ctx, const void* q_host, const 
         return fail(ctx, SANGAM_ERR_WORKSPACE, "iteration_host: batch / total_q / num_tokens above the ctx maxima");
     if (!q_host || !out_host || !block_table_host || !cu_q_lens_host || !ctx_lens_host || (num_tokens && (!k_host || !v_host || !slot_mapping_host)))
         return fail(ctx, SANGAM_ERR_INVALID_ARG, "iteration_host: null pointer");
+    ON_CTX_DEVICE(ctx);
     int rc = ensure_staging(ctx);
     if (rc != SANGAM_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
