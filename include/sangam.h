@@ -118,6 +118,12 @@ int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_pages, const
 #define SANGAM_DISPATCH_DECODE  2
 int sangam_set_dispatch(sangam_ctx* ctx, int32_t mode);
 
+/* Read-only facts about a ctx (host side, no device work); -1 for an unknown `what`. */
+#define SANGAM_QUERY_SM_COUNT            0   /* SMs of the ctx's device */
+#define SANGAM_QUERY_DECODE_CTAS_PER_SM  1   /* resident CTAs per SM of the decode kernel (0: kernel unavailable) */
+#define SANGAM_QUERY_DISPATCH            2   /* current SANGAM_DISPATCH_* mode */
+int32_t sangam_query(const sangam_ctx* ctx, int32_t what);
+
 /*
  * Same contract as sangam_block_attn, computed by a plain CUDA-core (no tensor core) kernel with
  * fp32 arithmetic.  A cross-check for the tcgen05 path on workloads too large for the CPU oracle;

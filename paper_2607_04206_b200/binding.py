@@ -11,7 +11,7 @@ LIB_PATH = os.path.join(HERE, "libsangam.so")
 DECLARED_SYMBOLS = [
     "sangam_create", "sangam_destroy", "sangam_kv_write", "sangam_block_attn", "sangam_block_attn_simt",
     "sangam_iteration_host", "sangam_device_status", "sangam_clear_device_status", "sangam_launch_count",
-    "sangam_last_error", "sangam_version", "sangam_set_dispatch",
+    "sangam_last_error", "sangam_version", "sangam_set_dispatch", "sangam_query",
 ]
 
 DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE = 0, 1, 2
@@ -57,6 +57,8 @@ def load_library(build_if_missing: bool = False):
     lib.sangam_last_error.restype = ctypes.c_char_p
     lib.sangam_version.restype = ctypes.c_char_p
     lib.sangam_set_dispatch.argtypes = [vp, i32]
+    lib.sangam_query.argtypes = [vp, i32]
+    lib.sangam_query.restype = i32
     _lib = lib
     return lib
 
@@ -127,6 +129,10 @@ class Sangam:
     def set_dispatch(self, mode: int):
         """DISPATCH_AUTO / DISPATCH_PREFILL / DISPATCH_DECODE: which attention kernel sangam_block_attn launches."""
         self._check(self.lib.sangam_set_dispatch(self.ctx, int(mode)))
+
+    def query(self, what: int) -> int:
+        """0: SM count, 1: decode-kernel CTAs per SM, 2: dispatch mode."""
+        return int(self.lib.sangam_query(self.ctx, int(what)))
 
     def device_status(self) -> int:
         f = ctypes.c_uint32(0)

@@ -65,6 +65,9 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
 }
 // Bounded wait: a protocol bug must end the kernel with a flag, never hang the GPU.
 // `abort_flag` is a CTA-shared word; once set every later wait returns at once.
+#ifndef SANGAM_WAIT_HINT_NS
+#define SANGAM_WAIT_HINT_NS 20000u
+#endif
 #ifndef SANGAM_WAIT_MAX_SPINS
 #define SANGAM_WAIT_MAX_SPINS (1u << 17)
 #endif
@@ -84,7 +87,7 @@ __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatil
 #endif
     uint32_t spins = 0;
     bool ok = true;
-    while (!mbar_try_wait_hint(bar, parity, 20000u)) {
+    while (!mbar_try_wait_hint(bar, parity, SANGAM_WAIT_HINT_NS)) {
         if ((++spins & 0xFu) == 0 && (*abort_flag || spins > SANGAM_WAIT_MAX_SPINS)) {
 #ifdef SANGAM_WAIT_TABLE
             if (!*abort_flag && atomicCAS(&g_timeout_info[0], 0u, bar | 0x80000000u) == 0u) {
@@ -251,6 +254,15 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
           "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
           "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
           "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
         : "r"(taddr)
         : "memory");
 }

@@ -125,7 +125,11 @@ extern "C" int sangam_create(const sangam_config* cfg, sangam_ctx** out) {
     const size_t plan_bytes = (size_t)(ctx->sm_count > 0 ? ctx->sm_count : 148) * PLAN_CACHE_INTS * sizeof(int32_t);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_plan_cache, plan_bytes);
     if (e == cudaSuccess) e = cudaMemset(ctx->d_plan_cache, 0, plan_bytes);
+#ifdef SANGAM_TRACE
+    if (e == cudaSuccess) { tc_configure(cfg->head_dim); cudaGetLastError(); }   // the trace build's static shared memory can push attn_kernel<128> over the limit
+#else
     if (e == cudaSuccess) e = tc_configure(cfg->head_dim);
+#endif
     if (e == cudaSuccess && ctx->G <= dec::NQ) {
         // decode kernel: dec_occ CTAs per SM; the flattened weighted unit list must stay below 2^31 coordinates
         const int64_t worst = (int64_t)cfg->max_total_q * cfg->num_kv_heads * ((int64_t)cfg->max_pages_per_req + dec::OV);
@@ -134,8 +138,10 @@ extern "C" int sangam_create(const sangam_config* cfg, sangam_ctx** out) {
             const size_t nslots = (size_t)2 * ctx->dec_occ * ctx->sm_count;
             e = cudaMalloc(&ctx->d_dec_part_o, nslots * dec::NQ * cfg->head_dim * sizeof(float));
             if (e == cudaSuccess) e = cudaMalloc(&ctx->d_dec_part_ml, nslots * dec::NQ * 2 * sizeof(float));
-            if (e == cudaSuccess) e = cudaMalloc(&ctx->d_dec_cnt, (size_t)ctx->dec_occ * ctx->sm_count * sizeof(int32_t));
-            if (e == cudaSuccess) e = cudaMemset(ctx->d_dec_cnt, 0, (size_t)ctx->dec_occ * ctx->sm_count * sizeof(int32_t));
+            // one arrival counter per work unit: at most Hkv * (rows + requests) units in a batch
+            const size_t ncnt = (size_t)cfg->num_kv_heads * ((size_t)cfg->max_total_q + cfg->max_batch);
+            if (e == cudaSuccess) e = cudaMalloc(&ctx->d_dec_cnt, ncnt * sizeof(int32_t));
+            if (e == cudaSuccess) e = cudaMemset(ctx->d_dec_cnt, 0, ncnt * sizeof(int32_t));
         }
     }
     if (e != cudaSuccess) {
@@ -302,8 +308,16 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
         d.Hq = c.num_q_heads; d.Hkv = c.num_kv_heads; d.G = ctx->G; d.W = c.max_pages_per_req; d.P = c.num_pages;
         d.tq = dec::NQ / ctx->G;
         d.tq_magic = (uint32_t)(0x100000000ull / (uint64_t)d.tq) + 1u;
+        d.g_magic = (uint32_t)(0x100000000ull / (uint64_t)ctx->G) + 1u;
         d.scale_log2 = scale * 1.4426950408889634f;
-        d.part_o = ctx->d_dec_part_o; d.part_ml = ctx->d_dec_part_ml; d.piece_cnt = ctx->d_dec_cnt; d.flags = ctx->d_flags;
+#ifdef SANGAM_TRACE
+        { unsigned int v = 0; cudaMemcpyFromSymbol(&v, g_trace_cta, sizeof v); d.trace_cta = (int)v; }
+#endif
+        d.part_o = ctx->d_dec_part_o; d.part_ml = ctx->d_dec_part_ml; d.unit_cnt = ctx->d_dec_cnt; d.min_w = dec::MIN_W; d.ov = dec::OV;
+#ifdef SANGAM_TUNING_ENV
+        if (const char* e_ = getenv("SANGAM_DEC_OV")) d.ov = atoi(e_);
+        if (const char* e_ = getenv("SANGAM_DEC_MINW")) d.min_w = atoi(e_);
+#endif d.flags = ctx->d_flags;
         cudaError_t e = dec_launch(d, kv->mk, kv->mv, qm->dec, c.head_dim, ctx->dec_occ * ctx->sm_count, (cudaStream_t)stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "block_attn launch (decode kernel)");
         ctx->launches += 1;
@@ -315,6 +329,16 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
     ctx->launches += launched;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "block_attn launch");
     return SANGAM_OK;
+}
+
+extern "C" int32_t sangam_query(const sangam_ctx* ctx, int32_t what) {
+    if (!ctx) return -1;
+    switch (what) {
+        case SANGAM_QUERY_SM_COUNT: return ctx->sm_count;
+        case SANGAM_QUERY_DECODE_CTAS_PER_SM: return ctx->dec_occ;
+        case SANGAM_QUERY_DISPATCH: return ctx->dispatch;
+        default: return -1;
+    }
 }
 
 extern "C" int sangam_set_dispatch(sangam_ctx* ctx, int32_t mode) {
@@ -393,7 +417,7 @@ extern "C" int sangam_debug_timeout_info(unsigned int* out20) {
 #ifdef SANGAM_TRACE
 extern "C" int sangam_trace_cta_times(unsigned long long* host_buf) {
     cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(host_buf, g_cta_times, sizeof(unsigned long long) * 512);
+    cudaMemcpyFromSymbol(host_buf, g_cta_times, sizeof(unsigned long long) * 1024);
     return 0;
 }
 extern "C" int sangam_trace_set_cta(int cta) {
