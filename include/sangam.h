@@ -37,9 +37,15 @@
  *
  * Errors: every call returns 0 on success or a negative sangam_status; nothing throws or aborts.
  * sangam_last_error gives a message for the last failing call on that ctx.  Conditions only the
- * device can see (a context needing more than max_pages_per_req pages, a page id >= num_pages,
- * a slot >= num_pages*16) never fault: the offending request/row is skipped and a sticky flag is
- * raised, readable with sangam_device_status after a stream sync.
+ * device can see never fault; each raises a sticky flag, readable with sangam_device_status after
+ * a stream sync, and is handled the same way by every kernel of the library:
+ *   - a page id outside [0, num_pages) among the first ceil(ctx_len/16) block-table entries
+ *     (SANGAM_DEV_BAD_PAGE): that page's 16 positions are read as K = V = 0 (logit 0, value 0);
+ *     the request is still computed, other requests are unaffected;
+ *   - a context needing more than max_pages_per_req pages (SANGAM_DEV_CTX_TOO_LONG): the request
+ *     is treated as ctx_len = 0, i.e. its output rows are zeros;
+ *   - a slot >= num_pages*16 in sangam_kv_write (SANGAM_DEV_BAD_SLOT): that row is not written.
+ * Negative ctx_lens are read as 0, decreasing cu_q_lens as an empty request (no flag).
  * One ctx per stream; calls on one ctx are not re-entrant.
  */
 #ifndef SANGAM_H_
@@ -63,8 +69,8 @@ typedef enum {
 
 /* sticky device-side flags (sangam_device_status) */
 #define SANGAM_DEV_BAD_SLOT   1u      /* kv_write: slot >= num_pages*16, row skipped */
-#define SANGAM_DEV_BAD_PAGE   2u      /* block_attn: page id out of [0,num_pages), request skipped */
-#define SANGAM_DEV_CTX_TOO_LONG 4u    /* block_attn: ctx_len needs more than max_pages_per_req pages */
+#define SANGAM_DEV_BAD_PAGE   2u      /* block_attn: page id out of [0,num_pages): the page reads as K = V = 0 */
+#define SANGAM_DEV_CTX_TOO_LONG 4u    /* block_attn: ctx_len needs more than max_pages_per_req pages: rows are zeros */
 #define SANGAM_DEV_TIMEOUT    8u      /* an in-kernel barrier wait gave up (internal error) */
 #define SANGAM_DEV_INTERNAL  16u      /* an internal bounds guard tripped; the access was skipped (internal error) */
 

@@ -35,11 +35,12 @@ attn_simt_kernel(AttnParams p) {
     const int32_t* bt = p.block_table + (int64_t)r * p.W;
     for (int32_t j = 0; j < c; ++j) {
         const int32_t page = __ldg(bt + (j >> 4));
-        if (page < 0 || page >= p.P) { raise_flag(p.flags, DEV_BAD_PAGE); continue; }
-        const int64_t row = (((int64_t)page * p.Hkv + g) * SANGAM_PAGE + (j & 15)) * D + lane * EPL;
+        const bool bad = page < 0 || page >= p.P;         // flagged; the page's positions read as K = V = 0 (sangam.h)
+        if (bad) raise_flag(p.flags, DEV_BAD_PAGE);
+        const int64_t row = (((int64_t)(bad ? 0 : page) * p.Hkv + g) * SANGAM_PAGE + (j & 15)) * D + lane * EPL;
         float dot = 0.f;
 #pragma unroll
-        for (int e = 0; e < EPL; ++e) dot += qv[e] * __bfloat162float(p.k_pages[row + e]);
+        for (int e = 0; e < EPL; ++e) dot += bad ? 0.f : qv[e] * __bfloat162float(p.k_pages[row + e]);
 #pragma unroll
         for (int s = 16; s > 0; s >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, s);
         const float sj = dot * p.scale;
@@ -47,7 +48,7 @@ attn_simt_kernel(AttnParams p) {
         const float corr = expf(m - mn), pj = expf(sj - mn);
         l = l * corr + pj;
 #pragma unroll
-        for (int e = 0; e < EPL; ++e) acc[e] = acc[e] * corr + pj * __bfloat162float(p.v_pages[row + e]);
+        for (int e = 0; e < EPL; ++e) acc[e] = acc[e] * corr + (bad ? 0.f : pj * __bfloat162float(p.v_pages[row + e]));
         m = mn;
     }
     const float inv = l > 0.f ? 1.f / l : 0.f;

@@ -410,9 +410,12 @@ __device__ __forceinline__ void producer_warp(const AttnParams& p, const CUtenso
                 ++pos;
                 __syncwarp();
                 if (pg < np) {
-                    if ((unsigned)page >= (unsigned)p.P) raise_flag(p.flags, DEV_BAD_PAGE);   // TMA zero-fills out of range
+                    // a page id outside [0, P): flag, and address the first box past the pool -- TMA fills zeros, so the
+                    // page's 16 positions read as K = V = 0 (sangam.h; the same in attn_dec.cuh and attn_simt.cuh)
+                    const bool bad = (unsigned)page >= (unsigned)p.P;
+                    if (bad) raise_flag(p.flags, DEV_BAD_PAGE);
                     ptx::tma_load_4d(sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES + pg * (2 * KV_ATOM_STRIDE<D>)),
-                                     is_v ? mapV : mapK, bar(L::B_KV_FULL + stage), 0, 0, 0, (page * p.Hkv + it.g) * 2);
+                                     is_v ? mapV : mapK, bar(L::B_KV_FULL + stage), 0, 0, 0, ((bad ? p.P : page) * p.Hkv + it.g) * 2);
                 }
                 TRACE_EV(54);
                 if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }

@@ -284,3 +284,34 @@ def sample_rows(b: Batch, per_request: int = 64, seed: int = 1234) -> np.ndarray
             pick.add(int(g.integers(0, n)))
         rows.extend(base + e for e in sorted(pick))
     return np.asarray(rows, dtype=np.int32)
+
+
+# ---------------------------------------------------------------------------------------
+# Seeded synthetic arrival traces for the worker-level scheduler.
+# They stand in for the paper's filtered ShareGPT / arXiv-summarization traces,
+# which are not in the container: lengths are drawn from log-normal laws fitted to the MEDIAN and P99
+# of Table 1 (sigma = ln(P99 / median) / 2.326), requests above 4096 tokens are clipped like the paper's
+# filter, 1024 / 512 MASK positions are appended, arrivals are Poisson.  No trace item is
+# reproduced.  Only draws live here: no scheduling decision is taken in this module.
+# ---------------------------------------------------------------------------------------
+TRACE_STATS = {   # name: (prompt median, prompt P99, output median, output P99, appended MASK tokens)
+    "sharegpt_like": (795, 2007, 266, 874, 1024),
+    "arxiv_like": (2827, 3923, 162, 360, 512),
+}
+
+
+def sched_trace(seed: int, n: int, qps: float, kind: str = "sharegpt_like", block: int = 32, max_steps: int = 12):
+    """n requests: dict of arrays arrival [s], prompt_len, response_len, output_len, and steps[n][max blocks]
+    (denoising iterations each block takes: the paper's confidence-threshold unmasking makes this data
+    dependent; here uniform integers in [2, max_steps])."""
+    pm, p99, om, o99, resp = TRACE_STATS[kind]
+    g = np.random.default_rng(seed)
+    arrival = np.cumsum(g.exponential(1.0 / qps, n))
+    out = np.exp(np.log(om) + np.log(o99 / om) / 2.326 * g.standard_normal(n))
+    out = np.clip(np.rint(out), 1, resp).astype(np.int32)
+    prm = np.exp(np.log(pm) + np.log(p99 / pm) / 2.326 * g.standard_normal(n))
+    prm = np.clip(np.rint(prm), 16, 4096 - out).astype(np.int32)
+    nblk = (resp + block - 1) // block
+    steps = g.integers(2, max_steps, (n, nblk), endpoint=True).astype(np.int32)
+    return {"arrival": arrival, "prompt_len": prm, "response_len": np.full(n, resp, np.int32), "output_len": out,
+            "steps": steps, "block": block, "kind": kind}

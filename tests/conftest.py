@@ -17,3 +17,14 @@ def oracle():
     import oracle as o
     o.build()
     return o
+
+
+@pytest.fixture(params=["auto", "prefill_kernel", "decode_kernel"])
+def dispatch(request):
+    """Runs a -m gpu test once per attention kernel: the shape-based default, the two-stream (prefill / hybrid) kernel
+    forced, the swapped-operand decode kernel forced.  Both kernels must be correct for every batch."""
+    import gpu_harness
+    mode = {"auto": 0, "prefill_kernel": 1, "decode_kernel": 2}[request.param]
+    gpu_harness.DEFAULT_DISPATCH = mode
+    yield mode
+    gpu_harness.DEFAULT_DISPATCH = 0

@@ -8,6 +8,10 @@ import sangam_inputs as si
 
 MAX_ABS, MEAN_ABS = 2e-2, 2e-3      # north_star tolerance for bf16-in / fp32-accumulate attention
 
+# which attention kernel sangam_block_attn launches in DeviceBatch (0 auto, 1 two-stream prefill kernel, 2 decode
+# kernel); set per test by the `dispatch` fixture of conftest.py so that every parity / edge case runs through both
+DEFAULT_DISPATCH = 0
+
 
 def t_bf16(bits: np.ndarray, device="cuda"):
     import torch
@@ -41,6 +45,8 @@ class DeviceBatch:
                              num_pages=b.num_pages, max_batch=max_batch or max(b.batch, 1),
                              max_total_q=max_total_q or max(b.total_q, len(b.slot_cache), 1),
                              max_pages_per_req=b.max_pages_per_req)
+        if DEFAULT_DISPATCH:
+            self.eng.set_dispatch(DEFAULT_DISPATCH)
 
     def load_cache(self):
         self.eng.kv_write(self.k_cache, self.v_cache, self.slot_cache, self.k_pages, self.v_pages)

@@ -9,7 +9,7 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("hq,hkv,d", [(4, 4, 64), (8, 8, 128), (14, 2, 128), (7, 1, 64)])
-def test_length_edges(oracle, hq, hkv, d):
+def test_length_edges(oracle, hq, hkv, d, dispatch):
     q_lens = [0, 1, 16, 32, 33, 127, 128, 129, 5, 3, 2, 40]
     ctx = [5, 1, 15, 16, 17, 127, 128, 129, 255, 256, 257, 0]
     b = si.custom(41, q_lens, ctx, num_q_heads=hq, num_kv_heads=hkv, head_dim=d)
@@ -31,7 +31,7 @@ def test_length_edges(oracle, hq, hkv, d):
 
 
 @pytest.mark.parametrize("ctx,d,g", [(700, 128, 1), (1500, 128, 7), (300, 64, 1)])
-def test_identity_needle_prefill(oracle, ctx, d, g):
+def test_identity_needle_prefill(oracle, ctx, d, g, dispatch):
     """q_t = beta * k_t: row t's logit at j = t dominates, so out[t] == V[t] to 1 bf16 ulp for every t.
     Covers every context position, page mapping and tile boundary in one launch."""
     b = si.custom(42, [ctx], [ctx], num_q_heads=g, num_kv_heads=1, head_dim=d)
@@ -48,7 +48,7 @@ def test_identity_needle_prefill(oracle, ctx, d, g):
     assert np.all(err <= ulp + 1e-30), f"needle mismatch: max err {err.max():.3e}"
 
 
-def test_needle_sweep_decode(oracle):
+def test_needle_sweep_decode(oracle, dispatch):
     """Dominant position on the first/last slot of every page and on c-1 (decode shape, split-KV active)."""
     c, d = 1000, 128
     pos = sorted(set([p for pg in range((c + 15) // 16) for p in (16 * pg, min(16 * pg + 15, c - 1))] + [c - 1]))
@@ -63,7 +63,7 @@ def test_needle_sweep_decode(oracle):
     assert np.all(np.abs(got - v) <= np.abs(v) * 2.0 ** -7 + 1e-30)
 
 
-def test_poison_independence_and_bad_block_table_tail(oracle):
+def test_poison_independence_and_bad_block_table_tail(oracle, dispatch):
     b = si.config2(4)
     ref, _, _ = oracle.iteration(b)
     db = DeviceBatch(b, poison=True)
@@ -79,7 +79,7 @@ def test_poison_independence_and_bad_block_table_tail(oracle):
     assert db.eng.device_status() == 0
 
 
-def test_bitwise_reproducible(oracle):
+def test_bitwise_reproducible(oracle, dispatch):
     b = si.config3(8)
     db = DeviceBatch(b)
     a = bits_of(db.iteration()).copy()
@@ -108,7 +108,8 @@ def test_row_independence_decode_vs_prefill(oracle):
     assert np.max(np.abs(got - full[sub])) <= 4e-3
 
 
-def test_graph_replay_with_changed_lengths(oracle):
+@pytest.mark.parametrize("mode", [0, 1, 2], ids=["auto", "prefill_kernel", "decode_kernel"])
+def test_graph_replay_with_changed_lengths(oracle, mode):
     """Capture kv_write -> block_attn once at fixed capacities, replay with different lengths, pages and
     data written into the same buffers; every replay checked against the oracle; identical replays are
     bit-identical (CUDA Graphs: PAPER.md:258)."""
@@ -117,6 +118,7 @@ def test_graph_replay_with_changed_lengths(oracle):
     Hq, Hkv, D, R, W, P, QCAP, TNEW = 8, 8, 128, 6, 40, 400, 6 * 64, 6 * 64
     eng = sg.Sangam(num_q_heads=Hq, num_kv_heads=Hkv, head_dim=D, num_pages=P, max_batch=R, max_total_q=QCAP,
                     max_pages_per_req=W)
+    eng.set_dispatch(mode)
     dev = "cuda"
     q = torch.zeros(QCAP, Hq, D, dtype=torch.bfloat16, device=dev)
     out = torch.zeros_like(q)
@@ -183,7 +185,7 @@ def test_graph_replay_with_changed_lengths(oracle):
 
 
 @pytest.mark.parametrize("scale", [-0.0883883461356163, 0.0, 0.35])
-def test_scale_sign_and_magnitude(oracle, scale):
+def test_scale_sign_and_magnitude(oracle, scale, dispatch):
     """The logit scale is a caller-supplied float (reading S5): negative (the kernel flips the sign of S and works
     with |scale|), zero (uniform weights: out = mean of V, oracle pin 7) and large (exercises the lazy rescale:
     logits of up to +-40 in log2 units move the reference maximum many times)."""
@@ -198,7 +200,7 @@ def test_scale_sign_and_magnitude(oracle, scale):
     assert db.eng.device_status() == 0
 
 
-def test_more_than_32_requests(oracle):
+def test_more_than_32_requests(oracle, dispatch):
     """The planner keeps the first 32 requests' metadata in registers and reads the rest from global memory."""
     rng = np.random.default_rng(5)
     R = 45
@@ -216,7 +218,7 @@ def test_more_than_32_requests(oracle):
 
 
 @pytest.mark.parametrize("hq,hkv,d", [(8, 2, 64), (14, 2, 128), (4, 4, 128)])
-def test_decode_units_split_into_many_pieces(oracle, hq, hkv, d):
+def test_decode_units_split_into_many_pieces(oracle, hq, hkv, d, dispatch):
     """Few (request, kv head) units with long contexts: the stream-K cut gives every CTA about one kv tile, so a unit is
     merged from tens of partial pieces by combine_kernel (both its row paths, every column slice of the GQA grid)."""
     b = si.custom(49, [32, 32, 5], [3000, 5003, 2049], num_q_heads=hq, num_kv_heads=hkv, head_dim=d)
