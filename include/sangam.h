@@ -162,6 +162,75 @@ int64_t sangam_launch_count(const sangam_ctx* ctx);
 const char* sangam_last_error(const sangam_ctx* ctx);
 const char* sangam_version(void);
 
+
+/* ------------------------------------------------------------------------------------------------------------
+ * Worker-level scheduler: Algorithm 1 "Deficit token-budget scheduling" plus the builder of the
+ * batch metadata that sangam_kv_write / sangam_block_attn consume.  Host code only (integer logic, no device
+ * work, no CUDA calls); every array of sangam_batch is HOST memory owned by the caller.
+ *
+ * Each iteration has a token budget tau.  sangam_sched_next seats every in-flight decode first (Tokens = one
+ * block; decodes are never displaced), then admits waiting prefills -- fresh requests and block-boundary
+ * re-prefills, in request ARRIVAL-TIME order -- while Tokens(p) = prompt + response fits
+ * budget = tau - Tokens(decodes) + deficit; the first prefill that does not fit stops the scan (prefills cannot
+ * be split); the unspent budget max(budget, 0) is carried as the next iteration's deficit; with no prefill
+ * waiting the iteration is decode-only and the deficit is cleared.  Idle rule (liveness): while the
+ * microbatch is still empty the head prefill is admitted even above the budget.  Over any busy period of W
+ * iterations the admitted prefill tokens total at most W tau - sum_t Tokens(decodes_t).
+ * Readings where the paper is silent (S20-S22): equal arrival times keep submission order; a head prefill
+ * whose KV pages do not fit the free pool, or that would exceed max_batch / max_total_q, "does not fit" (also under
+ * the idle rule); pages are taken at a request's first admission and returned when its last block resolves.
+ *
+ * Life cycle of a request (Fast-dLLM style caching): submit -> prefill (whole prompt +
+ * response region) -> decode of block 0, one microbatch per denoising step, until the caller reports the block
+ * resolved -> re-prefill queued with the request's original arrival time -> decode of block 1 -> ... for
+ * ceil(min(output_len, response_len) / block) blocks, then the request retires.
+ * Batch layout: requests in microbatch order, decodes first.  A decode's query rows are its current
+ * block, a prefill's the whole sequence; ctx_len = prompt + response for both; slot_mapping lists the slot
+ * (page * 16 + offset) of every query row in order: the K/V rows the iteration rewrites.
+ */
+typedef struct sangam_sched sangam_sched;
+
+typedef struct {
+    int32_t tau;                /* per-iteration token budget (PAPER.md:327 evaluates 512 .. 16384) */
+    int32_t block;              /* response block = query rows of a decode (32) */
+    int32_t page_size;          /* must be 16 */
+    int32_t num_pages;          /* KV pool capacity in pages */
+    int32_t max_batch;          /* capacities of the sangam_batch arrays (and of the sangam_ctx the batch is run on) */
+    int32_t max_total_q;
+    int32_t max_pages_per_req;  /* block_table row width W */
+} sangam_sched_config;
+
+typedef struct {
+    int32_t batch;              /* requests in the microbatch: num_decodes decodes, then batch - num_decodes prefills */
+    int32_t num_decodes;
+    int32_t total_q;            /* = cu_q_lens[batch] */
+    int32_t num_new_tokens;     /* entries of slot_mapping (= total_q) */
+    int64_t deficit;            /* carried to the next iteration */
+    int64_t* req_ids;           /* [max_batch]                      (any array may be NULL: not filled) */
+    int32_t* cu_q_lens;         /* [max_batch + 1] */
+    int32_t* ctx_lens;          /* [max_batch] */
+    int32_t* block_table;       /* [max_batch][max_pages_per_req], -1 padded */
+    int32_t* slot_mapping;      /* [max_total_q] */
+} sangam_batch;
+
+int sangam_sched_create(const sangam_sched_config* cfg, sangam_sched** out);
+int sangam_sched_destroy(sangam_sched* s);
+/* A request arrives.  SANGAM_ERR_WORKSPACE if it could never be scheduled (more pages than the pool or the
+ * block-table width, more tokens than max_total_q); SANGAM_ERR_INVALID_ARG for a duplicate id or bad lengths. */
+int sangam_sched_submit(sangam_sched* s, int64_t req_id, double arrival_time, int32_t prompt_len, int32_t response_len,
+                        int32_t output_len);
+/* One iteration of Algorithm 1; fills *out.  Must be followed by sangam_sched_complete before the next call. */
+int sangam_sched_next(sangam_sched* s, sangam_batch* out);
+/* After the microbatch ran: block_done[i] != 0 says decode i resolved its block (n = num_decodes of the last batch). */
+int sangam_sched_complete(sangam_sched* s, const int32_t* block_done, int32_t n);
+
+#define SANGAM_SCHED_DEFICIT        0
+#define SANGAM_SCHED_WAITING        1   /* prefills in the queue */
+#define SANGAM_SCHED_IN_FLIGHT      2   /* decodes in flight */
+#define SANGAM_SCHED_FREE_PAGES     3
+#define SANGAM_SCHED_LIVE_REQUESTS  4
+int64_t sangam_sched_query(const sangam_sched* s, int32_t what);
+
 #ifdef __cplusplus
 }
 #endif

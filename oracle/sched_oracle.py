@@ -23,6 +23,8 @@ What it follows, step by step and in the paper's notation:
   * request life cycle (Fast-dLLM style caching): prefill -> decode block 0 for some
     denoising steps -> at the block boundary the cache is recomputed: a re-prefill of the whole sequence, queued with
     the request's ORIGINAL arrival time -> decode block 1 -> ... for ceil(output_len / block) blocks.
+  * capacities (reading S22): a head prefill that would exceed the batch arrays (max_batch requests, max_total_q rows)
+    does not fit either.
   * memory (reading S21; the paper only says "when memory capacity is also available"): a request's pages
     are taken at its first admission; if the pool cannot hold it, the head prefill "does not fit" and stops the scan
     like any other misfit -- except under the idle rule, where nothing can be done and the scan also stops.
@@ -51,8 +53,9 @@ class Request:
 
 
 class SchedOracle:
-    def __init__(self, tau, block=32, num_pages=1 << 20):
+    def __init__(self, tau, block=32, num_pages=1 << 20, max_batch=None, max_total_q=None):
         self.tau, self.block = int(tau), int(block)
+        self.max_batch, self.max_total_q = max_batch, max_total_q       # capacities of the batch arrays (reading S22)
         self.deficit = 0
         self.decodes = []            # in-flight decodes, in the order they became decodes
         self.prefills = []           # waiting prefills: (arrival, seq_no, request)
@@ -85,11 +88,17 @@ class SchedOracle:
             return self.last
         budget = self.tau - self.block * len(decodes) + self.deficit
         admitted = []
+        rows = sum(min(self.block, r.seq_len - (r.prompt_len + r.cur_block * self.block)) for r in decodes)
         while self.prefills:
             p = self.prefills[0][2]
             idle = (len(decodes) + len(admitted) == 0)
             fits_memory = p.pages is not None or self._pages_needed(p) <= len(self.free_pages)
+            if self.max_batch is not None and len(decodes) + len(admitted) >= self.max_batch:
+                fits_memory = False
+            if self.max_total_q is not None and rows + p.seq_len > self.max_total_q:
+                fits_memory = False
             if (p.seq_len <= budget or idle) and fits_memory:
+                rows += p.seq_len
                 self.prefills.pop(0)
                 if p.pages is None:
                     p.pages = [self.free_pages.pop() for _ in range(self._pages_needed(p))]

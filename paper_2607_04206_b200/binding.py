@@ -12,6 +12,8 @@ DECLARED_SYMBOLS = [
     "sangam_create", "sangam_destroy", "sangam_kv_write", "sangam_block_attn", "sangam_block_attn_simt",
     "sangam_iteration_host", "sangam_device_status", "sangam_clear_device_status", "sangam_launch_count",
     "sangam_last_error", "sangam_version", "sangam_set_dispatch", "sangam_query",
+    "sangam_sched_create", "sangam_sched_destroy", "sangam_sched_submit", "sangam_sched_next", "sangam_sched_complete",
+    "sangam_sched_query",
 ]
 
 DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE = 0, 1, 2
@@ -25,6 +27,17 @@ class _Config(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in (
         "num_q_heads", "num_kv_heads", "head_dim", "page_size", "num_pages", "max_batch", "max_total_q",
         "max_pages_per_req", "device")]
+
+
+class _SchedConfig(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("tau", "block", "page_size", "num_pages", "max_batch", "max_total_q", "max_pages_per_req")]
+
+
+class _Batch(ctypes.Structure):
+    _fields_ = [("batch", ctypes.c_int32), ("num_decodes", ctypes.c_int32), ("total_q", ctypes.c_int32),
+                ("num_new_tokens", ctypes.c_int32), ("deficit", ctypes.c_int64),
+                ("req_ids", ctypes.c_void_p), ("cu_q_lens", ctypes.c_void_p), ("ctx_lens", ctypes.c_void_p),
+                ("block_table", ctypes.c_void_p), ("slot_mapping", ctypes.c_void_p)]
 
 
 _lib = None
@@ -59,6 +72,13 @@ def load_library(build_if_missing: bool = False):
     lib.sangam_set_dispatch.argtypes = [vp, i32]
     lib.sangam_query.argtypes = [vp, i32]
     lib.sangam_query.restype = i32
+    lib.sangam_sched_create.argtypes = [ctypes.POINTER(_SchedConfig), ctypes.POINTER(vp)]
+    lib.sangam_sched_destroy.argtypes = [vp]
+    lib.sangam_sched_submit.argtypes = [vp, ctypes.c_int64, ctypes.c_double, i32, i32, i32]
+    lib.sangam_sched_next.argtypes = [vp, ctypes.POINTER(_Batch)]
+    lib.sangam_sched_complete.argtypes = [vp, vp, i32]
+    lib.sangam_sched_query.argtypes = [vp, i32]
+    lib.sangam_sched_query.restype = ctypes.c_int64
     _lib = lib
     return lib
 
@@ -144,3 +164,63 @@ class Sangam:
 
     def launch_count(self) -> int:
         return int(self.lib.sangam_launch_count(self.ctx))
+
+
+class Scheduler:
+    """sangam_sched (Algorithm 1 + batch metadata).  Host only: works without a CUDA device.  The batch arrays are
+    torch tensors when `pinned` (pinned host memory, ready for cudaMemcpyAsync), numpy arrays otherwise."""
+
+    def __init__(self, *, tau, num_pages, max_batch, max_total_q, max_pages_per_req, block=32, page_size=16, pinned=False):
+        import numpy as np
+        self.lib = load_library()
+        self.cfg = _SchedConfig(tau, block, page_size, num_pages, max_batch, max_total_q, max_pages_per_req)
+        self.s = ctypes.c_void_p()
+        rc = self.lib.sangam_sched_create(ctypes.byref(self.cfg), ctypes.byref(self.s))
+        if rc != 0:
+            raise SangamError(f"sangam_sched_create failed: {rc}")
+        shapes = {"req_ids": ((max_batch,), np.int64), "cu_q_lens": ((max_batch + 1,), np.int32), "ctx_lens": ((max_batch,), np.int32),
+                  "block_table": ((max_batch, max_pages_per_req), np.int32), "slot_mapping": ((max_total_q,), np.int32)}
+        self.tensors = {}
+        self.arrays = {}
+        for k, (shp, dt) in shapes.items():
+            if pinned:
+                import torch
+                t = torch.zeros(shp, dtype=torch.int64 if dt is np.int64 else torch.int32).pin_memory()
+                self.tensors[k] = t
+                self.arrays[k] = t.numpy()
+            else:
+                self.arrays[k] = np.zeros(shp, dtype=dt)
+        self.b = _Batch()
+        for k, a in self.arrays.items():
+            setattr(self.b, k, a.ctypes.data)
+
+    def close(self):
+        if self.s:
+            self.lib.sangam_sched_destroy(self.s)
+            self.s = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def submit(self, req_id, arrival_time, prompt_len, response_len, output_len) -> int:
+        return int(self.lib.sangam_sched_submit(self.s, int(req_id), float(arrival_time), int(prompt_len), int(response_len), int(output_len)))
+
+    def next(self):
+        """Runs one iteration of Algorithm 1; returns the filled batch header (arrays in self.arrays / self.tensors)."""
+        rc = self.lib.sangam_sched_next(self.s, ctypes.byref(self.b))
+        if rc != 0:
+            raise SangamError(f"sangam_sched_next failed: {rc}")
+        return self.b
+
+    def complete(self, block_done):
+        import numpy as np
+        a = np.ascontiguousarray(block_done, dtype=np.int32)
+        rc = self.lib.sangam_sched_complete(self.s, ctypes.c_void_p(a.ctypes.data if len(a) else 0), int(len(a)))
+        if rc != 0:
+            raise SangamError(f"sangam_sched_complete failed: {rc}")
+
+    def query(self, what: int) -> int:
+        return int(self.lib.sangam_sched_query(self.s, int(what)))

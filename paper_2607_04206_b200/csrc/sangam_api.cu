@@ -14,6 +14,7 @@
 #include "attn_tc.cuh"
 #include "common.cuh"
 #include "kv_write.cuh"
+#include "sched.cuh"
 
 constexpr int MAP_CACHE = 64;
 struct MapCacheKV { const void *k, *v; uint64_t tick; CUtensorMap mk, mv; };
@@ -301,7 +302,7 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
         use_dec = true;
     }
     if (use_dec) {
-        DecParams d;
+        DecParams d = {};
         d.block_table = block_table; d.cu_q_lens = cu_q_lens; d.ctx_lens = ctx_lens;
         d.out = (__nv_bfloat16*)out;
         d.batch = batch; d.total_q = total_q;
@@ -317,7 +318,8 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
 #ifdef SANGAM_TUNING_ENV
         if (const char* e_ = getenv("SANGAM_DEC_OV")) d.ov = atoi(e_);
         if (const char* e_ = getenv("SANGAM_DEC_MINW")) d.min_w = atoi(e_);
-#endif d.flags = ctx->d_flags;
+#endif
+        d.flags = ctx->d_flags;
         cudaError_t e = dec_launch(d, kv->mk, kv->mv, qm->dec, c.head_dim, ctx->dec_occ * ctx->sm_count, (cudaStream_t)stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "block_attn launch (decode kernel)");
         ctx->launches += 1;

@@ -97,15 +97,15 @@ def test_decreasing_cu_q_lens_is_an_empty_request(oracle, path):
     db = DeviceBatch(b)
     db.eng.set_dispatch({"prefill_kernel": 1, "decode_kernel": 2}[path])
     db.load_cache(); db.write_new()
-    cu = b.cu_q_lens.copy(); cu[2] = cu[1] - 3              # request 1 "ends before it starts"
+    cu = b.cu_q_lens.copy(); cu[3] = cu[2] - 3              # the last request "ends before it starts"
     db.cu_q_lens = t_i32(cu)
     db.out.fill_(float("nan"))
     db.attend()
     torch.cuda.synchronize()
     assert db.eng.device_status() == 0
     got = si.bf16_bits_to_f64(bits_of(db.out))
-    assert np.all(np.isfinite(got[:b.cu_q_lens[1]]))        # request 0 is computed
-    assert np.all(np.isnan(got[b.cu_q_lens[1]:b.cu_q_lens[1] + 3]))   # rows of the malformed request stay untouched
+    assert np.all(np.isfinite(got[:b.cu_q_lens[2]]))        # requests 0 and 1 are computed
+    assert np.all(np.isnan(got[b.cu_q_lens[2]:]))           # the malformed request's rows stay untouched
 
 
 def test_out_of_range_slot_is_skipped_and_flagged(oracle):
