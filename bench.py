@@ -8,8 +8,14 @@ Headline workload (N = 1): BASELINE.json configs[1], the LLaDA-8B-like block dec
 rotate over several independent per-layer pool sets so that consecutive replays never find
 their K/V in L2 (cold-L2 rule).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5] [--all-configs]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5 | <variant name>] [--all-configs]
   python bench.py --impl reference ...      # times the fp64 CPU oracle on a bounded sample
+
+Besides the headline line it reports, under `all_configs`, every BASELINE.json config (min / median / max over
+repetitions, roofline fraction, the oracle timed on the host cores), under `variants` and `fig3_sweep` the shapes of
+SURVEY.md 8(f) rank 4 (dKV-Cache-PD refresh, the paper's real response regions, the Fig.-3-shaped batch sweep) and under
+`sched_series` the batches Algorithm 1 produces from a simulated arrival trace for tau in {512, 1024, 2048, 16384}
+(PAPER.md:327), run through the real kernels.
 
 Multi-GPU: the path does not shard ("replicas only"): under torchrun every rank runs
 the same workload on its own GPU, time = max over ranks, value = sum of work / that time.
@@ -38,6 +44,31 @@ WORKLOAD_NAMES = {1: "config1_tiny", 2: "config2_llada_block_decode", 3: "config
                   4: "config4_kv_refresh_prefill", 5: "config5_hybrid_mixed"}
 NSETS = {1: 8, 2: 10, 3: 6, 4: 1, 5: 1}        # independent pool sets rotated per step (>= 8x L2 of distinct data)
 BOUND = {1: "hbm", 2: "hbm", 3: "hbm", 4: "tensor", 5: "tensor"}
+L2_BYTES = 126e6
+
+
+def make_workload_batch(key):
+    """BASELINE.json config number or a variant name of sangam_inputs.VARIANTS."""
+    if isinstance(key, int) or str(key).isdigit():
+        return si.CONFIGS[int(key)](), WORKLOAD_NAMES[int(key)], NSETS[int(key)]
+    b = si.VARIANTS[key]()
+    return b, key, nsets_for(b)
+
+
+def nsets_for(b):
+    """Pool sets to rotate so that consecutive steps touch >= 8x L2 of distinct K/V (one set when a step alone exceeds L2)."""
+    by = b.attn_bytes()
+    return 1 if by > 2 * L2_BYTES else int(min(12, max(2, np.ceil(8 * L2_BYTES / by))))
+
+
+def sources_hash():
+    """sha256 over the CUDA sources: profiles/traffic.json records the hash of the build its ncu numbers came from."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2607_04206_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
 
 
 def load_peaks():
@@ -131,9 +162,12 @@ class Workload:
         import torch
         import paper_2607_04206_b200 as sg
         self.b, self.nsets, self.device = b, nsets, device
+        dev_index = torch.cuda.current_device()             # under torchrun: LOCAL_RANK's GPU (set in dist_setup)
         self.eng = sg.Sangam(num_q_heads=b.num_q_heads, num_kv_heads=b.num_kv_heads, head_dim=b.head_dim,
                              num_pages=b.num_pages, max_batch=b.batch, max_total_q=max(b.total_q, len(b.slot_new), 1),
-                             max_pages_per_req=b.max_pages_per_req)
+                             max_pages_per_req=b.max_pages_per_req, device=dev_index)
+        device = f"cuda:{dev_index}"
+        self.device = device
         self.block_table, self.cu_q_lens, self.ctx_lens = _i32(b.block_table, device), _i32(b.cu_q_lens, device), _i32(b.ctx_lens, device)
         self.slot_new = _i32(b.slot_new, device)
         k_cache, v_cache, slot_cache = _bf16(b.k_cache, device), _bf16(b.v_cache, device), _i32(b.slot_cache, device)
@@ -197,47 +231,63 @@ def roofline_time_us(b: si.Batch, peaks, which="attn"):
     return max(f, by), f, by
 
 
-def measure_config(cfg: int, steps: int, warmup: int, peaks, reps: int = 3):
-    """All figures of one config: iteration / attention / kv_write time, TFLOP/s, GB/s, roofline fraction."""
-    b = si.CONFIGS[cfg]()
-    w = Workload(b, NSETS[cfg])
+def measure_batch(b: si.Batch, name: str, nsets: int, steps: int, warmup: int, peaks, reps: int = 3, parts=("iteration", "attn", "kv_write")):
+    """All figures of one workload: iteration / attention / kv_write time (median, min, max over `reps` repetitions of `steps`
+    replays, clocks sampled during the repetitions), TFLOP/s, GB/s and the fraction of the shape's own roofline
+    (the slower of flops at the bf16 peak and algorithmic bytes at the HBM peak)."""
+    w = Workload(b, nsets)
     w.capture()
-    res = {"workload": WORKLOAD_NAMES[cfg], "pool_sets": w.nsets}
-    for key, graphs in (("iteration", w.iter_graphs), ("attn", w.attn_graphs), ("kv_write", w.write_graphs)):
-        per = [w.time_graphs(graphs, steps, warmup) / steps * 1e3 for _ in range(reps)]   # us per step
-        res[key + "_us"] = round(statistics.median(per), 3)
-        res[key + "_us_min"] = round(min(per), 3)
+    res = {"workload": name, "pool_sets": w.nsets, "steps": steps, "reps": reps}
+    graphs = {"iteration": w.iter_graphs, "attn": w.attn_graphs, "kv_write": w.write_graphs}
+    import torch
+    with ClockSampler(index=torch.cuda.current_device()) as cs:
+        for key in parts:
+            per = [w.time_graphs(graphs[key], steps, warmup) / steps * 1e3 for _ in range(reps)]   # us per step
+            res[key + "_us"] = round(statistics.median(per), 3)
+            res[key + "_us_min"] = round(min(per), 3)
+            res[key + "_us_max"] = round(max(per), 3)
+    res["clocks"] = cs.summary()
     t_roof, t_f, t_b = roofline_time_us(b, peaks)
     a = res["attn_us"]
     res.update({"flops": b.flops(), "attn_bytes": b.attn_bytes(), "write_bytes": b.write_bytes(),
                 "attn_tflops": round(b.flops() / a / 1e6, 2), "attn_gbs": round(b.attn_bytes() / a / 1e3, 1),
-                "kv_write_gbs": round(b.write_bytes() / max(res["kv_write_us"], 1e-9) / 1e3, 1),
-                "bound": BOUND[cfg], "t_roof_us": round(t_roof, 2), "roofline_frac": round(t_roof / a, 4),
+                "bound": "tensor" if t_f > t_b else "hbm", "t_roof_us": round(t_roof, 2), "roofline_frac": round(t_roof / a, 4),
+                "roofline_frac_best": round(t_roof / res["attn_us_min"], 4),
                 "device_flags": int(w.eng.device_status())})
+    if "kv_write" in parts:
+        res["kv_write_gbs"] = round(b.write_bytes() / max(res["kv_write_us"], 1e-9) / 1e3, 1)
     return res, w
+
+
+def measure_config(cfg: int, steps: int, warmup: int, peaks, reps: int = 3):
+    return measure_batch(si.CONFIGS[cfg](), WORKLOAD_NAMES[cfg], NSETS[cfg], steps, warmup, peaks, reps)
 
 
 # ------------------------------------------------------------------------------------------------
 # end to end through the C ABI with HOST buffers (sangam_iteration_host)
 # ------------------------------------------------------------------------------------------------
 def measure_e2e(w: Workload, steps: int, warmup: int):
+    """sangam_iteration_packed: per step ONE host-to-device copy of the packed pinned buffer (q, k, v and all metadata),
+    kv_write + block_attn, one device-to-host copy of `out`, stream synchronize."""
     import torch
     b = w.b
-
-    def pin(a, view_bf16=False):
-        t = torch.from_numpy(np.ascontiguousarray(a).view(np.int16) if view_bf16 else np.ascontiguousarray(a)).pin_memory()
-        return t.view(torch.bfloat16) if view_bf16 else t
-
-    q, kn, vn = pin(b.q, True), pin(b.k_new, True), pin(b.v_new, True)
-    slot, bt, cu, cl = pin(b.slot_new.astype(np.int32)), pin(b.block_table.astype(np.int32)), pin(b.cu_q_lens.astype(np.int32)), pin(b.ctx_lens.astype(np.int32))
-    out = torch.empty_like(q).pin_memory()
-    h2d = sum(int(t.numel()) * t.element_size() for t in (q, kn, vn, slot, bt, cu, cl))
+    nt = int(b.slot_new.shape[0])
+    off = w.eng.packed_layout(b.batch, b.total_q, nt)
+    packed = torch.zeros(off[7], dtype=torch.uint8).pin_memory()
+    pn = packed.numpy()
+    parts = [np.ascontiguousarray(b.q), np.ascontiguousarray(b.k_new), np.ascontiguousarray(b.v_new), b.slot_new.astype(np.int32),
+             b.block_table.astype(np.int32), b.cu_q_lens.astype(np.int32), b.ctx_lens.astype(np.int32)]
+    for o, a in zip(off, parts):
+        raw = a.reshape(-1).view(np.uint8)
+        pn[o:o + raw.size] = raw
+    out = torch.empty((b.total_q, b.num_q_heads, b.head_dim), dtype=torch.bfloat16).pin_memory()
+    h2d = int(off[7])
     d2h = int(out.numel()) * out.element_size()
     n = len(w.sets)
 
     def step(i):
         s = w.sets[i % n]
-        w.eng.iteration_host(q, kn, vn, slot, s["kp"], s["vp"], bt, cu, cl, float(b.scale), out, stream=w.stream)
+        w.eng.iteration_packed(packed, nt, s["kp"], s["vp"], b.batch, b.total_q, float(b.scale), out, stream=w.stream)
 
     for i in range(warmup):
         step(i)
@@ -247,7 +297,18 @@ def measure_e2e(w: Workload, steps: int, warmup: int):
         step(i)                         # each call ends with a stream synchronize (D2H of `out` complete)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
-    return dt / steps, h2d, d2h
+    # the copies alone (same buffers, same stream, one synchronize per step): the rest of a step is the kernels
+    dev = torch.empty(off[7], dtype=torch.uint8, device=w.device)
+    dout = torch.empty_like(out, device=w.device)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    with torch.cuda.stream(w.stream):
+        for i in range(steps):
+            dev.copy_(packed, non_blocking=True)
+            out.copy_(dout, non_blocking=True)
+            w.stream.synchronize()
+    dc = time.perf_counter() - t1
+    return dt / steps, h2d, d2h, dc / steps
 
 
 # ------------------------------------------------------------------------------------------------
@@ -298,12 +359,33 @@ def cpu_baseline(b: si.Batch, target_s: float = 15.0):
             "seconds": round(dt, 3), "sample_flops": f}
 
 
+def cpu_baseline_config(cfg: int, b: si.Batch):
+    """SURVEY.md 8(d) / BASELINE.md section 4: the oracle over the WHOLE config for configs 1-3; for the prefill-sized configs a
+    stratified row sample (tile-edge + seeded random rows, all heads) with the full-config time extrapolated by the exact
+    work ratio sum q_r c_r (all) / sum q_r c_r (evaluated), labelled "extrapolated"."""
+    if cfg in (1, 2, 3):
+        oracle, kp, vp, _ = oracle_sample(b, 1)
+        rows = np.arange(b.total_q, dtype=np.int32)
+        label = "full"
+    else:
+        oracle, kp, vp, rows = oracle_sample(b, 8 if cfg == 4 else 32)     # config 5: its 32-row decodes in full + 32 rows per prefill
+        label = "extrapolated"
+    t0 = time.perf_counter()
+    oracle_step(oracle, b, kp, vp, rows)
+    dt = time.perf_counter() - t0
+    f = sample_flops(b, rows)
+    full_s = dt * b.flops() / max(f, 1.0)
+    return {"value": round(f / dt / 1e12, 6), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{len(rows)} of {b.total_q} query rows, all heads, full contexts + the kv_write, 1 pass, fp64 C -O2 -fopenmp",
+            "seconds": round(dt, 3), "full_config_seconds": round(full_s, 3), "full_config": label}
+
+
 def run_reference(args):
     """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    cfg = args.workload
+    cfg = int(args.workload)
     b = si.CONFIGS[cfg]()
     oracle, kp, vp, rows = oracle_sample(b, 2)
     for _ in range(min(args.warmup, 3)):
@@ -362,7 +444,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20000)
     ap.add_argument("--warmup", type=int, default=200)
-    ap.add_argument("--workload", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--workload", default="2", help="BASELINE.json config 1..5 or a variant name (sangam_inputs.VARIANTS)")
+    ap.add_argument("--no-extras", action="store_true", help="skip variants, the Fig.-3 sweep and the scheduler series")
     ap.add_argument("--impl", default="sangam", choices=["sangam", "reference"])
     ap.add_argument("--all-configs", dest="all_configs", action="store_true", default=None)
     ap.add_argument("--no-all-configs", dest="all_configs", action="store_false")
@@ -376,12 +459,11 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (the sangam kernels have no CPU fallback)")
     peaks = load_peaks()
-    cfg = args.workload
     steps, warmup = max(1, args.steps), max(3, args.warmup)
-    b = si.CONFIGS[cfg]()
-    w = Workload(b, NSETS[cfg])
+    b, wname, nsets = make_workload_batch(args.workload)
+    cfg = int(args.workload) if str(args.workload).isdigit() else None
+    w = Workload(b, nsets)
     w.capture()
-    launches0 = w.eng.launch_count()
 
     # ---- timed region: K steps of the whole hot path, barrier + synchronize on both sides
     barrier(dist)
@@ -393,15 +475,22 @@ def main():
     ms_total = max_over_ranks(ms_total, dist)
     ms_step = ms_total / steps
     value = world * b.flops() / (ms_step * 1e-3) / 1e12
-    kernels_per_step = 3                      # kv_write, attention (device-side plan inside), split-KV combine (captured; replayed K times)
+    # kernels captured in one step's graph: kv_write + the attention kernel(s) the dispatch chose (decode kernel: 1, fused
+    # merge; two-stream kernel: attention + combine).  Counted from the library's launch counter over one eager iteration.
+    n0 = w.eng.launch_count()
+    w.run_iteration(w.sets[0], w.stream)
+    torch.cuda.synchronize()
+    kernels_per_step = w.eng.launch_count() - n0
     gpu_launches = steps * kernels_per_step
 
     # ---- dominant kernel (attention), timed alone, L2-cold
     attn_ms = w.time_graphs(w.attn_graphs, steps, warmup) / steps
     attn_ms = max_over_ranks(attn_ms, dist)
     write_ms = w.time_graphs(w.write_graphs, steps, warmup) / steps
-    traffic = load_traffic().get(WORLD_KEY(cfg))
-    if BOUND[cfg] == "hbm":
+    tj = load_traffic()
+    traffic = tj.get("workloads", tj).get(wname)
+    t_roof, t_f, t_b = roofline_time_us(b, peaks)
+    if t_b >= t_f:
         ach = b.attn_bytes() / (attn_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "achieved": round(ach, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "frac": round(ach / peaks["hbm_gbs"], 4)}
@@ -409,32 +498,35 @@ def main():
         ach = b.flops() / (attn_ms * 1e-3) / 1e12
         roof = {"bound": "tensor", "achieved": round(ach, 1), "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                 "frac": round(ach / peaks["bf16_tflops"], 4)}
-    roof.update({"traffic": traffic, "kernel": "tc::attn_kernel (device-side plan inside) + tc::combine_kernel, timed alone over the same rotation",
+    kernel_name = ("dec::decode_kernel (device-side plan, swapped-operand attention, fused split-KV merge)" if kernels_per_step == 2
+                   else "tc::attn_kernel (device-side plan inside) + tc::combine_kernel")
+    roof.update({"traffic": traffic, "traffic_sources_hash": tj.get("sources_hash"), "traffic_matches_this_build": tj.get("sources_hash") == sources_hash(),
+                 "kernel": kernel_name + ", timed alone over the same rotation",
                  "kernel_us": round(attn_ms * 1e3, 3), "peak_source": peaks["source"] + " (burst)",
                  "algorithmic_bytes": b.attn_bytes(), "algorithmic_flops": b.flops()})
 
     # ---- end to end from host buffers
     e2e_steps = max(10, min(steps, 300))
-    e2e_s, h2d, d2h = measure_e2e(w, e2e_steps, 5)
+    e2e_s, h2d, d2h, copies_s = measure_e2e(w, e2e_steps, 5)
     e2e_s = max_over_ranks(e2e_s, dist)
     e2e = {"value": round(world * b.flops() / e2e_s / 1e12, 4), "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": round(e2e_s * 1e3, 4), "steps": e2e_steps,
-           "api": "sangam_iteration_host (pinned host buffers, H2D + kv_write + block_attn + D2H per step)"}
+           "split_us": {"copies_and_sync_alone": round(copies_s * 1e6, 1), "kernels_graph_replay": round(ms_step * 1e3, 1)},
+           "api": "sangam_iteration_packed (one pinned packed host buffer: 1 H2D copy + kv_write + block_attn + 1 D2H copy + stream sync per step)"}
 
     line = {"metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
             "ms_per_step": round(ms_step, 6), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16", "data": "synthetic",
-            "config": {"workload": WORKLOAD_NAMES[cfg], "batch": b.batch, "total_q": b.total_q,
+            "config": {"workload": wname, "batch": b.batch, "total_q": b.total_q,
                        "sum_ctx": int(b.ctx_lens.sum()), "heads": f"{b.num_q_heads}/{b.num_kv_heads}",
                        "head_dim": b.head_dim, "page": si.PAGE, "parallelism": f"replicas x{world}",
                        "l2": f"cold: steps rotate over {w.nsets} independent pool sets "
                              f"({w.nsets * b.attn_bytes() / 1e6:.0f} MB distinct per rotation)",
-                       "step": "CUDA-graph replay of kv_write + block_attn (plan + tcgen05 attention + split-KV combine)"},
+                       "step": "CUDA-graph replay of kv_write + block_attn (device-side plan + tcgen05 attention + split-KV merge)"},
             "us_per_iteration": round(ms_step * 1e3, 3), "attn_us": round(attn_ms * 1e3, 3),
             "kv_write_us": round(write_ms * 1e3, 3),
-            "clocks": cs.summary(), "e2e": e2e, "gpu_launches": gpu_launches,
-            "launch_count_check": w.eng.launch_count() - launches0, "device_flags": int(w.eng.device_status()),
-            "roofline": roof}
+            "clocks": cs.summary(), "e2e": e2e, "gpu_launches": gpu_launches, "kernels_per_step": kernels_per_step,
+            "device_flags": int(w.eng.device_status()), "roofline": roof}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(b)
@@ -444,12 +536,18 @@ def main():
         torch.cuda.empty_cache()
         allc = []
         for c in (1, 2, 3, 4, 5):
-            st = {1: 2000, 2: 2000, 3: 1000, 4: 20, 5: 40}[c]
-            r, ww = measure_config(c, st, max(3, st // 10), peaks)
+            st, reps = {1: (2000, 5), 2: (2000, 5), 3: (1000, 5), 4: (20, 10), 5: (30, 10)}[c]
+            r, ww = measure_config(c, st, max(3, st // 10), peaks, reps)
+            if not args.no_cpu_baseline:
+                r["cpu_baseline"] = cpu_baseline_config(c, ww.b)
             allc.append(r)
             del ww
             torch.cuda.empty_cache()
         line["all_configs"] = allc
+        if not args.no_extras:
+            line["variants"] = measure_variants(peaks)
+            line["fig3_sweep"] = measure_fig3(peaks)
+            line["sched_series"] = measure_sched_series()
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:
@@ -457,8 +555,117 @@ def main():
     return 0
 
 
-def WORLD_KEY(cfg):
-    return WORKLOAD_NAMES[cfg]
+# ------------------------------------------------------------------------------------------------
+# variant shapes and the Fig.-3-shaped batch sweep (attention only)
+# ------------------------------------------------------------------------------------------------
+def measure_variants(peaks):
+    import torch
+    out = []
+    for name in si.VARIANTS:
+        b = si.VARIANTS[name]()
+        st = 300 if b.flops() < 5e10 else 30
+        r, w = measure_batch(b, name, nsets_for(b), st, max(3, st // 10), peaks, reps=3, parts=("iteration", "attn"))
+        out.append(r)
+        del w
+        torch.cuda.empty_cache()
+    return out
+
+
+def measure_fig3(peaks):
+    """Batch in {1 .. 64} block decodes at sequence length 1024, both head geometries: attention-only us and
+    the fraction of the HBM roofline."""
+    import torch
+    out = []
+    for model in ("llada", "dream"):
+        for nb in si.FIG3_BATCHES:
+            b = si.fig3_point(model, nb)
+            r, w = measure_batch(b, b.name, nsets_for(b), 500, 50, peaks, reps=3, parts=("attn",))
+            out.append({k: r[k] for k in ("workload", "pool_sets", "attn_us", "attn_us_min", "attn_gbs", "attn_tflops", "bound", "t_roof_us", "roofline_frac", "device_flags")})
+            del w
+            torch.cuda.empty_cache()
+    return out
+
+
+# ------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f) rank 1: Algorithm 1's batches from a simulated arrival trace, through the real kernels
+# ------------------------------------------------------------------------------------------------
+def measure_sched_series(taus=(512, 1024, 2048, 16384), iters=250, qps=6.0, n_req=96, iter_time=0.04):
+    """LLaDA-8B-like geometry, ShareGPT-like arrivals (Table-1 statistics, +1024 MASK).  The arrival clock advances by a fixed
+    nominal model-iteration time so that the batch sequence is deterministic; every produced microbatch runs
+    kv_write + block_attn on one persistent pool (metadata copied from the scheduler's pinned arrays) and is timed with
+    CUDA events."""
+    import torch
+    import paper_2607_04206_b200 as sg
+    geo = si.GEOMETRY["llada"]
+    Hq, Hkv, D = geo["num_q_heads"], geo["num_kv_heads"], geo["head_dim"]
+    P, MB, W = 24576, 64, (4096 + 15) // 16
+    out = []
+    for tau in taus:
+        MQ = tau + 4096 + 2048 + MB * 32
+        tr = si.sched_trace(21, n_req, qps, "sharegpt_like")
+        sch = sg.Scheduler(tau=tau, num_pages=P, max_batch=MB, max_total_q=MQ, max_pages_per_req=W, pinned=True)
+        eng = sg.Sangam(num_q_heads=Hq, num_kv_heads=Hkv, head_dim=D, num_pages=P, max_batch=MB, max_total_q=MQ,
+                        max_pages_per_req=W, device=torch.cuda.current_device())
+        g = torch.Generator(device="cuda"); g.manual_seed(5)
+        kp = torch.randn(P, Hkv, 16, D, dtype=torch.bfloat16, device="cuda", generator=g)
+        vp = torch.randn(P, Hkv, 16, D, dtype=torch.bfloat16, device="cuda", generator=g)
+        q = torch.randn(MQ, Hq, D, dtype=torch.bfloat16, device="cuda", generator=g)
+        kn = torch.randn(MQ, Hkv, D, dtype=torch.bfloat16, device="cuda", generator=g)
+        vn = torch.randn(MQ, Hkv, D, dtype=torch.bfloat16, device="cuda", generator=g)
+        o = torch.empty_like(q)
+        d_cu = torch.zeros(MB + 1, dtype=torch.int32, device="cuda"); d_cl = torch.zeros(MB, dtype=torch.int32, device="cuda")
+        d_bt = torch.zeros(MB, W, dtype=torch.int32, device="cuda"); d_sm = torch.zeros(MQ, dtype=torch.int32, device="cuda")
+        stream = torch.cuda.Stream()
+        steps_left, nxt, gpu_us, host_us, toks, pre_toks, ndec, hybrid = {}, 0, [], [], [], [], [], 0
+        scale = float(1.0 / np.sqrt(D))
+        for it in range(iters):
+            now = it * iter_time
+            t0 = time.perf_counter()
+            while nxt < n_req and tr["arrival"][nxt] <= now:
+                sch.submit(nxt, float(tr["arrival"][nxt]), int(tr["prompt_len"][nxt]), int(tr["response_len"][nxt]), int(tr["output_len"][nxt]))
+                nxt += 1
+            bb = sch.next()
+            t_host = time.perf_counter() - t0
+            R, nd, tq = bb.batch, bb.num_decodes, bb.total_q
+            ids = sch.arrays["req_ids"][:R].copy()
+            if R > 0:
+                with torch.cuda.stream(stream):
+                    d_cu[:R + 1].copy_(sch.tensors["cu_q_lens"][:R + 1], non_blocking=True)
+                    d_cl[:R].copy_(sch.tensors["ctx_lens"][:R], non_blocking=True)
+                    d_bt[:R].copy_(sch.tensors["block_table"][:R], non_blocking=True)
+                    d_sm[:tq].copy_(sch.tensors["slot_mapping"][:tq], non_blocking=True)
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(stream)
+                    eng.kv_write(kn[:tq], vn[:tq], d_sm[:tq], kp, vp, stream=stream)
+                    eng.block_attn(q[:tq], kp, vp, d_bt[:R], d_cu[:R + 1], d_cl[:R], scale, o[:tq], stream=stream)
+                    e1.record(stream)
+                    e1.synchronize()
+                gpu_us.append(e0.elapsed_time(e1) * 1e3)
+                toks.append(tq); pre_toks.append(tq - 32 * nd); ndec.append(nd); hybrid += int(nd > 0 and R > nd)
+            done = []
+            for rid in ids[:nd]:
+                # decodes keep their block index in the scheduler; the trace's step counts are consumed in order per request
+                key = int(rid)
+                cnt = steps_left.setdefault(key, [0, 0])           # [block index, steps taken in it]
+                cnt[1] += 1
+                fin = cnt[1] >= int(tr["steps"][key, cnt[0]])
+                if fin:
+                    cnt[0] += 1; cnt[1] = 0
+                done.append(1 if fin else 0)
+            t1 = time.perf_counter()
+            sch.complete(done)
+            host_us.append((t_host + time.perf_counter() - t1) * 1e6)
+        a = np.asarray(gpu_us)
+        out.append({"tau": tau, "iterations": iters, "iterations_with_work": int(len(a)), "requests_submitted": nxt, "qps": qps,
+                    "gpu_us_mean": round(float(a.mean()), 1), "gpu_us_p50": round(float(np.percentile(a, 50)), 1),
+                    "gpu_us_p99": round(float(np.percentile(a, 99)), 1), "gpu_us_max": round(float(a.max()), 1),
+                    "tokens_per_iteration_mean": round(float(np.mean(toks)), 1), "prefill_tokens_per_iteration_mean": round(float(np.mean(pre_toks)), 1),
+                    "prefill_tokens_per_iteration_max": int(np.max(pre_toks)), "decodes_per_iteration_mean": round(float(np.mean(ndec)), 2),
+                    "hybrid_iterations": hybrid, "scheduler_host_us_mean": round(float(np.mean(host_us)), 2),
+                    "device_flags": int(eng.device_status()), "waiting_at_end": sch.query(1), "in_flight_at_end": sch.query(2)})
+        del kp, vp, q, kn, vn, o, eng, sch
+        torch.cuda.empty_cache()
+    return out
 
 
 if __name__ == "__main__":

@@ -152,6 +152,16 @@ int sangam_iteration_host(sangam_ctx* ctx, const void* q_host, const void* k_hos
                           const int32_t* ctx_lens_host, int32_t batch, int32_t total_q,
                           float scale, void* out_host, void* stream);
 
+/*
+ * The same iteration from ONE packed host buffer: q | k | v | slot_mapping | block_table | cu_q_lens | ctx_lens, each part
+ * on a 256-byte boundary at the offsets sangam_packed_layout returns (offsets8[0..6]; offsets8[7] = total bytes).  One
+ * host-to-device copy of the whole buffer, both kernels, one device-to-host copy of `out`, stream synchronize.  Pin the
+ * buffers for full copy speed.  The ctx-owned device staging is allocated on the first call.
+ */
+int sangam_packed_layout(const sangam_ctx* ctx, int32_t batch, int32_t total_q, int32_t num_tokens, int64_t* offsets8);
+int sangam_iteration_packed(sangam_ctx* ctx, const void* packed_host, int32_t num_tokens, void* k_pages, void* v_pages,
+                            int32_t batch, int32_t total_q, float scale, void* out_host, void* stream);
+
 /* Reads and clears nothing: returns the sticky device flag word (synchronises the ctx's device). */
 int sangam_device_status(sangam_ctx* ctx, uint32_t* flags);
 int sangam_clear_device_status(sangam_ctx* ctx);

@@ -13,7 +13,7 @@ DECLARED_SYMBOLS = [
     "sangam_iteration_host", "sangam_device_status", "sangam_clear_device_status", "sangam_launch_count",
     "sangam_last_error", "sangam_version", "sangam_set_dispatch", "sangam_query",
     "sangam_sched_create", "sangam_sched_destroy", "sangam_sched_submit", "sangam_sched_next", "sangam_sched_complete",
-    "sangam_sched_query",
+    "sangam_sched_query", "sangam_packed_layout", "sangam_iteration_packed",
 ]
 
 DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE = 0, 1, 2
@@ -72,6 +72,8 @@ def load_library(build_if_missing: bool = False):
     lib.sangam_set_dispatch.argtypes = [vp, i32]
     lib.sangam_query.argtypes = [vp, i32]
     lib.sangam_query.restype = i32
+    lib.sangam_packed_layout.argtypes = [vp, i32, i32, i32, ctypes.POINTER(ctypes.c_int64)]
+    lib.sangam_iteration_packed.argtypes = [vp, vp, i32, vp, vp, i32, i32, f32, vp, vp]
     lib.sangam_sched_create.argtypes = [ctypes.POINTER(_SchedConfig), ctypes.POINTER(vp)]
     lib.sangam_sched_destroy.argtypes = [vp]
     lib.sangam_sched_submit.argtypes = [vp, ctypes.c_int64, ctypes.c_double, i32, i32, i32]
@@ -145,6 +147,17 @@ class Sangam:
             self.ctx, _ptr(q), _ptr(k), _ptr(v), _ptr(slot_mapping), int(slot_mapping.numel()), _ptr(k_pages),
             _ptr(v_pages), _ptr(block_table), _ptr(cu_q_lens), _ptr(ctx_lens), int(ctx_lens.numel()), int(q.shape[0]),
             float(scale), _ptr(out), _stream(stream)))
+
+    def packed_layout(self, batch, total_q, num_tokens):
+        """Byte offsets of q, k, v, slot_mapping, block_table, cu_q_lens, ctx_lens in the packed host buffer + total size."""
+        off = (ctypes.c_int64 * 8)()
+        self._check(self.lib.sangam_packed_layout(self.ctx, int(batch), int(total_q), int(num_tokens), off))
+        return list(off)
+
+    def iteration_packed(self, packed, num_tokens, k_pages, v_pages, batch, total_q, scale, out, stream=None):
+        """packed, out: HOST (pinned) tensors; one H2D copy, kv_write + block_attn, one D2H copy, stream synchronize."""
+        self._check(self.lib.sangam_iteration_packed(self.ctx, _ptr(packed), int(num_tokens), _ptr(k_pages), _ptr(v_pages), int(batch),
+                                                     int(total_q), float(scale), _ptr(out), _stream(stream)))
 
     def set_dispatch(self, mode: int):
         """DISPATCH_AUTO / DISPATCH_PREFILL / DISPATCH_DECODE: which attention kernel sangam_block_attn launches."""

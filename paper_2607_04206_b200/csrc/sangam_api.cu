@@ -44,6 +44,8 @@ struct sangam_ctx {
     uint64_t map_tick;
     // staging for sangam_iteration_host (allocated on first use)
     void *s_q, *s_k, *s_v, *s_out;
+    void* s_packed;               // staging of sangam_iteration_packed
+    int64_t s_packed_bytes;
     int32_t *s_slot, *s_bt, *s_cu, *s_ctx;
     int64_t launches;
     char err[512];
@@ -158,7 +160,7 @@ extern "C" int sangam_destroy(sangam_ctx* ctx) {
     DeviceGuard guard(ctx->cfg.device);
     cudaFree(ctx->d_dec_part_o); cudaFree(ctx->d_dec_part_ml); cudaFree(ctx->d_dec_cnt);
     cudaFree(ctx->d_flags); cudaFree(ctx->d_sched); cudaFree(ctx->d_part_o); cudaFree(ctx->d_part_ml); cudaFree(ctx->d_slot_meta); cudaFree(ctx->d_plan_cache);
-    cudaFree(ctx->s_q); cudaFree(ctx->s_k); cudaFree(ctx->s_v); cudaFree(ctx->s_out);
+    cudaFree(ctx->s_q); cudaFree(ctx->s_k); cudaFree(ctx->s_v); cudaFree(ctx->s_out); cudaFree(ctx->s_packed);
     cudaFree(ctx->s_slot); cudaFree(ctx->s_bt); cudaFree(ctx->s_cu); cudaFree(ctx->s_ctx);
     delete ctx;
     return SANGAM_OK;
@@ -355,6 +357,7 @@ extern "C" int sangam_set_dispatch(sangam_ctx* ctx, int32_t mode) {
 
 static int ensure_staging(sangam_ctx* ctx) {
     if (ctx->s_q) return SANGAM_OK;
+    if (ctx->s_out) { cudaFree(ctx->s_out); ctx->s_out = nullptr; }
     const sangam_config& c = ctx->cfg;
     const size_t qb = (size_t)c.max_total_q * c.num_q_heads * c.head_dim * 2;
     const size_t kb = (size_t)c.max_total_q * c.num_kv_heads * c.head_dim * 2;
@@ -404,17 +407,70 @@ extern "C" int sangam_iteration_host(sangam_ctx* ctx, const void* q_host, const 
     return SANGAM_OK;
 }
 
+
+// Layout of the packed host buffer of sangam_iteration_packed: q | k | v | slot_mapping | block_table | cu_q_lens | ctx_lens,
+// each part starting on a 256-byte boundary.  offsets[0..6] = byte offset of each part, offsets[7] = total bytes.
+static void packed_layout(const sangam_config& c, int32_t batch, int32_t total_q, int32_t num_tokens, int64_t offsets[8]) {
+    const int64_t sizes[7] = {(int64_t)total_q * c.num_q_heads * c.head_dim * 2, (int64_t)num_tokens * c.num_kv_heads * c.head_dim * 2,
+                              (int64_t)num_tokens * c.num_kv_heads * c.head_dim * 2, (int64_t)num_tokens * 4,
+                              (int64_t)batch * c.max_pages_per_req * 4, (int64_t)(batch + 1) * 4, (int64_t)batch * 4};
+    int64_t off = 0;
+    for (int i = 0; i < 7; ++i) { offsets[i] = off; off = (off + sizes[i] + 255) & ~(int64_t)255; }
+    offsets[7] = off;
+}
+
+extern "C" int sangam_packed_layout(const sangam_ctx* ctx, int32_t batch, int32_t total_q, int32_t num_tokens, int64_t* offsets8) {
+    if (!ctx || !offsets8 || batch < 0 || total_q < 0 || num_tokens < 0) return SANGAM_ERR_INVALID_ARG;
+    packed_layout(ctx->cfg, batch, total_q, num_tokens, offsets8);
+    return SANGAM_OK;
+}
+
+extern "C" int sangam_iteration_packed(sangam_ctx* ctx, const void* packed_host, int32_t num_tokens, void* k_pages, void* v_pages,
+                                       int32_t batch, int32_t total_q, float scale, void* out_host, void* stream) {
+    if (!ctx) return SANGAM_ERR_INVALID_ARG;
+    if (batch < 0 || total_q < 0 || num_tokens < 0) return fail(ctx, SANGAM_ERR_INVALID_ARG, "iteration_packed: negative count");
+    if (batch > ctx->cfg.max_batch || total_q > ctx->cfg.max_total_q || num_tokens > ctx->cfg.max_total_q)
+        return fail(ctx, SANGAM_ERR_WORKSPACE, "iteration_packed: batch / total_q / num_tokens above the ctx maxima");
+    if (!packed_host || !out_host || !k_pages || !v_pages) return fail(ctx, SANGAM_ERR_INVALID_ARG, "iteration_packed: null pointer");
+    ON_CTX_DEVICE(ctx);
+    int64_t off[8];
+    packed_layout(ctx->cfg, batch, total_q, num_tokens, off);
+    if (!ctx->s_packed || ctx->s_packed_bytes < off[7]) {        // grows to the largest request seen (first call: allocation)
+        int64_t cap[8];
+        packed_layout(ctx->cfg, ctx->cfg.max_batch, ctx->cfg.max_total_q, ctx->cfg.max_total_q, cap);
+        cudaFree(ctx->s_packed); ctx->s_packed = nullptr;
+        cudaFree(ctx->s_out); ctx->s_out = nullptr;
+        CK(cudaMalloc(&ctx->s_packed, (size_t)cap[7]));
+        ctx->s_packed_bytes = cap[7];
+        CK(cudaMalloc(&ctx->s_out, (size_t)ctx->cfg.max_total_q * ctx->cfg.num_q_heads * ctx->cfg.head_dim * 2));
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    char* d = static_cast<char*>(ctx->s_packed);
+    CK(cudaMemcpyAsync(d, packed_host, (size_t)off[7], cudaMemcpyHostToDevice, st));          // ONE host-to-device copy
+    int rc = sangam_kv_write(ctx, d + off[1], d + off[2], reinterpret_cast<const int32_t*>(d + off[3]), num_tokens, k_pages, v_pages, stream);
+    if (rc != SANGAM_OK) return rc;
+    rc = sangam_block_attn(ctx, d + off[0], k_pages, v_pages, reinterpret_cast<const int32_t*>(d + off[4]),
+                           reinterpret_cast<const int32_t*>(d + off[5]), reinterpret_cast<const int32_t*>(d + off[6]), batch, total_q, scale,
+                           ctx->s_out, stream);
+    if (rc != SANGAM_OK) return rc;
+    CK(cudaMemcpyAsync(out_host, ctx->s_out, (size_t)total_q * ctx->cfg.num_q_heads * ctx->cfg.head_dim * 2, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return SANGAM_OK;
+}
+
 #ifdef SANGAM_DEBUG_ITEM
 extern "C" int sangam_debug_bad_item(int* out16) {
     cudaDeviceSynchronize();
     return cudaMemcpyFromSymbol(out16, g_bad_item, 64) == cudaSuccess ? 0 : -4;
 }
 #endif
-// internal diagnostic (not part of include/sangam.h): which barrier the first watchdog timeout hit
+#ifdef SANGAM_WAIT_TABLE
+// debug builds only (not part of include/sangam.h): which barrier the first watchdog timeout hit
 extern "C" int sangam_debug_timeout_info(unsigned int* out20) {
     cudaDeviceSynchronize();
     return cudaMemcpyFromSymbol(out20, ptx::g_timeout_info, 80) == cudaSuccess ? 0 : -4;
 }
+#endif
 
 #ifdef SANGAM_TRACE
 extern "C" int sangam_trace_cta_times(unsigned long long* host_buf) {

@@ -219,7 +219,7 @@ CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
 
 
 def custom(seed: int, q_lens, ctx_lens, *, num_q_heads=4, num_kv_heads=4, head_dim=64, pool_slack=1.25,
-           min_width: int = 0) -> Batch:
+           min_width: int = 0, new_at_end: bool = False, name: str = "custom") -> Batch:
     """Arbitrary (q_r, c_r) pairs for edge-case tests.  Every request is laid out like a
     prefill whose first q_r rows are queried; K/V for all c_r positions are cache content
     and the 'new' rows rewrite the first min(q_r, c_r) positions."""
@@ -244,13 +244,16 @@ def custom(seed: int, q_lens, ctx_lens, *, num_q_heads=4, num_kv_heads=4, head_d
         slot_cache[cu_ctx[r]:cu_ctx[r + 1]] = block_table[r, j // PAGE].astype(np.int64) * PAGE + (j % PAGE)
     k_cache = _normal_bits(g, (int(ctx.sum()), num_kv_heads, head_dim))
     v_cache = _normal_bits(g, (int(ctx.sum()), num_kv_heads, head_dim))
-    new_slots = [slot_cache[cu_ctx[r]:cu_ctx[r] + min(int(q_lens[r]), int(ctx[r]))] for r in range(R)]
+    if new_at_end:   # the rewritten rows are the LAST min(q_r, c_r) positions (a response region at the end of the sequence)
+        new_slots = [slot_cache[cu_ctx[r + 1] - min(int(q_lens[r]), int(ctx[r])):cu_ctx[r + 1]] for r in range(R)]
+    else:
+        new_slots = [slot_cache[cu_ctx[r]:cu_ctx[r] + min(int(q_lens[r]), int(ctx[r]))] for r in range(R)]
     slot_new = np.concatenate(new_slots).astype(np.int32) if R else np.zeros(0, np.int32)
     k_new = _normal_bits(g, (len(slot_new), num_kv_heads, head_dim))
     v_new = _normal_bits(g, (len(slot_new), num_kv_heads, head_dim))
     q = _normal_bits(g, (int(q_lens.sum()), num_q_heads, head_dim))
     return Batch(
-        name="custom", num_q_heads=num_q_heads, num_kv_heads=num_kv_heads, head_dim=head_dim,
+        name=name, num_q_heads=num_q_heads, num_kv_heads=num_kv_heads, head_dim=head_dim,
         num_pages=P, max_pages_per_req=W, scale=np.float32(1.0 / np.sqrt(head_dim)),
         q_lens=q_lens.astype(np.int32), ctx_lens=ctx.astype(np.int32),
         cu_q_lens=np.concatenate([[0], np.cumsum(q_lens)]).astype(np.int32),
@@ -315,3 +318,49 @@ def sched_trace(seed: int, n: int, qps: float, kind: str = "sharegpt_like", bloc
     steps = g.integers(2, max_steps, (n, nblk), endpoint=True).astype(np.int32)
     return {"arrival": arrival, "prompt_len": prm, "response_len": np.full(n, resp, np.int32), "output_len": out,
             "steps": steps, "block": block, "kind": kind}
+
+
+# ---------------------------------------------------------------------------------------
+# Variant shapes: the same kernels at other points of the paper's workloads.
+# ---------------------------------------------------------------------------------------
+GEOMETRY = {"llada": dict(num_q_heads=32, num_kv_heads=32, head_dim=128),      # LLaDA-8B-like MHA
+            "dream": dict(num_q_heads=28, num_kv_heads=4, head_dim=128)}       # Dream-7B-like GQA 7:1
+
+
+def _trace_prompts(g: np.random.Generator, n: int, kind: str, shrink: int = 1):
+    pm, p99, _, _, resp = TRACE_STATS[kind]
+    prm = np.exp(np.log(pm) + np.log(p99 / pm) / 2.326 * g.standard_normal(n))
+    return np.clip(np.rint(prm), 16, 4096 - resp).astype(np.int64) // shrink, resp // shrink
+
+
+def paper_decode(model: str = "llada", trace: str = "sharegpt_like", batch: int = 16, seed: int = 11, shrink: int = 1) -> Batch:
+    """Block decode at the paper's real sequence lengths: prompts with the trace's Table-1 statistics
+    (<= 4096 tokens), 1024 (ShareGPT) / 512 (arXiv) appended MASK positions, block 32."""
+    def lens(g):
+        prm, resp = _trace_prompts(g, batch, trace, shrink)
+        return prm + resp, []
+    resp = TRACE_STATS[trace][4] // shrink
+    return make_batch(f"{model}_{trace}_decode", seed, decode_ctx=None, decode_q=32 // (1 if shrink == 1 else 1), response=resp,
+                      lengths_fn=lens, **GEOMETRY[model])
+
+
+def dkv_refresh(model: str = "llada", trace: str = "sharegpt_like", batch: int = 8, seed: int = 12, shrink: int = 1) -> Batch:
+    """dKV-Cache-PD style refresh: only the RESPONSE region is recomputed -- its rows are the queries and the
+    rewritten K/V rows -- while the prompt's K/V stay as cached; the context is still prompt + response."""
+    g = np.random.default_rng(seed)
+    prm, resp = _trace_prompts(g, batch, trace, shrink)
+    return custom(seed, [resp] * batch, (prm + resp).tolist(), new_at_end=True, name=f"{model}_{trace}_dkv_refresh", **GEOMETRY[model])
+
+
+def fig3_point(model: str, batch: int, seed: int = 13, ctx: int = 1024) -> Batch:
+    """One point of the Fig.-3-shaped sweep: `batch` block decodes at sequence length 1024, block 32."""
+    return make_batch(f"fig3_{model}_b{batch}", seed + batch, decode_ctx=[ctx] * batch, decode_q=32, response=256, **GEOMETRY[model])
+
+
+VARIANTS = {
+    "llada_sharegpt_decode": lambda shrink=1: paper_decode("llada", "sharegpt_like", 16, 11, shrink),
+    "dream_arxiv_decode": lambda shrink=1: paper_decode("dream", "arxiv_like", 16, 14, shrink),
+    "llada_dkv_refresh": lambda shrink=1: dkv_refresh("llada", "sharegpt_like", 8, 12, shrink),
+    "dream_dkv_refresh": lambda shrink=1: dkv_refresh("dream", "arxiv_like", 8, 15, shrink),
+}
+FIG3_BATCHES = (1, 2, 4, 8, 16, 32, 64)
