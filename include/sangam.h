@@ -72,6 +72,7 @@ typedef enum {
 #define SANGAM_DEV_BAD_PAGE   2u      /* block_attn: page id out of [0,num_pages): the page reads as K = V = 0 */
 #define SANGAM_DEV_CTX_TOO_LONG 4u    /* block_attn: ctx_len needs more than max_pages_per_req pages: rows are zeros */
 #define SANGAM_DEV_TIMEOUT    8u      /* an in-kernel barrier wait gave up (internal error) */
+#define SANGAM_DEV_BAD_POSITION 32u   /* kv_write_rope: position outside [0, max_pos), row skipped */
 #define SANGAM_DEV_INTERNAL  16u      /* an internal bounds guard tripped; the access was skipped (internal error) */
 
 typedef struct {
@@ -97,6 +98,30 @@ int sangam_destroy(sangam_ctx* ctx);
  */
 int sangam_kv_write(sangam_ctx* ctx, const void* k, const void* v, const int32_t* slot_mapping,
                     int32_t num_tokens, void* k_pages, void* v_pages, void* stream);
+
+/*
+ * KV write with rotary position embedding fused in (rotate K, then scatter; V is copied): the same contract as
+ * sangam_kv_write with  k_pages[s/16][h][s%16][:] = bf16( rope(k[i][h][:], positions[i]) ),  rotate-half convention
+ *   out[j] = x[j] cos(a_j) - x[j + D/2] sin(a_j),  out[j + D/2] = x[j + D/2] cos(a_j) + x[j] sin(a_j),  a_j = pos * base^(-2j/D),
+ * fp32 arithmetic, round to nearest even.  cos_sin is a device fp32 table [max_pos][head_dim]: row p holds cos(p * theta_j) for
+ * j < D/2 followed by sin(p * theta_j); the caller builds it once (any base / scaling).  positions: int32 [num_tokens], device.
+ * A position outside [0, max_pos) skips the row and raises SANGAM_DEV_BAD_POSITION.
+ */
+int sangam_kv_write_rope(sangam_ctx* ctx, const void* k, const void* v, const int32_t* slot_mapping, const int32_t* positions,
+                         const float* cos_sin, int32_t max_pos, int32_t num_tokens, void* k_pages, void* v_pages, void* stream);
+
+/*
+ * Confidence-threshold sampler over the rows the iteration decoded ("unmasks every masked position whose top-1 probability
+ * exceeds a threshold"; threshold 0.9).  logits: bf16 [num_rows][vocab] (device, 2-byte aligned
+ * rows); masked: int32 [num_rows], nonzero = still masked; cu_rows: int32 [num_requests + 1], rows of request r (its
+ * current block) are cu_rows[r] .. cu_rows[r+1]-1.  Outputs (device): token[t] = argmax_j logits[t][j] (lowest index on
+ * ties), conf[t] = softmax(logits[t])[token[t]] (fp32), unmask[t] = 1 for every masked row with conf > threshold; if no
+ * masked row of a request passes, its most confident masked row (lowest index on ties) is unmasked instead, so every
+ * step commits at least one position per request that still has masked rows.  Two kernels; no host sync.
+ */
+int sangam_confidence_sample(sangam_ctx* ctx, const void* logits, int32_t vocab, const int32_t* masked, const int32_t* cu_rows,
+                             int32_t num_requests, int32_t num_rows, float threshold, int32_t* token, float* conf,
+                             int32_t* unmask, void* stream);
 
 /*
  * Block attention (steps a3-a9): for request r < batch, row t in [cu_q_lens[r], cu_q_lens[r+1]),

@@ -4,5 +4,5 @@ Thin Python binding over the C ABI in include/sangam.h.  Argument marshalling on
 of the path runs in the CUDA kernels of csrc/.  There is no CPU fallback -- if libsangam.so is
 missing or a CUDA device is absent the calls raise.
 """
-from .binding import (SangamError, Sangam, Scheduler, load_library, exported_symbols, DECLARED_SYMBOLS,  # noqa: F401
+from .binding import (SangamError, Sangam, Scheduler, rope_table, load_library, exported_symbols, DECLARED_SYMBOLS,  # noqa: F401
                       DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE)

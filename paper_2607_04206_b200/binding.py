@@ -14,6 +14,7 @@ DECLARED_SYMBOLS = [
     "sangam_last_error", "sangam_version", "sangam_set_dispatch", "sangam_query",
     "sangam_sched_create", "sangam_sched_destroy", "sangam_sched_submit", "sangam_sched_next", "sangam_sched_complete",
     "sangam_sched_query", "sangam_packed_layout", "sangam_iteration_packed",
+    "sangam_kv_write_rope", "sangam_confidence_sample",
 ]
 
 DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE = 0, 1, 2
@@ -74,6 +75,8 @@ def load_library(build_if_missing: bool = False):
     lib.sangam_query.restype = i32
     lib.sangam_packed_layout.argtypes = [vp, i32, i32, i32, ctypes.POINTER(ctypes.c_int64)]
     lib.sangam_iteration_packed.argtypes = [vp, vp, i32, vp, vp, i32, i32, f32, vp, vp]
+    lib.sangam_kv_write_rope.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, vp, vp, vp]
+    lib.sangam_confidence_sample.argtypes = [vp, vp, i32, vp, vp, i32, i32, f32, vp, vp, vp, vp]
     lib.sangam_sched_create.argtypes = [ctypes.POINTER(_SchedConfig), ctypes.POINTER(vp)]
     lib.sangam_sched_destroy.argtypes = [vp]
     lib.sangam_sched_submit.argtypes = [vp, ctypes.c_int64, ctypes.c_double, i32, i32, i32]
@@ -98,6 +101,15 @@ def _stream(stream):
     import torch
     s = stream if stream is not None else torch.cuda.current_stream()
     return ctypes.c_void_p(s.cuda_stream)
+
+
+def rope_table(max_pos: int, head_dim: int, base: float = 10000.0):
+    """Host-side cos/sin cache for sangam_kv_write_rope: float32 numpy [max_pos][head_dim], row p = cos(p theta_j) for j < D/2
+    then sin(p theta_j), theta_j = base^(-2j/D), evaluated in float64 (what serving stacks cache once per model)."""
+    import numpy as np
+    j = np.arange(head_dim // 2, dtype=np.float64)
+    ang = np.arange(max_pos, dtype=np.float64)[:, None] * (float(base) ** (-2.0 * j / head_dim))[None, :]
+    return np.concatenate([np.cos(ang), np.sin(ang)], axis=1).astype(np.float32)
 
 
 class Sangam:
@@ -134,6 +146,17 @@ class Sangam:
     def kv_write(self, k, v, slot_mapping, k_pages, v_pages, stream=None):
         self._check(self.lib.sangam_kv_write(self.ctx, _ptr(k), _ptr(v), _ptr(slot_mapping), int(slot_mapping.numel()),
                                              _ptr(k_pages), _ptr(v_pages), _stream(stream)))
+
+    def kv_write_rope(self, k, v, slot_mapping, positions, cos_sin, k_pages, v_pages, stream=None):
+        """cos_sin: device fp32 [max_pos][head_dim] (see rope_table)."""
+        self._check(self.lib.sangam_kv_write_rope(self.ctx, _ptr(k), _ptr(v), _ptr(slot_mapping), _ptr(positions), _ptr(cos_sin),
+                                                  int(cos_sin.shape[0]), int(slot_mapping.numel()), _ptr(k_pages), _ptr(v_pages), _stream(stream)))
+
+    def confidence_sample(self, logits, masked, cu_rows, threshold, token, conf, unmask, stream=None):
+        """logits bf16 [rows][vocab]; masked int32 [rows]; cu_rows int32 [R+1]; outputs token int32, conf fp32, unmask int32."""
+        self._check(self.lib.sangam_confidence_sample(self.ctx, _ptr(logits), int(logits.shape[1]), _ptr(masked), _ptr(cu_rows),
+                                                      int(cu_rows.numel()) - 1, int(logits.shape[0]), float(threshold), _ptr(token),
+                                                      _ptr(conf), _ptr(unmask), _stream(stream)))
 
     def block_attn(self, q, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, scale, out, stream=None, simt=False):
         fn = self.lib.sangam_block_attn_simt if simt else self.lib.sangam_block_attn

@@ -12,6 +12,7 @@
 #define DEV_BAD_PAGE 2u
 #define DEV_CTX_TOO_LONG 4u
 #define DEV_TIMEOUT 8u
+#define DEV_BAD_POSITION 32u       // kv_write_rope: position outside the cos/sin table, row skipped
 #define DEV_INTERNAL 16u           // an internal bounds guard tripped (library bug; the access was skipped)
 
 struct AttnParams {

@@ -14,6 +14,7 @@
 #include "attn_tc.cuh"
 #include "common.cuh"
 #include "kv_write.cuh"
+#include "neighbours.cuh"
 #include "sched.cuh"
 
 constexpr int MAP_CACHE = 64;
@@ -44,6 +45,8 @@ struct sangam_ctx {
     uint64_t map_tick;
     // staging for sangam_iteration_host (allocated on first use)
     void *s_q, *s_k, *s_v, *s_out;
+    ConfPartial* d_conf_part;     // sampler: per (row, vocabulary slice) partials, grown on demand
+    int64_t conf_part_cap;
     void* s_packed;               // staging of sangam_iteration_packed
     int64_t s_packed_bytes;
     int32_t *s_slot, *s_bt, *s_cu, *s_ctx;
@@ -160,6 +163,7 @@ extern "C" int sangam_destroy(sangam_ctx* ctx) {
     DeviceGuard guard(ctx->cfg.device);
     cudaFree(ctx->d_dec_part_o); cudaFree(ctx->d_dec_part_ml); cudaFree(ctx->d_dec_cnt);
     cudaFree(ctx->d_flags); cudaFree(ctx->d_sched); cudaFree(ctx->d_part_o); cudaFree(ctx->d_part_ml); cudaFree(ctx->d_slot_meta); cudaFree(ctx->d_plan_cache);
+    cudaFree(ctx->d_conf_part);
     cudaFree(ctx->s_q); cudaFree(ctx->s_k); cudaFree(ctx->s_v); cudaFree(ctx->s_out); cudaFree(ctx->s_packed);
     cudaFree(ctx->s_slot); cudaFree(ctx->s_bt); cudaFree(ctx->s_cu); cudaFree(ctx->s_ctx);
     delete ctx;
@@ -201,6 +205,58 @@ extern "C" int sangam_kv_write(sangam_ctx* ctx, const void* k, const void* v, co
                   (const uint4*)k, (const uint4*)v, slot_mapping, num_tokens, (uint4*)k_pages, (uint4*)v_pages,
                   (int32_t)ctx->cfg.num_kv_heads, (int32_t)cpr, (int32_t)(ctx->cfg.num_pages * SANGAM_PAGE), ctx->d_flags));
     ctx->launches += 1;
+    CK(cudaGetLastError());
+    return SANGAM_OK;
+}
+
+
+extern "C" int sangam_kv_write_rope(sangam_ctx* ctx, const void* k, const void* v, const int32_t* slot_mapping, const int32_t* positions,
+                                    const float* cos_sin, int32_t max_pos, int32_t num_tokens, void* k_pages, void* v_pages, void* stream) {
+    if (!ctx) return SANGAM_ERR_INVALID_ARG;
+    if (num_tokens < 0 || max_pos <= 0) return fail(ctx, SANGAM_ERR_INVALID_ARG, "kv_write_rope: bad count");
+    if (num_tokens == 0) return SANGAM_OK;
+    if (!k || !v || !slot_mapping || !positions || !cos_sin || !k_pages || !v_pages) return fail(ctx, SANGAM_ERR_INVALID_ARG, "kv_write_rope: null pointer");
+    if (!aligned16(k) || !aligned16(v) || !aligned16(k_pages) || !aligned16(v_pages) || !aligned16(cos_sin))
+        return fail(ctx, SANGAM_ERR_INVALID_ARG, "kv_write_rope: pointer not 16-byte aligned");
+    ON_CTX_DEVICE(ctx);
+    const int64_t total = (int64_t)num_tokens * ctx->cfg.num_kv_heads * (ctx->cfg.head_dim / 16);
+    int64_t blocks = (total + 255) / 256;
+    const int64_t cap = (int64_t)ctx->sm_count * 16;
+    if (blocks > cap) blocks = cap;
+    CK(launch_pdl(kv_write_rope_kernel, dim3((unsigned)blocks), 256u, 0, (cudaStream_t)stream, (const uint4*)k, (const uint4*)v, slot_mapping,
+                  positions, cos_sin, max_pos, num_tokens, (uint4*)k_pages, (uint4*)v_pages, (int32_t)ctx->cfg.num_kv_heads,
+                  (int32_t)ctx->cfg.head_dim, (int32_t)(ctx->cfg.num_pages * SANGAM_PAGE), ctx->d_flags));
+    ctx->launches += 1;
+    CK(cudaGetLastError());
+    return SANGAM_OK;
+}
+
+extern "C" int sangam_confidence_sample(sangam_ctx* ctx, const void* logits, int32_t vocab, const int32_t* masked, const int32_t* cu_rows,
+                                        int32_t num_requests, int32_t num_rows, float threshold, int32_t* token, float* conf,
+                                        int32_t* unmask, void* stream) {
+    if (!ctx) return SANGAM_ERR_INVALID_ARG;
+    if (vocab <= 0 || num_requests < 0 || num_rows < 0) return fail(ctx, SANGAM_ERR_INVALID_ARG, "confidence_sample: bad count");
+    if (num_requests == 0 || num_rows == 0) return SANGAM_OK;
+    if (!logits || !masked || !cu_rows || !token || !conf || !unmask) return fail(ctx, SANGAM_ERR_INVALID_ARG, "confidence_sample: null pointer");
+    if (reinterpret_cast<uintptr_t>(logits) & 1u) return fail(ctx, SANGAM_ERR_INVALID_ARG, "confidence_sample: logits not 2-byte aligned");
+    ON_CTX_DEVICE(ctx);
+    // enough (row, slice) blocks to fill the machine a few times over; slices of a multiple of 8 elements
+    int slices = (8 * ctx->sm_count + num_rows - 1) / num_rows;
+    slices = slices < 1 ? 1 : (slices > 64 ? 64 : slices);
+    int slice_len = ((vocab + slices - 1) / slices + 7) & ~7;
+    slices = (vocab + slice_len - 1) / slice_len;
+    const int64_t need = (int64_t)num_rows * slices;
+    if (need > ctx->conf_part_cap) {                       // first use / larger batch: (re)allocate (not during graph capture)
+        cudaFree(ctx->d_conf_part); ctx->d_conf_part = nullptr; ctx->conf_part_cap = 0;
+        const int64_t cap = need > (int64_t)ctx->cfg.max_total_q * 8 ? need : (int64_t)ctx->cfg.max_total_q * 8;
+        CK(cudaMalloc(&ctx->d_conf_part, (size_t)cap * sizeof(ConfPartial)));
+        ctx->conf_part_cap = cap;
+    }
+    CK(launch_pdl(confidence_pass1_kernel, dim3((unsigned)slices, (unsigned)num_rows), (unsigned)CONF_THREADS, 0, (cudaStream_t)stream,
+                  (const __nv_bfloat16*)logits, vocab, (int32_t)slice_len, ctx->d_conf_part));
+    CK(launch_pdl(confidence_pass2_kernel, dim3((unsigned)((num_requests + 3) / 4)), 128u, 0, (cudaStream_t)stream,
+                  (const ConfPartial*)ctx->d_conf_part, (int32_t)slices, masked, cu_rows, num_requests, threshold, token, conf, unmask));
+    ctx->launches += 2;
     CK(cudaGetLastError());
     return SANGAM_OK;
 }
