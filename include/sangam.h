@@ -111,6 +111,19 @@ int sangam_kv_write_rope(sangam_ctx* ctx, const void* k, const void* v, const in
                          const float* cos_sin, int32_t max_pos, int32_t num_tokens, void* k_pages, void* v_pages, void* stream);
 
 /*
+ * KV page transfer between workers, the two single-GPU halves (a prefill worker
+ * hands a request's KV to a decode-role worker).  gather copies the pool pages listed in page_ids (device int32, the
+ * request's block-table row) into contiguous staging buffers bf16 [num_pages_listed][Hkv][16][D]; scatter writes such
+ * buffers into the pages page_ids names in the destination pools (the receiver's own allocation).  What moves between
+ * the GPUs is the staging buffer (NCCL send / recv or a peer copy: paper_2607_04206_b200/kv_transfer.py).  A page id
+ * outside [0, num_pages) skips that page and raises SANGAM_DEV_BAD_PAGE.
+ */
+int sangam_kv_gather(sangam_ctx* ctx, const void* k_pages, const void* v_pages, const int32_t* page_ids, int32_t num_pages_listed,
+                     void* k_stage, void* v_stage, void* stream);
+int sangam_kv_scatter(sangam_ctx* ctx, const void* k_stage, const void* v_stage, const int32_t* page_ids, int32_t num_pages_listed,
+                      void* k_pages, void* v_pages, void* stream);
+
+/*
  * Confidence-threshold sampler over the rows the iteration decoded ("unmasks every masked position whose top-1 probability
  * exceeds a threshold"; threshold 0.9).  logits: bf16 [num_rows][vocab] (device, 2-byte aligned
  * rows); masked: int32 [num_rows], nonzero = still masked; cu_rows: int32 [num_requests + 1], rows of request r (its

@@ -77,3 +77,20 @@ def confidence_sample(logits_bits, masked, cu_rows, threshold):
             best = max(cand, key=lambda t: (conf[t], -t))
             unmask[best] = 1
     return token, conf, unmask
+
+
+def kv_gather(k_pages, v_pages, page_ids):
+    """Pools uint16 [P][Hkv][16][D], page_ids int [n]  ->  staging copies [n][Hkv][16][D] (whole-request KV)."""
+    ks = np.empty((len(page_ids),) + k_pages.shape[1:], k_pages.dtype)
+    vs = np.empty_like(ks)
+    for i, pg in enumerate(page_ids):
+        ks[i] = k_pages[int(pg)]
+        vs[i] = v_pages[int(pg)]
+    return ks, vs
+
+
+def kv_scatter(k_stage, v_stage, page_ids, k_pages, v_pages):
+    """In place: the receiver's pages take the staged copies."""
+    for i, pg in enumerate(page_ids):
+        k_pages[int(pg)] = k_stage[i]
+        v_pages[int(pg)] = v_stage[i]

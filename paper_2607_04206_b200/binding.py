@@ -14,7 +14,7 @@ DECLARED_SYMBOLS = [
     "sangam_last_error", "sangam_version", "sangam_set_dispatch", "sangam_query",
     "sangam_sched_create", "sangam_sched_destroy", "sangam_sched_submit", "sangam_sched_next", "sangam_sched_complete",
     "sangam_sched_query", "sangam_packed_layout", "sangam_iteration_packed",
-    "sangam_kv_write_rope", "sangam_confidence_sample",
+    "sangam_kv_write_rope", "sangam_confidence_sample", "sangam_kv_gather", "sangam_kv_scatter",
 ]
 
 DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE = 0, 1, 2
@@ -77,6 +77,8 @@ def load_library(build_if_missing: bool = False):
     lib.sangam_iteration_packed.argtypes = [vp, vp, i32, vp, vp, i32, i32, f32, vp, vp]
     lib.sangam_kv_write_rope.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, vp, vp, vp]
     lib.sangam_confidence_sample.argtypes = [vp, vp, i32, vp, vp, i32, i32, f32, vp, vp, vp, vp]
+    lib.sangam_kv_gather.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp]
+    lib.sangam_kv_scatter.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp]
     lib.sangam_sched_create.argtypes = [ctypes.POINTER(_SchedConfig), ctypes.POINTER(vp)]
     lib.sangam_sched_destroy.argtypes = [vp]
     lib.sangam_sched_submit.argtypes = [vp, ctypes.c_int64, ctypes.c_double, i32, i32, i32]
@@ -157,6 +159,14 @@ class Sangam:
         self._check(self.lib.sangam_confidence_sample(self.ctx, _ptr(logits), int(logits.shape[1]), _ptr(masked), _ptr(cu_rows),
                                                       int(cu_rows.numel()) - 1, int(logits.shape[0]), float(threshold), _ptr(token),
                                                       _ptr(conf), _ptr(unmask), _stream(stream)))
+
+    def kv_gather(self, k_pages, v_pages, page_ids, k_stage, v_stage, stream=None):
+        self._check(self.lib.sangam_kv_gather(self.ctx, _ptr(k_pages), _ptr(v_pages), _ptr(page_ids), int(page_ids.numel()),
+                                              _ptr(k_stage), _ptr(v_stage), _stream(stream)))
+
+    def kv_scatter(self, k_stage, v_stage, page_ids, k_pages, v_pages, stream=None):
+        self._check(self.lib.sangam_kv_scatter(self.ctx, _ptr(k_stage), _ptr(v_stage), _ptr(page_ids), int(page_ids.numel()),
+                                               _ptr(k_pages), _ptr(v_pages), _stream(stream)))
 
     def block_attn(self, q, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, scale, out, stream=None, simt=False):
         fn = self.lib.sangam_block_attn_simt if simt else self.lib.sangam_block_attn

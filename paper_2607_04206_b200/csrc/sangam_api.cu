@@ -13,6 +13,7 @@
 #include "attn_simt.cuh"
 #include "attn_tc.cuh"
 #include "common.cuh"
+#include "kv_transfer.cuh"
 #include "kv_write.cuh"
 #include "neighbours.cuh"
 #include "sched.cuh"
@@ -259,6 +260,40 @@ extern "C" int sangam_confidence_sample(sangam_ctx* ctx, const void* logits, int
     ctx->launches += 2;
     CK(cudaGetLastError());
     return SANGAM_OK;
+}
+
+static int kv_pages_copy(sangam_ctx* ctx, bool gather, void* k_pages, void* v_pages, void* k_stage, void* v_stage, const int32_t* page_ids,
+                         int32_t n, void* stream) {
+    if (!ctx) return SANGAM_ERR_INVALID_ARG;
+    if (n < 0) return fail(ctx, SANGAM_ERR_INVALID_ARG, "kv_gather/scatter: negative count");
+    if (n == 0) return SANGAM_OK;
+    if (!k_pages || !v_pages || !k_stage || !v_stage || !page_ids) return fail(ctx, SANGAM_ERR_INVALID_ARG, "kv_gather/scatter: null pointer");
+    if (!aligned16(k_pages) || !aligned16(v_pages) || !aligned16(k_stage) || !aligned16(v_stage))
+        return fail(ctx, SANGAM_ERR_INVALID_ARG, "kv_gather/scatter: pointer not 16-byte aligned");
+    ON_CTX_DEVICE(ctx);
+    const int32_t cpp = ctx->cfg.num_kv_heads * SANGAM_PAGE * ctx->cfg.head_dim / 8;
+    int64_t blocks = ((int64_t)n * cpp + 255) / 256;
+    const int64_t cap = (int64_t)ctx->sm_count * 16;
+    if (blocks > cap) blocks = cap;
+    if (gather)
+        CK(launch_pdl(kv_pages_copy_kernel<true>, dim3((unsigned)blocks), 256u, 0, (cudaStream_t)stream, (uint4*)k_pages, (uint4*)v_pages,
+                      (uint4*)k_stage, (uint4*)v_stage, page_ids, n, cpp, (int32_t)ctx->cfg.num_pages, ctx->d_flags));
+    else
+        CK(launch_pdl(kv_pages_copy_kernel<false>, dim3((unsigned)blocks), 256u, 0, (cudaStream_t)stream, (uint4*)k_pages, (uint4*)v_pages,
+                      (uint4*)k_stage, (uint4*)v_stage, page_ids, n, cpp, (int32_t)ctx->cfg.num_pages, ctx->d_flags));
+    ctx->launches += 1;
+    CK(cudaGetLastError());
+    return SANGAM_OK;
+}
+
+extern "C" int sangam_kv_gather(sangam_ctx* ctx, const void* k_pages, const void* v_pages, const int32_t* page_ids, int32_t num_pages_listed,
+                                void* k_stage, void* v_stage, void* stream) {
+    return kv_pages_copy(ctx, true, const_cast<void*>(k_pages), const_cast<void*>(v_pages), k_stage, v_stage, page_ids, num_pages_listed, stream);
+}
+
+extern "C" int sangam_kv_scatter(sangam_ctx* ctx, const void* k_stage, const void* v_stage, const int32_t* page_ids, int32_t num_pages_listed,
+                                 void* k_pages, void* v_pages, void* stream) {
+    return kv_pages_copy(ctx, false, k_pages, v_pages, const_cast<void*>(k_stage), const_cast<void*>(v_stage), page_ids, num_pages_listed, stream);
 }
 
 static int check_attn_args(sangam_ctx* ctx, const void* q, const void* k_pages, const void* v_pages,

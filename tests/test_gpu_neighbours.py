@@ -114,3 +114,45 @@ def test_sampler_fallback_and_exact_threshold_on_the_gpu():
         torch.cuda.synchronize()
         assert np.array_equal(d_tok.cpu().numpy(), ref[0]) and np.array_equal(d_un.cpu().numpy(), ref[2])
         assert np.array_equal(d_conf.cpu().numpy().astype(np.float64), ref[1])          # these confidences are exact in fp32
+
+
+def test_kv_page_gather_scatter_bit_exact():
+    """The single-GPU halves of the KV transfer: gather a request's pages, scatter them into another pool under
+    different page ids; the receiver then attends over them and gets the sender's result bit for bit."""
+    import torch
+    b = si.custom(82, [32, 20], [1000, 333], num_q_heads=8, num_kv_heads=4, head_dim=128)
+    src = DeviceBatch(b)
+    out_src = bits_of(src.iteration()).copy()
+    dst = DeviceBatch(b)                                   # same geometry, empty (poisoned) pools
+    g = np.random.default_rng(6)
+    new_bt = np.full_like(b.block_table, -1)
+    free = g.permutation(b.num_pages)
+    used = 0
+    for r in range(b.batch):
+        n = (int(b.ctx_lens[r]) + 15) // 16
+        ids_src = b.block_table[r, :n]
+        ids_dst = free[used:used + n].astype(np.int32); used += n
+        new_bt[r, :n] = ids_dst
+        shape = (n, b.num_kv_heads, 16, b.head_dim)
+        ks = torch.zeros(shape, dtype=torch.bfloat16, device="cuda"); vs = torch.zeros_like(ks)
+        src.eng.kv_gather(src.k_pages, src.v_pages, t_i32(ids_src), ks, vs)
+        kr, vr = nb.kv_gather(bits_of(src.k_pages), bits_of(src.v_pages), ids_src)
+        torch.cuda.synchronize()
+        assert np.array_equal(bits_of(ks), kr) and np.array_equal(bits_of(vs), vr)
+        dst.eng.kv_scatter(ks, vs, t_i32(ids_dst), dst.k_pages, dst.v_pages)
+    torch.cuda.synchronize()
+    kd = np.full((b.num_pages, b.num_kv_heads, 16, b.head_dim), si.POISON, np.uint16); vd = kd.copy()
+    for r in range(b.batch):
+        n = (int(b.ctx_lens[r]) + 15) // 16
+        nb.kv_scatter(*nb.kv_gather(bits_of(src.k_pages), bits_of(src.v_pages), b.block_table[r, :n]), new_bt[r, :n], kd, vd)
+    assert np.array_equal(bits_of(dst.k_pages), kd) and np.array_equal(bits_of(dst.v_pages), vd)
+    dst.block_table = t_i32(new_bt)
+    dst.attend()
+    torch.cuda.synchronize()
+    assert np.array_equal(bits_of(dst.out), out_src), "attention over the transferred pages differs from the sender's"
+    # a bad page id is skipped and flagged
+    ids = t_i32(np.array([0, b.num_pages, 1], np.int32))
+    ks = torch.zeros((3, b.num_kv_heads, 16, b.head_dim), dtype=torch.bfloat16, device="cuda"); vs = torch.zeros_like(ks)
+    src.eng.kv_gather(src.k_pages, src.v_pages, ids, ks, vs)
+    assert src.eng.device_status() == 2
+    assert np.all(bits_of(ks)[1] == 0)

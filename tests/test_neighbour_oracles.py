@@ -88,3 +88,23 @@ def test_sampler_fallback_and_masks():
     assert list(un) == [0, 0, 1, 0, 1]                    # row 1 is the most confident of request 0 but already committed -> row 2
     tok, conf, un = nb.confidence_sample(_bits(x), [0, 0, 0, 0, 0], [0, 3, 5], 0.9)
     assert un.sum() == 0                                  # nothing masked, nothing to do
+
+
+def test_kv_gather_scatter_oracle_round_trip_and_brute_force():
+    g = np.random.default_rng(4)
+    P, Hkv, D = 20, 3, 8
+    kp = g.integers(0, 65535, (P, Hkv, 16, D)).astype(np.uint16); vp = g.integers(0, 65535, (P, Hkv, 16, D)).astype(np.uint16)
+    src_ids = [7, 2, 19, 0]
+    ks, vs = nb.kv_gather(kp, vp, src_ids)
+    for i, pg in enumerate(src_ids):                       # element by element
+        for h in range(Hkv):
+            for o in range(16):
+                for d in range(D):
+                    assert ks[i, h, o, d] == kp[pg, h, o, d] and vs[i, h, o, d] == vp[pg, h, o, d]
+    kd = np.zeros_like(kp); vd = np.zeros_like(vp)
+    dst_ids = [1, 5, 3, 11]
+    nb.kv_scatter(ks, vs, dst_ids, kd, vd)
+    for s, t in zip(src_ids, dst_ids):
+        assert np.array_equal(kd[t], kp[s]) and np.array_equal(vd[t], vp[s])
+    untouched = [p for p in range(P) if p not in dst_ids]
+    assert np.all(kd[untouched] == 0) and np.all(vd[untouched] == 0)
