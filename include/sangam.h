@@ -160,12 +160,15 @@ int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_pages, const
 #define SANGAM_DISPATCH_AUTO    0
 #define SANGAM_DISPATCH_PREFILL 1
 #define SANGAM_DISPATCH_DECODE  2
+#define SANGAM_DISPATCH_GQA_PAIR 3   /* the CTA-pair decode kernel of GQA models (AUTO picks it for block decodes of up to
+                                        2 * floor(128 / G) tokens per request on average, 1 < G <= 128) */
 int sangam_set_dispatch(sangam_ctx* ctx, int32_t mode);
 
 /* Read-only facts about a ctx (host side, no device work); -1 for an unknown `what`. */
 #define SANGAM_QUERY_SM_COUNT            0   /* SMs of the ctx's device */
 #define SANGAM_QUERY_DECODE_CTAS_PER_SM  1   /* resident CTAs per SM of the decode kernel (0: kernel unavailable) */
 #define SANGAM_QUERY_DISPATCH            2   /* current SANGAM_DISPATCH_* mode */
+#define SANGAM_QUERY_GQA_PAIR_KERNEL     3   /* 1 if the CTA-pair decode kernel exists for the geometry */
 int32_t sangam_query(const sangam_ctx* ctx, int32_t what);
 
 /*

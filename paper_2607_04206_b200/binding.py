@@ -17,7 +17,7 @@ DECLARED_SYMBOLS = [
     "sangam_kv_write_rope", "sangam_confidence_sample", "sangam_kv_gather", "sangam_kv_scatter",
 ]
 
-DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE = 0, 1, 2
+DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE, DISPATCH_GQA_PAIR = 0, 1, 2, 3
 
 
 class SangamError(RuntimeError):

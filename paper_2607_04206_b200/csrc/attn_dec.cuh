@@ -37,7 +37,8 @@ struct DecParams {
     __nv_bfloat16* out;            // [total_q][Hq][D]
     int32_t batch, total_q;
     int32_t Hq, Hkv, G, W, P;
-    int32_t tq;                    // query tokens per unit = 32 / G
+    int32_t tq;                    // query tokens per unit: 32 / G (decode kernel), 2 tpt (GQA pair kernel)
+    int32_t tpt;                   // GQA pair kernel: tokens per 128-row q tile = 128 / G
     uint32_t tq_magic;             // floor(2^32 / tq) + 1: x / tq = umulhi(x, magic) for x < 2^24 (unused when tq = 1)
     uint32_t g_magic;              // floor(2^32 / G) + 1 (unused when G = 1)
     float scale_log2;              // scale * log2(e)
@@ -186,105 +187,103 @@ __device__ __forceinline__ int owner(int y, const PlanConst& pc) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// warp 0: device-side plan (a3) + TMA page gather (a4) + Q loads
+// Device-side plan (a3), one warp, all lanes: stream-K cut of the flattened weighted unit list at page granularity.
+// `nc` workers (CTAs, or clusters) share the T coordinates equally; worker `b` walks its range with next().
 // ------------------------------------------------------------------------------------------------
-template <int D>
-__device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensorMap* mapK, const CUtensorMap* mapV,
-                                              const CUtensorMap* mapQ, uint8_t* smem, uint32_t sbase, Item* items,
-                                              volatile uint32_t* abort_flag, int lane) {
-    using L = Smem<D>;
-    const unsigned FULL = 0xffffffffu;
-    const int NC = gridDim.x, b = blockIdx.x, R = p.batch;
-    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
-    DT(1);
-    // lane r keeps request r (< 32) in registers; later look-ups are shuffles
-    int rq0 = 0, rqn = 0, rc = 0;
-    if (lane < R) load_req(p, lane, rq0, rqn, rc);
-    auto get = [&](int r) {                                  // warp-uniform r
+struct Planner {
+    int rq0, rqn, rc;        // request `lane` (< 32) in registers; later look-ups are shuffles
+    PlanConst pc;
+    int R, b, remaining, r_cur, u_in_r, off, unit_base, unit_gid;
+    ReqInfo cur;
+
+    __device__ __forceinline__ ReqInfo get(const DecParams& p, int r) const {             // warp-uniform r
         int a, q, c;
-        if (r < 32) { a = __shfl_sync(FULL, rq0, r); q = __shfl_sync(FULL, rqn, r); c = __shfl_sync(FULL, rc, r); }
+        if (r < 32) { a = __shfl_sync(0xffffffffu, rq0, r); q = __shfl_sync(0xffffffffu, rqn, r); c = __shfl_sync(0xffffffffu, rc, r); }
         else load_req(p, r, a, q, c);
         return derive(p, a, q, c);
-    };
-    // weighted length and unit count of the first 32 requests, inclusive prefix sums over the lanes
-    const ReqInfo mine = derive(p, rq0, rqn, rc);
-    const int my_t = lane < R ? mine.units * mine.w : 0, my_u = lane < R ? mine.units : 0;
-    int incl_t = my_t, incl_u = my_u;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int vt = __shfl_up_sync(FULL, incl_t, o), vu = __shfl_up_sync(FULL, incl_u, o);
-        if (lane >= o) { incl_t += vt; incl_u += vu; }
     }
-    int T = __shfl_sync(FULL, incl_t, 31);
-    for (int base = 32; base < R; base += 32) {             // batches of more than 32 requests (rare)
-        int t = 0;
-        if (base + lane < R) { int a, q, c; load_req(p, base + lane, a, q, c); const ReqInfo x = derive(p, a, q, c); t = x.units * x.w; }
+
+    __device__ __forceinline__ void init(const DecParams& p, int lane, int nc, int b_) {
+        const unsigned FULL = 0xffffffffu;
+        R = p.batch; b = b_;
+        rq0 = 0; rqn = 0; rc = 0;
+        if (lane < R) load_req(p, lane, rq0, rqn, rc);
+        // weighted length and unit count of the first 32 requests, inclusive prefix sums over the lanes
+        const ReqInfo mine = derive(p, rq0, rqn, rc);
+        const int my_t = lane < R ? mine.units * mine.w : 0, my_u = lane < R ? mine.units : 0;
+        int incl_t = my_t, incl_u = my_u;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(FULL, t, o);
-        T += t;
-    }
-    // Stream-K cut: Geff CTAs share the T coordinates equally; a CTA's share is never smaller than min_w (tiny
-    // batches use fewer CTAs instead of cutting every unit into slivers).
-    PlanConst pc;
-    pc.T = T;
-    int ge = T > 0 ? div_floor((uint64_t)(uint32_t)T, (uint32_t)(p.min_w > 0 ? p.min_w : 1)) : 0;
-    ge = ge < 1 ? 1 : ge;
-    pc.Geff = T <= 0 ? 0 : (NC < ge ? NC : ge);
-    int remaining = 0, r_cur = R, u_in_r = 0, off = 0, unit_base = 0, unit_gid = 0;
-    ReqInfo cur = mine;
-    if (b < pc.Geff) {
-        const int x0 = cut(b, pc), x1 = cut(b + 1, pc);
-        remaining = x1 - x0;
-        // the request holding coordinate x0
-        int found = -1, req_base = 0, gid_base = 0;
-        const unsigned m = __ballot_sync(FULL, incl_t > x0);
-        if (m) {
-            found = __ffs(m) - 1;
-            req_base = __shfl_sync(FULL, incl_t - my_t, found);
-            gid_base = __shfl_sync(FULL, incl_u - my_u, found);
-        } else {
-            int acc = __shfl_sync(FULL, incl_t, 31), accu = __shfl_sync(FULL, incl_u, 31);
-            for (int base = 32; base < R && found < 0; base += 32) {
-                int tl = 0, ul = 0;
-                if (base + lane < R) { int a, q, c; load_req(p, base + lane, a, q, c); const ReqInfo x = derive(p, a, q, c); tl = x.units * x.w; ul = x.units; }
-                int it2 = tl, iu2 = ul;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int vt = __shfl_up_sync(FULL, incl_t, o), vu = __shfl_up_sync(FULL, incl_u, o);
+            if (lane >= o) { incl_t += vt; incl_u += vu; }
+        }
+        int T = __shfl_sync(FULL, incl_t, 31);
+        for (int base = 32; base < R; base += 32) {             // batches of more than 32 requests (rare)
+            int t = 0;
+            if (base + lane < R) { int a, q, c; load_req(p, base + lane, a, q, c); const ReqInfo x = derive(p, a, q, c); t = x.units * x.w; }
 #pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int vt = __shfl_up_sync(FULL, it2, o), vu = __shfl_up_sync(FULL, iu2, o);
-                    if (lane >= o) { it2 += vt; iu2 += vu; }
-                }
-                const unsigned m2 = __ballot_sync(FULL, acc + it2 > x0);
-                if (m2) {
-                    const int l = __ffs(m2) - 1;
-                    found = base + l;
-                    req_base = acc + __shfl_sync(FULL, it2 - tl, l);
-                    gid_base = accu + __shfl_sync(FULL, iu2 - ul, l);
-                } else {
-                    acc += __shfl_sync(FULL, it2, 31); accu += __shfl_sync(FULL, iu2, 31);
+            for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(FULL, t, o);
+            T += t;
+        }
+        // Geff workers share the T coordinates equally; a share is never smaller than min_w (tiny batches use fewer
+        // workers instead of cutting every unit into slivers)
+        pc.T = T;
+        int ge = T > 0 ? div_floor((uint64_t)(uint32_t)T, (uint32_t)(p.min_w > 0 ? p.min_w : 1)) : 0;
+        ge = ge < 1 ? 1 : ge;
+        pc.Geff = T <= 0 ? 0 : (nc < ge ? nc : ge);
+        remaining = 0; r_cur = R; u_in_r = 0; off = 0; unit_base = 0; unit_gid = 0;
+        cur = mine;
+        if (b < pc.Geff) {
+            const int x0 = cut(b, pc), x1 = cut(b + 1, pc);
+            remaining = x1 - x0;
+            // the request holding coordinate x0
+            int found = -1, req_base = 0, gid_base = 0;
+            const unsigned m = __ballot_sync(FULL, incl_t > x0);
+            if (m) {
+                found = __ffs(m) - 1;
+                req_base = __shfl_sync(FULL, incl_t - my_t, found);
+                gid_base = __shfl_sync(FULL, incl_u - my_u, found);
+            } else {
+                int acc = __shfl_sync(FULL, incl_t, 31), accu = __shfl_sync(FULL, incl_u, 31);
+                for (int base = 32; base < R && found < 0; base += 32) {
+                    int tl = 0, ul = 0;
+                    if (base + lane < R) { int a, q, c; load_req(p, base + lane, a, q, c); const ReqInfo x = derive(p, a, q, c); tl = x.units * x.w; ul = x.units; }
+                    int it2 = tl, iu2 = ul;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int vt = __shfl_up_sync(FULL, it2, o), vu = __shfl_up_sync(FULL, iu2, o);
+                        if (lane >= o) { it2 += vt; iu2 += vu; }
+                    }
+                    const unsigned m2 = __ballot_sync(FULL, acc + it2 > x0);
+                    if (m2) {
+                        const int l = __ffs(m2) - 1;
+                        found = base + l;
+                        req_base = acc + __shfl_sync(FULL, it2 - tl, l);
+                        gid_base = accu + __shfl_sync(FULL, iu2 - ul, l);
+                    } else {
+                        acc += __shfl_sync(FULL, it2, 31); accu += __shfl_sync(FULL, iu2, 31);
+                    }
                 }
             }
-        }
-        if (found >= 0) {
-            r_cur = found;
-            cur = get(r_cur);
-            const int pos = x0 - req_base;
-            u_in_r = div_floor((uint64_t)(uint32_t)pos, (uint32_t)cur.w);
-            off = pos - u_in_r * cur.w;
-            unit_base = req_base + u_in_r * cur.w;
-            unit_gid = gid_base + u_in_r;
-        } else {
-            remaining = 0;
+            if (found >= 0) {
+                r_cur = found;
+                cur = get(p, r_cur);
+                const int pos = x0 - req_base;
+                u_in_r = div_floor((uint64_t)(uint32_t)pos, (uint32_t)cur.w);
+                off = pos - u_in_r * cur.w;
+                unit_base = req_base + u_in_r * cur.w;
+                unit_gid = gid_base + u_in_r;
+            } else {
+                remaining = 0;
+            }
         }
     }
-    DT(2);
 
-    uint32_t stage = 0, phase = 0, icount = 0, qcount = 0;
-    while (true) {
-        if (*abort_flag) break;
-        Item it;
+    // the next piece of work of this worker (it.valid = 0: none left)
+    __device__ __forceinline__ void next(const DecParams& p, Item& it) {
         it.valid = 0; it.r = 0; it.g = 0; it.tok0 = 0; it.ntok = 0; it.q_start = 0; it.c = 0; it.pg0 = 0; it.pg1 = 0;
         it.part_slot = -1; it.unit = 0; it.y0 = 0; it.upages = 0; it.b_head = -1; it.b_last = -1; it.pad0 = 0;
-        // this CTA owns the weighted coordinates [x0, x1) of the flattened unit list; a unit spans OV + max(pages, 1)
+        // this worker owns the weighted coordinates [x0, x1) of the flattened unit list; a unit spans OV + max(pages, 1)
         // of them, coordinate OV + j being its page j.  A range covering only overhead coordinates yields no work there.
         while (remaining > 0 && r_cur < R && !it.valid) {
             const int take = remaining < cur.w - off ? remaining : cur.w - off;
@@ -299,7 +298,7 @@ __device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensor
                 it.ntok = left < p.tq ? left : p.tq;
                 it.q_start = cur.q0; it.c = cur.c;
                 it.pg0 = a; it.pg1 = e < cur.pages ? e : cur.pages;      // empty context: pages = 0 -> no tiles
-                if (!(a == 0 && e == cur.w - OV)) {                       // a piece of a unit split across CTAs
+                if (!(a == 0 && e == cur.w - OV)) {                       // a piece of a unit split across workers
                     it.part_slot = 2 * b + (a == 0 ? 1 : 0);
                     it.unit = unit_gid; it.y0 = unit_base + OV; it.upages = cur.pages;
                     it.b_head = a == 0 ? b : owner(it.y0, pc);
@@ -316,11 +315,35 @@ __device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensor
                     u_in_r = 0;
                     do {
                         ++r_cur;
-                        if (r_cur < R) cur = get(r_cur);
+                        if (r_cur < R) cur = get(p, r_cur);
                     } while (r_cur < R && cur.units == 0);
                 }
             }
         }
+    }
+};
+
+// ------------------------------------------------------------------------------------------------
+// warp 0: device-side plan (a3) + TMA page gather (a4) + Q loads
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensorMap* mapK, const CUtensorMap* mapV,
+                                              const CUtensorMap* mapQ, uint8_t* smem, uint32_t sbase, Item* items,
+                                              volatile uint32_t* abort_flag, int lane) {
+    using L = Smem<D>;
+    const unsigned FULL = 0xffffffffu;
+    const int NC = gridDim.x, b = blockIdx.x;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    DT(1);
+    Planner plan;
+    plan.init(p, lane, NC, b);
+    DT(2);
+
+    uint32_t stage = 0, phase = 0, icount = 0, qcount = 0;
+    while (true) {
+        if (*abort_flag) break;
+        Item it;
+        plan.next(p, it);
         // publish
         const uint32_t islot = icount & 1u;
         ptx::mbar_wait(bar(L::B_ITEM_EMPTY + islot), ((icount >> 1) & 1u) ^ 1u, abort_flag);

@@ -1,0 +1,672 @@
+// attn_gqa.cuh -- steps a3..a9 for DECODE-shaped batches of GQA models: paged, varlen, non-causal block attention on
+// tcgen05 (sm_100a) with CTA PAIRS sharing every K/V tile through TMA multicast.
+//
+// A GQA block decode packs (tokens x G heads) query rows per kv head -- 224 rows for a 32-token block at 7:1 (Dream-7B,
+// PAPER.md:315) -- i.e. two 128-row q tiles that need the same K/V stream.  One CTA holding both tiles makes
+// the SM's tensor pipe, MUFU and shared memory all co-critical with its share of HBM (the shape sits at
+// the ridge).  Here a CLUSTER of two CTAs (two SMs) owns a unit: CTA c computes q tile c, and each K/V tile is loaded ONCE
+// from L2 -- CTA c fetches half of its pages -- and multicast into both CTAs' shared memory.  Per SM and kv tile that
+// leaves one 128x128 QK^T, one PV and 16 K exponentials against 32 KB of HBM traffic: every pipe has slack again and
+// HBM is the only bound.
+//
+// Per CTA: 256 threads; warp 0 = device-side plan (a3) + TMA producer (a4), 1 = MMA issuer (a5, a7), 2 = arrival agent of
+// split units, 4..7 = softmax (a6: thread i owns row i of the CTA's q tile), epilogue (a8) and the fused split-KV merge
+// (a9).  Work unit = (request, kv head, pair of q tiles); the flattened (unit, page) list is cut into one contiguous range
+// per CLUSTER (stream-K, the planner of attn_dec.cuh); both CTAs of a cluster derive the same plan and walk it in
+// lockstep (a K/V stage is refilled only after both CTAs released it).  Pieces of split units are merged by the piece
+// that arrives last, as in attn_dec.cuh.
+#pragma once
+#include <cuda.h>
+
+#include "attn_dec.cuh"
+#include "common.cuh"
+#include "ptx.cuh"
+
+namespace gqa {
+
+using dec::Deferred;
+using dec::Item;
+using dec::OutRef;
+using dec::Planner;
+
+constexpr int BM = 128;          // rows of a q tile (UMMA M)
+constexpr int BN = 128;          // kv positions per tile (8 pages)
+constexpr int NSTAGE = 5;        // ring of K / V tiles
+constexpr int NTHREADS = 256;
+constexpr int SLAB = 128 * 128;  // bytes of one 64-wide swizzled slab of the q tile
+constexpr float LAZY_T = 8.f;
+#ifndef SANGAM_GQA_OV
+#define SANGAM_GQA_OV 16
+#endif
+constexpr int OV = SANGAM_GQA_OV;   // fixed cost of starting / finishing a unit, in pages (stream-K weight)
+constexpr int MIN_W = 64;           // smallest share of the weighted unit list given to a cluster
+template <int D> constexpr int KV_ATOM_STRIDE = 1024 * (D / 64);
+
+template <int D>
+struct Smem {
+    static constexpr int KV_BYTES = BN * D * 2;
+    static constexpr int Q_BYTES = BM * D * 2;
+    static constexpr int OFF_KV = 0;
+    static constexpr int OFF_Q = NSTAGE * KV_BYTES;
+    static constexpr int OFF_BAR = OFF_Q + Q_BYTES;
+    static constexpr int B_KV_FULL = 0, B_KV_EMPTY = NSTAGE, B_ITEM_FULL = 2 * NSTAGE, B_ITEM_EMPTY = B_ITEM_FULL + 2,
+                         B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 1, B_S_FULL = B_Q_EMPTY + 1 /* [2] */,
+                         B_P_FULL = B_S_FULL + 2, B_PV_DONE = B_P_FULL + 1 /* [2] */, B_O_FREE = B_PV_DONE + 2,
+                         B_AGENT_REQ = B_O_FREE + 1, B_AGENT_DONE = B_AGENT_REQ + 1, NBAR = B_AGENT_DONE + 1;
+    static constexpr int OFF_ITEMS = OFF_BAR + ((NBAR * 8 + 15) / 16) * 16;
+    // misc block: +0 tmem slot, +8 merge flag, +16 agent_req[2], +32 Deferred[2], +96 abort word (+ wait table in debug builds)
+    static constexpr int OFF_MISC = OFF_ITEMS + 2 * (int)sizeof(Item);
+    static constexpr int OFF_ABORT = OFF_MISC + 96;
+    static constexpr int TOTAL = OFF_ABORT + 80;
+    static constexpr int ALLOC = TOTAL + 1024;           // slack to align the base to 1024 B
+};
+static_assert(Smem<128>::ALLOC <= 232448, "shared memory budget (227 KB)");
+
+__device__ __forceinline__ uint32_t cluster_rank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// the same shared-memory offset in the peer CTA of the cluster (shared::cluster address)
+__device__ __forceinline__ uint32_t peer_addr(uint32_t local, uint32_t peer) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(peer));
+    return r;
+}
+// one (page, head) box into BOTH CTAs of the pair: same offset, each CTA's own barrier gets the bytes
+__device__ __forceinline__ void tma_load_4d_mc(uint32_t dst_smem, const CUtensorMap* m, uint32_t bar, int32_t c3, uint16_t mask) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%3, %3, %3, %4}], [%2], %5;"
+        ::"r"(dst_smem), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(0), "r"(c3), "h"(mask)
+        : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// warp 0: plan + TMA (this CTA's half of every tile's pages, multicast to the pair) + its q tile
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensorMap* mapK, const CUtensorMap* mapV, const CUtensorMap* mapQ,
+                                              uint32_t sbase, Item* items, volatile uint32_t* abort_flag, int lane, uint32_t rank) {
+    using L = Smem<D>;
+    const unsigned FULL = 0xffffffffu;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    Planner plan;
+    plan.init(p, lane, (int)gridDim.x >> 1, (int)blockIdx.x >> 1);
+    uint32_t stage = 0, phase = 0, icount = 0, qcount = 0;
+    while (true) {
+        if (*abort_flag) break;
+        Item it;
+        plan.next(p, it);
+        const uint32_t islot = icount & 1u;
+        ptx::mbar_wait(bar(L::B_ITEM_EMPTY + islot), ((icount >> 1) & 1u) ^ 1u, abort_flag);
+        if (lane == 0) {
+            items[islot] = it;
+            ptx::mbar_arrive(bar(L::B_ITEM_FULL + islot));
+        }
+        __syncwarp();
+        ++icount;
+        if (!it.valid) break;
+        const int npg = it.pg1 - it.pg0;
+        if (npg <= 0) continue;
+        const int32_t* bt = p.block_table + (int64_t)it.r * p.W + it.pg0;
+        const int nt = (npg + 7) >> 3;
+        // page ids: lane pg (< 8) keeps page pg of the tiles in flight in a 4-entry window indexed by tile & 3 (K runs at most
+        // two tiles ahead of V); the ids of tile kq + 1 are requested when K(kq) is issued
+        auto ld_ids = [&](int t) { return (t < nt && lane < 8 && 8 * t + lane < npg) ? __ldg(bt + 8 * t + lane) : 0; };
+        int w0 = ld_ids(0), w1 = ld_ids(1), w2 = 0, w3 = 0;
+        const int ntok_c = it.ntok - (int)rank * p.tpt;                       // tokens of this CTA's q tile
+        if (ntok_c > 0) {
+            ptx::mbar_wait(bar(L::B_Q_EMPTY), (qcount & 1u) ^ 1u, abort_flag);
+            if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_Q_FULL), (uint32_t)(p.tpt * p.G * D * 2));
+            __syncwarp();
+            if (lane < D / 64)
+                ptx::tma_load_3d(sbase + (uint32_t)(L::OFF_Q + lane * SLAB), mapQ, bar(L::B_Q_FULL), lane * 64, it.g * p.G,
+                                 it.q_start + it.tok0 + (int)rank * p.tpt);
+            ++qcount;
+        }
+        // ring order K(0) K(1) V(0) K(2) V(1) ...: the issuer runs QK one tile ahead of PV
+        int kq = 0, vq = 0;
+        while (vq < nt) {
+            const bool is_v = !(kq < nt && kq <= vq + 1);
+            const int t = is_v ? vq : kq;
+            const int sel = t & 3;
+            int page = sel == 0 ? w0 : sel == 1 ? w1 : sel == 2 ? w2 : w3;
+            int np = npg - 8 * t;
+            np = np > 8 ? 8 : np;
+            const bool mine = lane < np && (lane >> 2) == (int)rank;              // pages 0..3: CTA 0, pages 4..7: CTA 1
+            if (mine && (unsigned)page >= (unsigned)p.P) { raise_flag(p.flags, DEV_BAD_PAGE); page = p.P; }
+            ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), phase ^ 1u, abort_flag);   // both CTAs have released the stage
+            if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_KV_FULL + stage), (uint32_t)(np * SANGAM_PAGE * D * 2));
+            __syncwarp();
+            if (mine)
+                tma_load_4d_mc(sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES + lane * (2 * KV_ATOM_STRIDE<D>)), is_v ? mapV : mapK,
+                               bar(L::B_KV_FULL + stage), (page * p.Hkv + it.g) * 2, (uint16_t)3);
+            if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+            if (is_v) {
+                ++vq;
+            } else {
+                ++kq;
+                const int nx = ld_ids(kq + 1), s2 = (kq + 1) & 3;
+                if (s2 == 0) w0 = nx; else if (s2 == 1) w1 = nx; else if (s2 == 2) w2 = nx; else w3 = nx;
+            }
+            if (*abort_flag) break;
+        }
+    }
+    for (int k = 0; k < NSTAGE; ++k) {      // every commit aimed at this CTA's barriers has landed before it may exit
+        ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), phase ^ 1u, abort_flag);
+        if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+    }
+    ptx::mbar_wait(bar(L::B_Q_EMPTY), (qcount & 1u) ^ 1u, abort_flag);
+}
+
+// ------------------------------------------------------------------------------------------------
+// warp 1: MMA issuer.  S[b] = Q K(j)^T into TMEM buffer b = j & 1 (128 columns), O += P(j) V(j) with P read from TMEM
+// (bf16, packed over the first 32 columns of each 64-column half of S[b]).  QK runs one tile ahead of PV.
+// TMEM: S[0] = columns [0, 128), S[1] = [128, 256), O = [256, 256 + D).
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uint32_t tmem, const Item* items, volatile uint32_t* abort_flag,
+                                         int lane, uint32_t rank) {
+    using L = Smem<D>;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    const uint64_t q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);
+    const uint64_t k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, KV_ATOM_STRIDE<D>);
+    const uint64_t v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 1024, KV_ATOM_STRIDE<D>);
+    constexpr uint32_t VSTEP = (uint32_t)(2 * KV_ATOM_STRIDE<D>) >> 4;
+    constexpr uint32_t IDESC_PV = ptx::idesc_bf16(BM, D, 0, 1);
+    const uint32_t peer = rank ^ 1u;
+    uint32_t stage = 0, phase = 0, icount = 0, qcount = 0, tcount = 0, ocount = 0;
+    auto release = [&](uint32_t s) {         // this CTA is done with stage s: tell both producers of the pair
+        ptx::mma_commit(bar(L::B_KV_EMPTY + s));
+        ptx::mma_commit(peer_addr(bar(L::B_KV_EMPTY + s), peer));
+    };
+    while (true) {
+        if (*abort_flag) break;
+        const uint32_t islot = icount & 1u;
+        ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
+        const Item it = items[islot];
+        if (!it.valid) break;
+        const int npg = it.pg1 - it.pg0, nt = (npg + 7) >> 3;
+        const bool active = it.ntok - (int)rank * p.tpt > 0;
+        if (nt > 0) {
+            const int c_lim = it.c < it.pg1 * SANGAM_PAGE ? it.c : it.pg1 * SANGAM_PAGE;
+            auto nv_of = [&](int t) { int nv = c_lim - (it.pg0 + 8 * t) * SANGAM_PAGE; return nv > BN ? BN : nv; };
+            if (active) { ptx::mbar_wait(bar(L::B_Q_FULL), qcount & 1u, abort_flag); ++qcount; }
+            auto issue_qk = [&](int t) {
+                const uint32_t sk = stage;
+                ptx::mbar_wait(bar(L::B_KV_FULL + sk), phase, abort_flag);
+                if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+                ptx::tc_fence_after();
+                if (ptx::elect_one()) {
+                    if (active) {
+                        const int ncol = (nv_of(t) + 15) & ~15;
+                        const uint32_t s_tmem = tmem + (uint32_t)(((tcount + (uint32_t)t) & 1u) * 128u);
+                        const uint64_t b_desc = k_desc0 + (uint64_t)(sk * (L::KV_BYTES >> 4));
+                        const uint32_t idesc = ptx::idesc_bf16(BM, (uint32_t)ncol, 0, 0);
+                        ptx::mma_ss_x4(s_tmem, q_desc0, b_desc, idesc, 0u, 2u);
+                        if (D == 128) ptx::mma_ss_x4(s_tmem, q_desc0 + (SLAB >> 4), b_desc + (1024 >> 4), idesc, 1u, 2u);
+                    }
+                    release(sk);
+                    if (active) {
+                        ptx::mma_commit(bar(L::B_S_FULL + ((tcount + (uint32_t)t) & 1u)));
+                        if (t == nt - 1) ptx::mma_commit(bar(L::B_Q_EMPTY));
+                    }
+                }
+                __syncwarp();
+            };
+            issue_qk(0);
+            for (int j = 0; j < nt; ++j) {
+                if (*abort_flag) break;
+                if (j + 1 < nt) issue_qk(j + 1);
+                const uint32_t sv = stage;
+                ptx::mbar_wait(bar(L::B_KV_FULL + sv), phase, abort_flag);
+                if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+                const int nv = nv_of(j);
+                if (active) {
+                    if (nv & 15) dec::zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
+                    if (j == 0 && ocount > 0) ptx::mbar_wait(bar(L::B_O_FREE), (ocount - 1u) & 1u, abort_flag);
+                    ptx::mbar_wait(bar(L::B_P_FULL), (tcount + (uint32_t)j) & 1u, abort_flag);
+                }
+                ptx::tc_fence_after();
+                if (ptx::elect_one()) {
+                    if (active) {
+                        const uint32_t s_tmem = tmem + (uint32_t)(((tcount + (uint32_t)j) & 1u) * 128u), o_tmem = tmem + 256u;
+                        const uint64_t b0 = v_desc0 + (uint64_t)(sv * (L::KV_BYTES >> 4));
+                        const int ks_n = (nv + 15) >> 4;                       // one K-step = 16 kv rows = one page
+                        if (ks_n == 8) {
+                            ptx::mma_ts_x4(o_tmem, s_tmem, b0, IDESC_PV, j > 0 ? 1u : 0u, VSTEP);
+                            ptx::mma_ts_x4(o_tmem, s_tmem + 64u, b0 + 4 * VSTEP, IDESC_PV, 1u, VSTEP);
+                        } else {
+                            for (int ks = 0; ks < ks_n; ++ks)       // P of page ks: half ks / 4, 8 packed columns per page inside the half
+                                ptx::mma_ts(o_tmem, s_tmem + (uint32_t)((ks >> 2) * 64 + (ks & 3) * 8), b0 + (uint64_t)(ks * VSTEP), IDESC_PV,
+                                            (j > 0 || ks > 0) ? 1u : 0u);
+                        }
+                    }
+                    release(sv);
+                    if (active) ptx::mma_commit(bar(L::B_PV_DONE + ((tcount + (uint32_t)j) & 1u)));
+                }
+                __syncwarp();
+            }
+            if (active) { tcount += (uint32_t)nt; ++ocount; }
+        }
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
+        ++icount;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// warps 4..7: softmax (thread `row` owns row `row` of the CTA's q tile = TMEM lane `row`), epilogue, merge
+// ------------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem, uint32_t sbase, uint32_t tmem, const Item* items,
+                                              volatile uint32_t* abort_flag, int warp, int lane, uint32_t rank) {
+    using L = Smem<D>;
+    const unsigned FULL = 0xffffffffu;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    const int qd = warp & 3, row = qd * 32 + lane;
+    const uint32_t lane_base = (uint32_t)(qd * 32) << 16;
+    const uint32_t o_taddr = tmem + lane_base + 256u;
+    volatile int* merge_flag = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 8);
+    volatile int* agent_req = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 16);
+    const float sc = fabsf(p.scale_log2);
+    const uint32_t flip = p.scale_log2 < 0.f ? 0x80000000u : 0u;
+    const int NS = 4 * ((int)gridDim.x >> 1);                 // partial slots: 2 per cluster x 2 CTAs
+    constexpr int SLOT_F4 = (D / 4) * BM;                      // float4 per partial slot: [D/4 column groups][128 rows]
+
+    // out row of packed row `row` of a unit: token row / G, head row % G
+    auto out_ptr = [&](const OutRef& r) {
+        const int tl = p.G == 1 ? row : (int)__umulhi((uint32_t)row, p.g_magic), hh = row - tl * p.G;
+        const int tok = r.q_start + r.tok0 + (int)rank * p.tpt + tl;
+        return p.out + ((int64_t)tok * p.Hq + (int64_t)r.g * p.G + hh) * D;
+    };
+    auto rows_of = [&](const OutRef& r) { int n = r.ntok - (int)rank * p.tpt; n = n > p.tpt ? p.tpt : n; return n > 0 ? n * p.G : 0; };
+    auto ref_ok = [&](const OutRef& r) {
+        return r.q_start + r.tok0 >= 0 && r.q_start + r.tok0 + r.ntok <= p.total_q && (unsigned)r.g < (unsigned)p.Hkv;
+    };
+    // General merge of this CTA's tile of a split unit: pieces in clusters bh .. bl, in that order whoever merges
+    auto merge_unit = [&](const OutRef& r, int unit, int bh, int bl) {
+        const bool ok = row < rows_of(r) && ref_ok(r);
+        auto slot_of = [&](int bb) { return (bb == bh ? 2 * bh + 1 : 2 * bb) * 2 + (int)rank; };
+        const float2* ml = reinterpret_cast<const float2*>(p.part_ml);
+        float M = -INFINITY;
+        for (int bb = bh; bb <= bl; ++bb) M = fmaxf(M, __ldcg(ml + (int64_t)slot_of(bb) * BM + row).x);
+        float Lsum = 0.f;
+        for (int bb = bh; bb <= bl; ++bb) { const float2 x = __ldcg(ml + (int64_t)slot_of(bb) * BM + row); Lsum = fmaf(x.y, ptx::ex2(x.x - M), Lsum); }
+        const float inv = Lsum > 0.f ? 1.f / Lsum : 0.f;
+        __nv_bfloat16* dst = out_ptr(r);
+#pragma unroll 1
+        for (int c = 0; c < D / 32; ++c) {
+            float f[32];
+#pragma unroll
+            for (int e = 0; e < 32; ++e) f[e] = 0.f;
+            for (int bb = bh; bb <= bl; ++bb) {
+                const int slot = slot_of(bb);
+                const float w = ptx::ex2(__ldcg(ml + (int64_t)slot * BM + row).x - M);
+                const float4* so = reinterpret_cast<const float4*>(p.part_o) + (int64_t)slot * SLOT_F4 + (int64_t)(c * 8) * BM + row;
+#pragma unroll
+                for (int v = 0; v < 8; ++v) {
+                    const float4 o = __ldcg(so + v * BM);
+                    f[4 * v] = fmaf(o.x, w, f[4 * v]); f[4 * v + 1] = fmaf(o.y, w, f[4 * v + 1]);
+                    f[4 * v + 2] = fmaf(o.z, w, f[4 * v + 2]); f[4 * v + 3] = fmaf(o.w, w, f[4 * v + 3]);
+                }
+            }
+            if (ok) {
+#pragma unroll
+                for (int v = 0; v < 4; ++v) {
+                    uint4 w4;
+                    w4.x = ptx::pack_bf16(f[8 * v] * inv, f[8 * v + 1] * inv); w4.y = ptx::pack_bf16(f[8 * v + 2] * inv, f[8 * v + 3] * inv);
+                    w4.z = ptx::pack_bf16(f[8 * v + 4] * inv, f[8 * v + 5] * inv); w4.w = ptx::pack_bf16(f[8 * v + 6] * inv, f[8 * v + 7] * inv);
+                    reinterpret_cast<uint4*>(dst)[c * 4 + v] = w4;
+                }
+            }
+        }
+        ptx::bar_sync(1, 128);
+        if (qd == 0 && lane == 0) p.unit_cnt[2 * unit + (int)rank] = 0;       // re-arm for the next launch
+    };
+
+    uint32_t icount = 0, tcount = 0;
+    // PV(k) signals PV_DONE[k & 1]: two barriers, so that a wait for tile k (whose PV(k - 2) is known to be complete: it
+    // precedes QK(k) on the in-order tensor pipe) finds its barrier in phase k or k + 2, never further -- a parity wait
+    // cannot tell phases two apart, and these waits are not taken for every tile
+    auto wait_pv = [&](uint32_t k) { ptx::mbar_wait(bar(L::B_PV_DONE + (k & 1u)), (k >> 1) & 1u, abort_flag); };
+    while (true) {
+        if (*abort_flag) break;
+        const uint32_t islot = icount & 1u;
+        ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
+        const Item it = items[islot];
+        if (!it.valid) break;
+        OutRef ref;
+        ref.q_start = it.q_start; ref.tok0 = it.tok0; ref.ntok = it.ntok; ref.g = it.g;
+        const int rows = rows_of(ref);
+        const int npg = it.pg1 - it.pg0, nt = rows > 0 ? (npg + 7) >> 3 : 0;
+        const int c_lim = it.c < it.pg1 * SANGAM_PAGE ? it.c : it.pg1 * SANGAM_PAGE;
+        const bool row_ok = row < rows && ref_ok(ref);
+        if (rows > 0 && !ref_ok(ref) && lane == 0) raise_flag(p.flags, DEV_INTERNAL | 0x400u);
+        float m_ref = -INFINITY, l = 0.f;
+        int peek = -1;
+        for (int t = 0; t < nt; ++t) {
+            if (*abort_flag) break;
+            int nv = c_lim - (it.pg0 + 8 * t) * SANGAM_PAGE;
+            nv = nv > BN ? BN : nv;
+            const uint32_t b = tcount & 1u;
+            const uint32_t s_taddr = tmem + lane_base + b * 128u;
+            if (t == nt - 1 && it.part_slot >= 0 && qd == 0 && lane == 0)
+                asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(peek) : "l"(p.unit_cnt + 2 * it.unit + (int)rank) : "memory");
+            ptx::mbar_wait(bar(L::B_S_FULL + b), (tcount >> 1) & 1u, abort_flag);
+            ptx::tc_fence_after();
+            // pass 1: the row's maximum over the tile (positions >= nv masked)
+            float mx = -INFINITY;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (nv - 64 * h <= 0) continue;
+                uint32_t r0[32], r1[32];
+                ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h), r0);
+                ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h + 32), r1);
+                ptx::tmem_wait_ld();
+                const int lim = nv - 64 * h;
+#pragma unroll
+                for (int i = 0; i < 32; ++i) {
+                    const float a = __uint_as_float(r0[i] ^ flip), c2 = __uint_as_float(r1[i] ^ flip);
+                    mx = fmaxf(mx, fmaxf(i < lim ? a : -INFINITY, 32 + i < lim ? c2 : -INFINITY));
+                }
+            }
+            mx *= sc;
+            const bool grow = mx > m_ref + LAZY_T;
+            const float m_new = grow ? mx : m_ref;
+            const float alpha = grow ? ptx::ex2(m_ref - m_new) : 1.f;
+            m_ref = m_new;
+            l *= alpha;
+            if (t > 0 && __any_sync(FULL, alpha != 1.f)) {
+                // rare (lazy reference maximum): every PV so far must have landed in O before the rows shrink
+                wait_pv(tcount - 1u);
+                ptx::tc_fence_after();
+#pragma unroll 1
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t o[32];
+                    ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
+                    ptx::tmem_wait_ld();
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
+                    ptx::tmem_st32(o_taddr + (uint32_t)(c * 32), o);
+                }
+                ptx::tmem_wait_st();
+            }
+            // pass 2: P = 2^(s scale - m_ref) as bf16 pairs over the first 32 columns of each half, row sum into l
+            float sum = 0.f;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (nv - 64 * h <= 0) continue;
+                uint32_t r0[32], r1[32];
+                ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h), r0);
+                ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h + 32), r1);
+                ptx::tmem_wait_ld();
+                const int lim = nv - 64 * h;
+                uint32_t pk[32];
+#pragma unroll
+                for (int i = 0; i < 32; i += 2) {
+                    float a0 = ptx::ex2(fmaf(__uint_as_float(r0[i] ^ flip), sc, -m_ref)), a1 = ptx::ex2(fmaf(__uint_as_float(r0[i + 1] ^ flip), sc, -m_ref));
+                    float c0 = ptx::ex2(fmaf(__uint_as_float(r1[i] ^ flip), sc, -m_ref)), c1 = ptx::ex2(fmaf(__uint_as_float(r1[i + 1] ^ flip), sc, -m_ref));
+                    if (i >= lim) a0 = 0.f;
+                    if (i + 1 >= lim) a1 = 0.f;
+                    if (32 + i >= lim) c0 = 0.f;
+                    if (33 + i >= lim) c1 = 0.f;
+                    sum += (a0 + a1) + (c0 + c1);
+                    pk[i >> 1] = ptx::pack_bf16(a0, a1);
+                    pk[16 + (i >> 1)] = ptx::pack_bf16(c0, c1);
+                }
+                ptx::tmem_st16(s_taddr + (uint32_t)(64 * h), pk);
+                ptx::tmem_st16(s_taddr + (uint32_t)(64 * h + 16), pk + 16);
+            }
+            l += sum;
+            ptx::tmem_wait_st();
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL));
+            ++tcount;
+        }
+        // ---------------- epilogue
+        const bool split = nt > 0 && it.part_slot >= 0;
+        const int np_u = it.b_last - it.b_head + 1, k_me = ((int)blockIdx.x >> 1) - it.b_head;
+        bool early = false;
+        if (split) {
+            if (qd == 0 && lane == 0) {
+                const int e = (np_u == 2 && (k_me == 0 || k_me == 1) && peek + npg == it.upages) ? 1 : 0;
+                if (e) asm volatile("fence.acq_rel.gpu;" ::: "memory");
+                *merge_flag = e;
+            }
+            ptx::bar_sync(1, 128);
+            early = *merge_flag != 0;
+            ptx::bar_sync(1, 128);
+        }
+        __nv_bfloat16* dst = out_ptr(ref);
+        if (rows > 0 && nt == 0) {
+            if (row_ok && it.part_slot < 0) {                    // empty context: zero rows (reading S13)
+#pragma unroll
+                for (int c = 0; c < D / 8; ++c) reinterpret_cast<uint4*>(dst)[c] = make_uint4(0, 0, 0, 0);
+            }
+        } else if (nt > 0) {
+            // the other piece of a two-piece unit is requested before the last PV is awaited (early merge, see attn_dec.cuh)
+            const int other = (k_me == 0 ? 2 * (it.b_head + 1) : 2 * it.b_head + 1) * 2 + (int)rank;
+            float2 xo = make_float2(-INFINITY, 0.f);
+            if (early) xo = __ldcg(reinterpret_cast<const float2*>(p.part_ml) + (int64_t)other * BM + row);
+            wait_pv(tcount - 1u);                                 // the unit's last PV (PVs complete in order)
+            ptx::tc_fence_after();
+            const bool partial = split && !early;
+            const bool slot_ok = !partial || (it.part_slot * 2 + (int)rank < NS && it.unit >= 0);
+            if (!slot_ok && lane == 0) raise_flag(p.flags, DEV_INTERNAL | 0x100u);
+            const int slot = it.part_slot * 2 + (int)rank;
+            float w_own = 1.f, w_oth = 0.f, inv = l > 0.f ? 1.f / l : 0.f;
+            if (early) {                                         // pieces in order: k_me = 0: own, other;  1: other, own
+                const float M = fmaxf(m_ref, xo.x);
+                w_own = ptx::ex2(m_ref - M); w_oth = ptx::ex2(xo.x - M);
+                const float Lsum = k_me == 0 ? fmaf(xo.y, w_oth, fmaf(l, w_own, 0.f)) : fmaf(l, w_own, fmaf(xo.y, w_oth, 0.f));
+                inv = Lsum > 0.f ? 1.f / Lsum : 0.f;
+            }
+#pragma unroll 1
+            for (int c = 0; c < D / 32; ++c) {
+                uint32_t o[32];
+                float4 ov[8];
+                if (early) {
+                    const float4* so = reinterpret_cast<const float4*>(p.part_o) + (int64_t)other * SLOT_F4 + (int64_t)(c * 8) * BM + row;
+#pragma unroll
+                    for (int v = 0; v < 8; ++v) ov[v] = __ldcg(so + v * BM);
+                }
+                ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
+                ptx::tmem_wait_ld();
+                float f[32];
+                if (early) {
+#pragma unroll
+                    for (int v = 0; v < 8; ++v) {
+                        const float e0 = ov[v].x, e1 = ov[v].y, e2 = ov[v].z, e3 = ov[v].w;
+                        const float a0 = __uint_as_float(o[4 * v]), a1 = __uint_as_float(o[4 * v + 1]), a2 = __uint_as_float(o[4 * v + 2]), a3 = __uint_as_float(o[4 * v + 3]);
+                        if (k_me == 0) {
+                            f[4 * v] = fmaf(e0, w_oth, fmaf(a0, w_own, 0.f)); f[4 * v + 1] = fmaf(e1, w_oth, fmaf(a1, w_own, 0.f));
+                            f[4 * v + 2] = fmaf(e2, w_oth, fmaf(a2, w_own, 0.f)); f[4 * v + 3] = fmaf(e3, w_oth, fmaf(a3, w_own, 0.f));
+                        } else {
+                            f[4 * v] = fmaf(a0, w_own, fmaf(e0, w_oth, 0.f)); f[4 * v + 1] = fmaf(a1, w_own, fmaf(e1, w_oth, 0.f));
+                            f[4 * v + 2] = fmaf(a2, w_own, fmaf(e2, w_oth, 0.f)); f[4 * v + 3] = fmaf(a3, w_own, fmaf(e3, w_oth, 0.f));
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(o[e]);
+                }
+                if (partial) {
+                    if (slot_ok && row < rows) {
+                        float4* po = reinterpret_cast<float4*>(p.part_o) + (int64_t)slot * SLOT_F4 + (int64_t)(c * 8) * BM + row;
+#pragma unroll
+                        for (int v = 0; v < 8; ++v) po[v * BM] = make_float4(f[4 * v], f[4 * v + 1], f[4 * v + 2], f[4 * v + 3]);
+                    }
+                } else if (row_ok) {
+#pragma unroll
+                    for (int v = 0; v < 4; ++v) {
+                        uint4 w4;
+                        w4.x = ptx::pack_bf16(f[8 * v] * inv, f[8 * v + 1] * inv); w4.y = ptx::pack_bf16(f[8 * v + 2] * inv, f[8 * v + 3] * inv);
+                        w4.z = ptx::pack_bf16(f[8 * v + 4] * inv, f[8 * v + 5] * inv); w4.w = ptx::pack_bf16(f[8 * v + 6] * inv, f[8 * v + 7] * inv);
+                        reinterpret_cast<uint4*>(dst)[c * 4 + v] = w4;
+                    }
+                }
+            }
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_O_FREE));
+            if (partial && slot_ok && row < rows) reinterpret_cast<float2*>(p.part_ml)[(int64_t)slot * BM + row] = make_float2(m_ref, l);
+            if (split) {
+                if (qd == 0 && lane == 0) {
+                    agent_req[islot] = (partial && slot_ok) ? 1 : 0;
+                    if (early) p.unit_cnt[2 * it.unit + (int)rank] = 0;        // re-arm the counter
+                }
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(bar(L::B_AGENT_REQ));
+            }
+        }
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
+        ++icount;
+    }
+    ptx::mbar_wait(bar(L::B_AGENT_DONE), 0u, abort_flag);
+    const Deferred* defer = reinterpret_cast<const Deferred*>(smem + L::OFF_MISC + 32);
+    for (int k = 0; k < 2; ++k) {
+        const Deferred dr = defer[k];
+        if (dr.valid) {
+            OutRef r;
+            r.q_start = dr.q_start; r.tok0 = dr.tok0; r.ntok = dr.ntok; r.g = dr.g;
+            merge_unit(r, dr.unit, dr.b_head, dr.b_last);
+        }
+    }
+}
+
+// warp 2: arrival agent (attn_dec.cuh): gpu-scope release of a stored piece, arrival count, Deferred record if it was the last
+template <int D>
+__device__ __forceinline__ void agent_warp(const DecParams& p, uint8_t* smem, uint32_t sbase, const Item* items, volatile uint32_t* abort_flag,
+                                           int lane, uint32_t rank) {
+    using L = Smem<D>;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    volatile int* agent_req = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 16);
+    Deferred* defer = reinterpret_cast<Deferred*>(smem + L::OFF_MISC + 32);
+    uint32_t icount = 0, rcount = 0;
+    int ndef = 0;
+    while (true) {
+        if (*abort_flag) break;
+        const uint32_t islot = icount & 1u;
+        ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
+        const Item it = items[islot];
+        if (!it.valid) break;
+        const int npg = it.pg1 - it.pg0;
+        const bool active = it.ntok - (int)rank * p.tpt > 0;
+        if (npg > 0 && it.part_slot >= 0 && active) {
+            ptx::mbar_wait(bar(L::B_AGENT_REQ), rcount & 1u, abort_flag);
+            ++rcount;
+            if (lane == 0 && agent_req[islot] != 0) {
+                int old;
+                asm volatile("fence.acq_rel.gpu;" ::: "memory");
+                asm volatile("atom.relaxed.gpu.global.add.s32 %0, [%1], %2;" : "=r"(old) : "l"(p.unit_cnt + 2 * it.unit + (int)rank), "r"(npg) : "memory");
+                if (old + npg == it.upages) {
+                    asm volatile("fence.acq_rel.gpu;" ::: "memory");
+                    if (ndef < 2) {
+                        Deferred dr;
+                        dr.valid = 1; dr.unit = it.unit; dr.b_head = it.b_head; dr.b_last = it.b_last;
+                        dr.q_start = it.q_start; dr.tok0 = it.tok0; dr.ntok = it.ntok; dr.g = it.g;
+                        defer[ndef++] = dr;
+                    } else {
+                        raise_flag(p.flags, DEV_INTERNAL | 0x200u);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
+        ++icount;
+    }
+    __syncwarp();
+    if (lane == 0) ptx::mbar_arrive(bar(L::B_AGENT_DONE));
+}
+
+template <int D>
+__global__ void __launch_bounds__(NTHREADS, 1)
+gqa_decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
+                  const __grid_constant__ CUtensorMap mapQ, const DecParams p) {
+    using L = Smem<D>;
+    extern __shared__ uint8_t smem_raw[];
+    // both CTAs of the pair must use the SAME offsets inside their shared-memory windows (multicast writes land at the
+    // issuing CTA's offset): the dynamic base is the same in every CTA of a launch, so is the alignment fix-up
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    const uint32_t sbase = ptx::smem_u32(smem);
+    Item* items = reinterpret_cast<Item*>(smem + L::OFF_ITEMS);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::OFF_MISC);
+    volatile uint32_t* abort_flag = reinterpret_cast<volatile uint32_t*>(smem + L::OFF_ABORT);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t rank = cluster_rank();
+    if (tid == 0) {
+        auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+        for (int s = 0; s < NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 2); }   // both CTAs release
+        for (int s = 0; s < 2; ++s) {
+            ptx::mbar_init(bar(L::B_ITEM_FULL + s), 1); ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 6);      // MMA warp + agent + 4 softmax warps
+            ptx::mbar_init(bar(L::B_S_FULL + s), 1);
+        }
+        ptx::mbar_init(bar(L::B_Q_FULL), 1); ptx::mbar_init(bar(L::B_Q_EMPTY), 1);
+        ptx::mbar_init(bar(L::B_P_FULL), 4); ptx::mbar_init(bar(L::B_PV_DONE), 1); ptx::mbar_init(bar(L::B_PV_DONE + 1), 1);
+        ptx::mbar_init(bar(L::B_O_FREE), 4);
+        ptx::mbar_init(bar(L::B_AGENT_REQ), 4); ptx::mbar_init(bar(L::B_AGENT_DONE), 1);
+        for (int k = 1; k < (L::TOTAL - L::OFF_MISC) / 4; ++k) tmem_slot[k] = 0u;
+        ptx::fence_mbar_init();
+        ptx::prefetch_tensormap(&mapK);
+        ptx::prefetch_tensormap(&mapV);
+        ptx::prefetch_tensormap(&mapQ);
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
+        ptx::tmem_relinquish();
+    }
+    if (warp >= 4) {       // rows of the q tile that no TMA box writes (tpt G < 128) stay zero
+        for (int e = tid - 128; e < L::Q_BYTES / 16; e += 128)
+            asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(sbase + (uint32_t)(L::OFF_Q + e * 16)), "r"(0) : "memory");
+        ptx::fence_proxy_async_smem();
+    }
+    ptx::pdl_wait();
+    ptx::pdl_trigger();
+    ptx::tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();            // the peer's barriers exist before anything is multicast to it or arrives on them
+    ptx::tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    if (warp == 0) producer_warp<D>(p, &mapK, &mapV, &mapQ, sbase, items, abort_flag, lane, rank);
+    else if (warp == 1) mma_warp<D>(p, sbase, tmem, items, abort_flag, lane, rank);
+    else if (warp == 2) agent_warp<D>(p, smem, sbase, items, abort_flag, lane, rank);
+    else if (warp >= 4) softmax_warps<D>(p, smem, sbase, tmem, items, abort_flag, warp, lane, rank);
+    ptx::tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();            // neither CTA leaves while the other may still write into it
+    if (tid == 0 && *abort_flag) raise_flag(p.flags, DEV_TIMEOUT);
+    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+}
+
+}  // namespace gqa
+
+static inline cudaError_t gqa_configure(int head_dim) {
+    cudaError_t e;
+    if (head_dim == 128) e = cudaFuncSetAttribute(gqa::gqa_decode_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, gqa::Smem<128>::ALLOC);
+    else e = cudaFuncSetAttribute(gqa::gqa_decode_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, gqa::Smem<64>::ALLOC);
+    return e;
+}
+
+static inline cudaError_t gqa_launch(const DecParams& p, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mq, int head_dim,
+                                     int num_ctas, cudaStream_t stream) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(num_ctas & ~1); cfg.blockDim = dim3(gqa::NTHREADS); cfg.stream = stream;
+    cfg.dynamicSmemBytes = head_dim == 128 ? gqa::Smem<128>::ALLOC : gqa::Smem<64>::ALLOC;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    at[1].id = cudaLaunchAttributeClusterDimension;
+    at[1].val.clusterDim.x = 2; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 2;
+    cudaError_t e = head_dim == 128 ? cudaLaunchKernelEx(&cfg, gqa::gqa_decode_kernel<128>, mk, mv, mq, p)
+                                    : cudaLaunchKernelEx(&cfg, gqa::gqa_decode_kernel<64>, mk, mv, mq, p);
+    if (e != cudaSuccess) return e;
+    return cudaGetLastError();
+}

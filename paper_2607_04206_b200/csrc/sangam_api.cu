@@ -7,9 +7,11 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <algorithm>
 #include <new>
 
 #include "attn_dec.cuh"
+#include "attn_gqa.cuh"
 #include "attn_simt.cuh"
 #include "attn_tc.cuh"
 #include "common.cuh"
@@ -35,6 +37,7 @@ struct sangam_ctx {
     int32_t num_slots;
     // decode kernel (attn_dec.cuh): resident CTAs per SM (0: unavailable), its split-KV workspace
     int dec_occ;
+    int gqa_ok;                   // GQA pair kernel (attn_gqa.cuh) available for this geometry
     int dispatch;                 // SANGAM_DISPATCH_*
     float* d_dec_part_o;
     float* d_dec_part_ml;
@@ -137,16 +140,22 @@ extern "C" int sangam_create(const sangam_config* cfg, sangam_ctx** out) {
 #else
     if (e == cudaSuccess) e = tc_configure(cfg->head_dim);
 #endif
-    if (e == cudaSuccess && ctx->G <= dec::NQ) {
-        // decode kernel: dec_occ CTAs per SM; the flattened weighted unit list must stay below 2^31 coordinates
-        const int64_t worst = (int64_t)cfg->max_total_q * cfg->num_kv_heads * ((int64_t)cfg->max_pages_per_req + dec::OV);
-        ctx->dec_occ = worst < 0x7fffffffLL ? dec_configure(cfg->head_dim) : 0;
-        if (ctx->dec_occ > 0) {
-            const size_t nslots = (size_t)2 * ctx->dec_occ * ctx->sm_count;
-            e = cudaMalloc(&ctx->d_dec_part_o, nslots * dec::NQ * cfg->head_dim * sizeof(float));
-            if (e == cudaSuccess) e = cudaMalloc(&ctx->d_dec_part_ml, nslots * dec::NQ * 2 * sizeof(float));
-            // one arrival counter per work unit: at most Hkv * (rows + requests) units in a batch
-            const size_t ncnt = (size_t)cfg->num_kv_heads * ((size_t)cfg->max_total_q + cfg->max_batch);
+    {
+        // decode kernels (attn_dec.cuh: dec_occ CTAs per SM; attn_gqa.cuh: CTA pairs) share one split-KV workspace; the
+        // flattened weighted unit list must stay below 2^31 coordinates
+        const int64_t worst = (int64_t)cfg->max_total_q * cfg->num_kv_heads * ((int64_t)cfg->max_pages_per_req + 64);
+        if (e == cudaSuccess && worst < 0x7fffffffLL) {
+            if (ctx->G <= dec::NQ) ctx->dec_occ = dec_configure(cfg->head_dim);
+            if (ctx->G > 1 && ctx->G <= 128 && (ctx->sm_count & 1) == 0) ctx->gqa_ok = gqa_configure(cfg->head_dim) == cudaSuccess ? 1 : 0;
+            cudaGetLastError();
+        }
+        if (e == cudaSuccess && (ctx->dec_occ > 0 || ctx->gqa_ok)) {
+            // partial slots: decode kernel 2 per CTA of 32 rows; pair kernel 2 per CTA of 128 rows
+            const size_t o_floats = std::max((size_t)2 * ctx->dec_occ * ctx->sm_count * dec::NQ, ctx->gqa_ok ? (size_t)2 * ctx->sm_count * gqa::BM : 0) * cfg->head_dim;
+            e = cudaMalloc(&ctx->d_dec_part_o, o_floats * sizeof(float));
+            if (e == cudaSuccess) e = cudaMalloc(&ctx->d_dec_part_ml, o_floats / cfg->head_dim * 2 * sizeof(float));
+            // arrival counters: one per work unit (two for the pair kernel): at most Hkv * (rows + requests) units in a batch
+            const size_t ncnt = (size_t)2 * cfg->num_kv_heads * ((size_t)cfg->max_total_q + cfg->max_batch);
             if (e == cudaSuccess) e = cudaMalloc(&ctx->d_dec_cnt, ncnt * sizeof(int32_t));
             if (e == cudaSuccess) e = cudaMemset(ctx->d_dec_cnt, 0, ncnt * sizeof(int32_t));
         }
@@ -389,32 +398,42 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
     // compute the same function for any batch; the choice only affects speed.  Lengths live on the device, so the
     // host decides on the counts it knows: total_q and batch.
     bool use_dec = ctx->dec_occ > 0 && (int64_t)total_q * ctx->G <= (int64_t)dec::NQ * batch;
-    if (ctx->dispatch == SANGAM_DISPATCH_PREFILL) use_dec = false;
+    // GQA models: block decodes of up to two 128-row q tiles per kv head go to the CTA-pair kernel
+    const int tpt = 128 / ctx->G;
+    bool use_gqa = !use_dec && ctx->gqa_ok && (int64_t)total_q <= (int64_t)2 * tpt * batch;
+    if (ctx->dispatch == SANGAM_DISPATCH_PREFILL) { use_dec = false; use_gqa = false; }
     if (ctx->dispatch == SANGAM_DISPATCH_DECODE) {
         if (ctx->dec_occ <= 0) return fail(ctx, SANGAM_ERR_UNSUPPORTED, "block_attn: the decode kernel is not available for this geometry");
-        use_dec = true;
+        use_dec = true; use_gqa = false;
     }
-    if (use_dec) {
+    if (ctx->dispatch == SANGAM_DISPATCH_GQA_PAIR) {
+        if (!ctx->gqa_ok) return fail(ctx, SANGAM_ERR_UNSUPPORTED, "block_attn: the GQA pair kernel is not available for this geometry");
+        use_gqa = true; use_dec = false;
+    }
+    if (use_dec || use_gqa) {
         DecParams d = {};
         d.block_table = block_table; d.cu_q_lens = cu_q_lens; d.ctx_lens = ctx_lens;
         d.out = (__nv_bfloat16*)out;
         d.batch = batch; d.total_q = total_q;
         d.Hq = c.num_q_heads; d.Hkv = c.num_kv_heads; d.G = ctx->G; d.W = c.max_pages_per_req; d.P = c.num_pages;
-        d.tq = dec::NQ / ctx->G;
+        d.tpt = tpt;
+        d.tq = use_gqa ? 2 * tpt : dec::NQ / ctx->G;
         d.tq_magic = (uint32_t)(0x100000000ull / (uint64_t)d.tq) + 1u;
         d.g_magic = (uint32_t)(0x100000000ull / (uint64_t)ctx->G) + 1u;
         d.scale_log2 = scale * 1.4426950408889634f;
 #ifdef SANGAM_TRACE
         { unsigned int v = 0; cudaMemcpyFromSymbol(&v, g_trace_cta, sizeof v); d.trace_cta = (int)v; }
 #endif
-        d.part_o = ctx->d_dec_part_o; d.part_ml = ctx->d_dec_part_ml; d.unit_cnt = ctx->d_dec_cnt; d.min_w = dec::MIN_W; d.ov = dec::OV;
+        d.part_o = ctx->d_dec_part_o; d.part_ml = ctx->d_dec_part_ml; d.unit_cnt = ctx->d_dec_cnt;
+        d.min_w = use_gqa ? gqa::MIN_W : dec::MIN_W; d.ov = use_gqa ? gqa::OV : dec::OV;
 #ifdef SANGAM_TUNING_ENV
         if (const char* e_ = getenv("SANGAM_DEC_OV")) d.ov = atoi(e_);
         if (const char* e_ = getenv("SANGAM_DEC_MINW")) d.min_w = atoi(e_);
 #endif
         d.flags = ctx->d_flags;
-        cudaError_t e = dec_launch(d, kv->mk, kv->mv, qm->dec, c.head_dim, ctx->dec_occ * ctx->sm_count, (cudaStream_t)stream);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "block_attn launch (decode kernel)");
+        cudaError_t e = use_gqa ? gqa_launch(d, kv->mk, kv->mv, qm->main, c.head_dim, ctx->sm_count, (cudaStream_t)stream)
+                                : dec_launch(d, kv->mk, kv->mv, qm->dec, c.head_dim, ctx->dec_occ * ctx->sm_count, (cudaStream_t)stream);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, use_gqa ? "block_attn launch (GQA pair kernel)" : "block_attn launch (decode kernel)");
         ctx->launches += 1;
         return SANGAM_OK;
     }
@@ -432,14 +451,17 @@ extern "C" int32_t sangam_query(const sangam_ctx* ctx, int32_t what) {
         case SANGAM_QUERY_SM_COUNT: return ctx->sm_count;
         case SANGAM_QUERY_DECODE_CTAS_PER_SM: return ctx->dec_occ;
         case SANGAM_QUERY_DISPATCH: return ctx->dispatch;
+        case SANGAM_QUERY_GQA_PAIR_KERNEL: return ctx->gqa_ok;
         default: return -1;
     }
 }
 
 extern "C" int sangam_set_dispatch(sangam_ctx* ctx, int32_t mode) {
     if (!ctx) return SANGAM_ERR_INVALID_ARG;
-    if (mode != SANGAM_DISPATCH_AUTO && mode != SANGAM_DISPATCH_PREFILL && mode != SANGAM_DISPATCH_DECODE)
+    if (mode != SANGAM_DISPATCH_AUTO && mode != SANGAM_DISPATCH_PREFILL && mode != SANGAM_DISPATCH_DECODE && mode != SANGAM_DISPATCH_GQA_PAIR)
         return fail(ctx, SANGAM_ERR_INVALID_ARG, "set_dispatch: unknown mode");
+    if (mode == SANGAM_DISPATCH_GQA_PAIR && !ctx->gqa_ok)
+        return fail(ctx, SANGAM_ERR_UNSUPPORTED, "set_dispatch: the GQA pair kernel is not available for this geometry");
     if (mode == SANGAM_DISPATCH_DECODE && ctx->dec_occ <= 0)
         return fail(ctx, SANGAM_ERR_UNSUPPORTED, "set_dispatch: the decode kernel is not available for this geometry");
     ctx->dispatch = mode;
