@@ -155,6 +155,9 @@ def _i32(a, device):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.int32)).to(device)
 
 
+DISPATCH = 0          # sangam_set_dispatch mode of every engine this run creates (--dispatch; 0 = the library's own choice)
+
+
 class Workload:
     """A Batch resident in HBM: `nsets` independent (pools, q, k_new, v_new, out) sets + shared metadata."""
 
@@ -166,6 +169,8 @@ class Workload:
         self.eng = sg.Sangam(num_q_heads=b.num_q_heads, num_kv_heads=b.num_kv_heads, head_dim=b.head_dim,
                              num_pages=b.num_pages, max_batch=b.batch, max_total_q=max(b.total_q, len(b.slot_new), 1),
                              max_pages_per_req=b.max_pages_per_req, device=dev_index)
+        if DISPATCH:
+            self.eng.set_dispatch(DISPATCH)
         device = f"cuda:{dev_index}"
         self.device = device
         self.block_table, self.cu_q_lens, self.ctx_lens = _i32(b.block_table, device), _i32(b.cu_q_lens, device), _i32(b.ctx_lens, device)
@@ -446,6 +451,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=200)
     ap.add_argument("--workload", default="2", help="BASELINE.json config 1..5 or a variant name (sangam_inputs.VARIANTS)")
     ap.add_argument("--no-extras", action="store_true", help="skip variants, the Fig.-3 sweep and the scheduler series")
+    ap.add_argument("--dispatch", default="auto", choices=["auto", "prefill", "decode", "gqa_pair"],
+                    help="attention kernel sangam_block_attn launches (sangam_set_dispatch); auto = the library's own choice")
     ap.add_argument("--impl", default="sangam", choices=["sangam", "reference"])
     ap.add_argument("--all-configs", dest="all_configs", action="store_true", default=None)
     ap.add_argument("--no-all-configs", dest="all_configs", action="store_false")
@@ -455,6 +462,8 @@ def main():
         return run_reference(args)
 
     import torch
+    global DISPATCH
+    DISPATCH = {"auto": 0, "prefill": 1, "decode": 2, "gqa_pair": 3}[args.dispatch]
     rank, world, dist = dist_setup()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (the sangam kernels have no CPU fallback)")
@@ -519,7 +528,7 @@ def main():
             "dtype": "bf16", "data": "synthetic",
             "config": {"workload": wname, "batch": b.batch, "total_q": b.total_q,
                        "sum_ctx": int(b.ctx_lens.sum()), "heads": f"{b.num_q_heads}/{b.num_kv_heads}",
-                       "head_dim": b.head_dim, "page": si.PAGE, "parallelism": f"replicas x{world}",
+                       "head_dim": b.head_dim, "page": si.PAGE, "parallelism": f"replicas x{world}", "dispatch": args.dispatch,
                        "l2": f"cold: steps rotate over {w.nsets} independent pool sets "
                              f"({w.nsets * b.attn_bytes() / 1e6:.0f} MB distinct per rotation)",
                        "step": "CUDA-graph replay of kv_write + block_attn (device-side plan + tcgen05 attention + split-KV merge)"},

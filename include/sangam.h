@@ -153,15 +153,17 @@ int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_pages, const
 /*
  * Kernel choice of sangam_block_attn.  AUTO (default): decode-shaped batches (total_q * G <= 32 * batch, i.e. on
  * average at most one 32-row unit per request and kv head -- block decodes, block 32) run
- * the swapped-operand decode kernel, everything else the two-stream prefill / hybrid kernel.  Both kernels compute
- * the same function for every batch; PREFILL / DECODE force one of them (tests, measurements).  DECODE returns
- * SANGAM_ERR_UNSUPPORTED for geometries the decode kernel is not built for (num_q_heads / num_kv_heads > 32).
+ * the swapped-operand decode kernel, everything else the two-stream prefill / hybrid kernel.  All kernels compute
+ * the same function for every batch they accept; PREFILL / DECODE / GQA_PAIR force one of them (tests, measurements).
+ * DECODE returns SANGAM_ERR_UNSUPPORTED for geometries the decode kernel is not built for (num_q_heads /
+ * num_kv_heads > 32), GQA_PAIR for MHA (G = 1) and G > 128.  GQA_PAIR is the CTA-pair decode kernel of GQA models
+ * (two SMs share every K/V tile through TMA multicast, each computes one 128-row q tile of the request's block); AUTO
+ * never picks it: on the Dream-like shapes it is measured slower than the two-stream kernel.
  */
 #define SANGAM_DISPATCH_AUTO    0
 #define SANGAM_DISPATCH_PREFILL 1
 #define SANGAM_DISPATCH_DECODE  2
-#define SANGAM_DISPATCH_GQA_PAIR 3   /* the CTA-pair decode kernel of GQA models (AUTO picks it for block decodes of up to
-                                        2 * floor(128 / G) tokens per request on average, 1 < G <= 128) */
+#define SANGAM_DISPATCH_GQA_PAIR 3
 int sangam_set_dispatch(sangam_ctx* ctx, int32_t mode);
 
 /* Read-only facts about a ctx (host side, no device work); -1 for an unknown `what`. */

@@ -57,17 +57,22 @@ struct DecParams {
 namespace dec {
 
 #ifdef SANGAM_TRACE
-__device__ __forceinline__ void dtrace(const DecParams& p, unsigned ev) {
+// debug builds: per-warp event trace of one CTA; the event index lives in a register of the role function (DT_DECL), so an
+// event costs one clock read and one store
+__device__ __forceinline__ void dtrace(const DecParams& p, unsigned ev, unsigned& i) {
     if ((int)blockIdx.x == p.trace_cta && (threadIdx.x & 31) == 0) {
         unsigned long long t;
         asm volatile("mov.u64 %0, %%clock64;" : "=l"(t));
-        const unsigned w = threadIdx.x >> 5, i = g_trace_n[w];
-        g_trace_n[w] = i + 1;
+        const unsigned w = threadIdx.x >> 5;
         if (i < SANGAM_TRACE_CAP) g_trace[w * SANGAM_TRACE_CAP + i] = (t << 16) | ((unsigned long long)w << 8) | ev;
+        ++i;
+        g_trace_n[w] = i;
     }
 }
-#define DT(ev) dtrace(p, ev)
+#define DT_DECL unsigned dt_i_ = 0
+#define DT(ev) dtrace(p, ev, dt_i_)
 #else
+#define DT_DECL [[maybe_unused]] unsigned dt_i_ = 0
 #define DT(ev) ((void)0)
 #endif
 
@@ -334,6 +339,7 @@ __device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensor
     const unsigned FULL = 0xffffffffu;
     const int NC = gridDim.x, b = blockIdx.x;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    DT_DECL;
     DT(1);
     Planner plan;
     plan.init(p, lane, NC, b);
@@ -438,6 +444,7 @@ template <int D>
 __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uint32_t tmem, const Item* items,
                                          volatile uint32_t* abort_flag, int lane) {
     using L = Smem<D>;
+    DT_DECL;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
     const uint64_t k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, KV_ATOM_STRIDE<D>);      // A, K-major (kv rows x d)
     const uint64_t v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 1024, KV_ATOM_STRIDE<D>);    // A, MN-major (d x kv)
@@ -535,6 +542,7 @@ template <int D>
 __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem, uint32_t sbase, uint32_t tmem, const Item* items,
                                               volatile uint32_t* abort_flag, int warp, int lane) {
     using L = Smem<D>;
+    DT_DECL;
     const unsigned FULL = 0xffffffffu;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
     const int qd = warp & 3, jl = qd * 32 + lane;
@@ -953,7 +961,6 @@ decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ 
     volatile uint32_t* abort_flag = reinterpret_cast<volatile uint32_t*>(smem + L::OFF_ABORT);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     TRACE_CTA(0);
-    DT(40);
     if (tid == 0) {
         auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
         for (int s = 0; s < NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 1); }
@@ -986,13 +993,11 @@ decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ 
     const bool base_ok = (sbase & 1023u) == 0u;               // the layout relies on a 1024-byte aligned base
     if (!base_ok && tid == 0) raise_flag(p.flags, DEV_INTERNAL | 0x800u);
     auto start = [&]() {                                      // executed by every warp, once, in its own branch
-        DT(41);
         ptx::pdl_wait();
         ptx::pdl_trigger();
         ptx::tc_fence_before();
         ptx::bar_sync(0, NTHREADS);
         ptx::tc_fence_after();
-        DT(43);
         return *tmem_slot;
     };
     uint32_t tmem;
@@ -1007,10 +1012,8 @@ decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ 
         else if (base_ok && warp == 1) mma_warp<D>(p, sbase, tmem, items, abort_flag, lane);
         else if (base_ok && warp == 2) agent_warp<D>(p, smem, sbase, items, abort_flag, lane);
     }
-    DT(44);
     ptx::tc_fence_before();
     __syncthreads();
-    DT(45);
     TRACE_CTA(1);
     if (tid == 0 && *abort_flag) raise_flag(p.flags, DEV_TIMEOUT);
     if (warp == 1) ptx::tmem_dealloc(tmem, 64);

@@ -9,9 +9,12 @@
 // leaves one 128x128 QK^T, one PV and 16 K exponentials against 32 KB of HBM traffic: every pipe has slack again and
 // HBM is the only bound.
 //
-// Per CTA: 256 threads; warp 0 = device-side plan (a3) + TMA producer (a4), 1 = MMA issuer (a5, a7), 2 = arrival agent of
-// split units, 4..7 = softmax (a6: thread i owns row i of the CTA's q tile), epilogue (a8) and the fused split-KV merge
-// (a9).  Work unit = (request, kv head, pair of q tiles); the flattened (unit, page) list is cut into one contiguous range
+// Per CTA: 384 threads; warp 0 = device-side plan (a3) + TMA producer (a4), 1 = MMA issuer (a5, a7), 2 = arrival agent of
+// split units, 4..7 and 8..11 = two softmax warpgroups (a6: thread i of a group owns row i of the CTA's q tile).  The kv
+// tiles of a unit alternate between the groups (stream b takes the tiles of parity b, with its own S buffer, its own
+// running (max, sum) and its own O accumulator in TMEM; the two partial results are merged in the epilogue): one warp
+// per SM sub-partition cannot hide the TMEM / MUFU latencies of a tile's 128 exponentials per row, two can.  Group 0
+// also runs the epilogue (a8) and the fused split-KV merge (a9).  Work unit = (request, kv head, pair of q tiles); the flattened (unit, page) list is cut into one contiguous range
 // per CLUSTER (stream-K, the planner of attn_dec.cuh); both CTAs of a cluster derive the same plan and walk it in
 // lockstep (a K/V stage is refilled only after both CTAs released it).  Pieces of split units are merged by the piece
 // that arrives last, as in attn_dec.cuh.
@@ -28,11 +31,15 @@ using dec::Deferred;
 using dec::Item;
 using dec::OutRef;
 using dec::Planner;
+#ifdef SANGAM_TRACE
+using dec::dtrace;
+#endif
 
 constexpr int BM = 128;          // rows of a q tile (UMMA M)
 constexpr int BN = 128;          // kv positions per tile (8 pages)
-constexpr int NSTAGE = 5;        // ring of K / V tiles
-constexpr int NTHREADS = 256;
+constexpr int NSTAGE = 3;        // stages of the K ring and of the V ring (separate rings: a V tile waits for its
+                                 // softmax much longer than a K tile for its QK, and must not hold up the K loads)
+constexpr int NTHREADS = 384;
 constexpr int SLAB = 128 * 128;  // bytes of one 64-wide swizzled slab of the q tile
 constexpr float LAZY_T = 8.f;
 #ifndef SANGAM_GQA_OV
@@ -46,19 +53,20 @@ template <int D>
 struct Smem {
     static constexpr int KV_BYTES = BN * D * 2;
     static constexpr int Q_BYTES = BM * D * 2;
-    static constexpr int OFF_KV = 0;
-    static constexpr int OFF_Q = NSTAGE * KV_BYTES;
+    static constexpr int OFF_KV = 0;                     // stages 0 .. NSTAGE-1: K ring, NSTAGE .. 2 NSTAGE-1: V ring
+    static constexpr int OFF_Q = 2 * NSTAGE * KV_BYTES;
     static constexpr int OFF_BAR = OFF_Q + Q_BYTES;
-    static constexpr int B_KV_FULL = 0, B_KV_EMPTY = NSTAGE, B_ITEM_FULL = 2 * NSTAGE, B_ITEM_EMPTY = B_ITEM_FULL + 2,
-                         B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 1, B_S_FULL = B_Q_EMPTY + 1 /* [2] */,
-                         B_P_FULL = B_S_FULL + 2, B_PV_DONE = B_P_FULL + 1 /* [2] */, B_O_FREE = B_PV_DONE + 2,
-                         B_AGENT_REQ = B_O_FREE + 1, B_AGENT_DONE = B_AGENT_REQ + 1, NBAR = B_AGENT_DONE + 1;
+    static constexpr int B_KV_FULL = 0, B_KV_EMPTY = 2 * NSTAGE, B_ITEM_FULL = 4 * NSTAGE, B_ITEM_EMPTY = B_ITEM_FULL + 2,
+                         B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 1, B_S_FULL = B_Q_EMPTY + 1 /* [stream] */,
+                         B_P_FULL = B_S_FULL + 2 /* [stream] */, B_PV_DONE = B_P_FULL + 2 /* [stream] */, B_O_FREE = B_PV_DONE + 2 /* [stream] */,
+                         B_EPI = B_O_FREE + 2 /* [item slot] */, B_AGENT_REQ = B_EPI + 2, B_AGENT_DONE = B_AGENT_REQ + 1, NBAR = B_AGENT_DONE + 1;
     static constexpr int OFF_ITEMS = OFF_BAR + ((NBAR * 8 + 15) / 16) * 16;
+    static constexpr int OFF_ML = OFF_ITEMS + 2 * (int)sizeof(Item);     // [2 item slots][128 rows] (m, l) of stream 1
     // misc block: +0 tmem slot, +8 merge flag, +16 agent_req[2], +32 Deferred[2], +96 abort word (+ wait table in debug builds)
-    static constexpr int OFF_MISC = OFF_ITEMS + 2 * (int)sizeof(Item);
+    static constexpr int OFF_MISC = OFF_ML + 2 * BM * 8;
     static constexpr int OFF_ABORT = OFF_MISC + 96;
     static constexpr int TOTAL = OFF_ABORT + 80;
-    static constexpr int ALLOC = TOTAL + 1024;           // slack to align the base to 1024 B
+    static constexpr int ALLOC = TOTAL;                  // no alignment slack: the dynamic base is 1024-byte aligned (checked at run time)
 };
 static_assert(Smem<128>::ALLOC <= 232448, "shared memory budget (227 KB)");
 
@@ -87,15 +95,55 @@ __device__ __forceinline__ void tma_load_4d_mc(uint32_t dst_smem, const CUtensor
 // ------------------------------------------------------------------------------------------------
 // warp 0: plan + TMA (this CTA's half of every tile's pages, multicast to the pair) + its q tile
 // ------------------------------------------------------------------------------------------------
+// One unit's kv tiles of one ring (K or V), this CTA's half of every tile multicast to both CTAs of the pair.
+// Page ids come in 64-page windows, lane l holding entries l and 32 + l; the window after the current one is requested when
+// the current one is entered, eight tiles before it is needed: no load waits on a block-table read except the unit's first.
 template <int D>
-__device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensorMap* mapK, const CUtensorMap* mapV, const CUtensorMap* mapQ,
-                                              uint32_t sbase, Item* items, volatile uint32_t* abort_flag, int lane, uint32_t rank) {
+__device__ __forceinline__ void load_tiles(const DecParams& p, const CUtensorMap* map, uint32_t sbase, const Item& it, uint32_t rank, int lane,
+                                           uint32_t ring0, uint32_t& st, uint32_t& ph, volatile uint32_t* abort_flag, [[maybe_unused]] unsigned& dt_i_) {
     using L = Smem<D>;
     const unsigned FULL = 0xffffffffu;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    const int npg = it.pg1 - it.pg0, nt = (npg + 7) >> 3;
+    const int32_t* bt = p.block_table + (int64_t)it.r * p.W + it.pg0;
+    auto ld_win = [&](int w, int half) { const int e = 64 * w + 32 * half + lane; return e < npg ? __ldg(bt + e) : 0; };
+    int clo = ld_win(0, 0), chi = ld_win(0, 1), nlo = ld_win(1, 0), nhi = ld_win(1, 1);
+    const bool my_lane = (lane >> 2) == (int)rank && lane < 8;                // pages 0..3 of a tile: CTA 0, pages 4..7: CTA 1
+    const uint32_t dst0 = sbase + (uint32_t)(L::OFF_KV + lane * (2 * KV_ATOM_STRIDE<D>));
+    for (int t = 0; t < nt; ++t) {
+        const int tw = t & 7;
+        if (tw == 0 && t > 0) { clo = nlo; chi = nhi; nlo = ld_win((t >> 3) + 1, 0); nhi = ld_win((t >> 3) + 1, 1); }
+        const int src = (8 * tw + lane) & 31;
+        const int xlo = __shfl_sync(FULL, clo, src), xhi = __shfl_sync(FULL, chi, src);
+        int page = tw < 4 ? xlo : xhi;
+        int np = npg - 8 * t;
+        np = np > 8 ? 8 : np;
+        const bool mine = my_lane && lane < np;
+        if (mine && (unsigned)page >= (unsigned)p.P) { raise_flag(p.flags, DEV_BAD_PAGE); page = p.P; }
+        const uint32_t stage = ring0 + st;
+        DT((ring0 ? 200 : 180) + (t & 15));
+        ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), ph ^ 1u, abort_flag);      // both CTAs have released the stage
+        if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_KV_FULL + stage), (uint32_t)(np * SANGAM_PAGE * D * 2));
+        __syncwarp();
+        if (mine) tma_load_4d_mc(dst0 + stage * L::KV_BYTES, map, bar(L::B_KV_FULL + stage), (page * p.Hkv + it.g) * 2, (uint16_t)3);
+        if (++st == NSTAGE) { st = 0; ph ^= 1u; }
+        DT((ring0 ? 120 : 100) + (t & 15));
+        if (*abort_flag) break;
+    }
+}
+
+// warp 0: device-side plan (a3), Q loads, the K ring
+template <int D>
+__device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensorMap* mapK, const CUtensorMap* mapQ, uint32_t sbase, Item* items,
+                                              volatile uint32_t* abort_flag, int lane, uint32_t rank) {
+    using L = Smem<D>;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    DT_DECL;
+    DT(1);
     Planner plan;
     plan.init(p, lane, (int)gridDim.x >> 1, (int)blockIdx.x >> 1);
-    uint32_t stage = 0, phase = 0, icount = 0, qcount = 0;
+    DT(2);
+    uint32_t kst = 0, kph = 0, icount = 0, qcount = 0;
     while (true) {
         if (*abort_flag) break;
         Item it;
@@ -109,14 +157,7 @@ __device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensor
         __syncwarp();
         ++icount;
         if (!it.valid) break;
-        const int npg = it.pg1 - it.pg0;
-        if (npg <= 0) continue;
-        const int32_t* bt = p.block_table + (int64_t)it.r * p.W + it.pg0;
-        const int nt = (npg + 7) >> 3;
-        // page ids: lane pg (< 8) keeps page pg of the tiles in flight in a 4-entry window indexed by tile & 3 (K runs at most
-        // two tiles ahead of V); the ids of tile kq + 1 are requested when K(kq) is issued
-        auto ld_ids = [&](int t) { return (t < nt && lane < 8 && 8 * t + lane < npg) ? __ldg(bt + 8 * t + lane) : 0; };
-        int w0 = ld_ids(0), w1 = ld_ids(1), w2 = 0, w3 = 0;
+        if (it.pg1 - it.pg0 <= 0) continue;
         const int ntok_c = it.ntok - (int)rank * p.tpt;                       // tokens of this CTA's q tile
         if (ntok_c > 0) {
             ptx::mbar_wait(bar(L::B_Q_EMPTY), (qcount & 1u) ^ 1u, abort_flag);
@@ -127,58 +168,63 @@ __device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensor
                                  it.q_start + it.tok0 + (int)rank * p.tpt);
             ++qcount;
         }
-        // ring order K(0) K(1) V(0) K(2) V(1) ...: the issuer runs QK one tile ahead of PV
-        int kq = 0, vq = 0;
-        while (vq < nt) {
-            const bool is_v = !(kq < nt && kq <= vq + 1);
-            const int t = is_v ? vq : kq;
-            const int sel = t & 3;
-            int page = sel == 0 ? w0 : sel == 1 ? w1 : sel == 2 ? w2 : w3;
-            int np = npg - 8 * t;
-            np = np > 8 ? 8 : np;
-            const bool mine = lane < np && (lane >> 2) == (int)rank;              // pages 0..3: CTA 0, pages 4..7: CTA 1
-            if (mine && (unsigned)page >= (unsigned)p.P) { raise_flag(p.flags, DEV_BAD_PAGE); page = p.P; }
-            ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), phase ^ 1u, abort_flag);   // both CTAs have released the stage
-            if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_KV_FULL + stage), (uint32_t)(np * SANGAM_PAGE * D * 2));
-            __syncwarp();
-            if (mine)
-                tma_load_4d_mc(sbase + (uint32_t)(L::OFF_KV + stage * L::KV_BYTES + lane * (2 * KV_ATOM_STRIDE<D>)), is_v ? mapV : mapK,
-                               bar(L::B_KV_FULL + stage), (page * p.Hkv + it.g) * 2, (uint16_t)3);
-            if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
-            if (is_v) {
-                ++vq;
-            } else {
-                ++kq;
-                const int nx = ld_ids(kq + 1), s2 = (kq + 1) & 3;
-                if (s2 == 0) w0 = nx; else if (s2 == 1) w1 = nx; else if (s2 == 2) w2 = nx; else w3 = nx;
-            }
-            if (*abort_flag) break;
-        }
+        load_tiles<D>(p, mapK, sbase, it, rank, lane, 0u, kst, kph, abort_flag, dt_i_);
     }
     for (int k = 0; k < NSTAGE; ++k) {      // every commit aimed at this CTA's barriers has landed before it may exit
-        ptx::mbar_wait(bar(L::B_KV_EMPTY + stage), phase ^ 1u, abort_flag);
-        if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+        ptx::mbar_wait(bar(L::B_KV_EMPTY + kst), kph ^ 1u, abort_flag);
+        if (++kst == NSTAGE) { kst = 0; kph ^= 1u; }
     }
     ptx::mbar_wait(bar(L::B_Q_EMPTY), (qcount & 1u) ^ 1u, abort_flag);
 }
 
+// warp 3: the V ring (a ring and an issuing warp of its own: a V tile is needed a whole softmax later than its K tile, and one
+// warp's instruction stream cannot issue both rings at the rate HBM delivers them)
+template <int D>
+__device__ __forceinline__ void v_producer_warp(const DecParams& p, const CUtensorMap* mapV, uint32_t sbase, const Item* items,
+                                                volatile uint32_t* abort_flag, int lane, uint32_t rank) {
+    using L = Smem<D>;
+    auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    DT_DECL;
+    uint32_t vst = 0, vph = 0, icount = 0;
+    while (true) {
+        if (*abort_flag) break;
+        const uint32_t islot = icount & 1u;
+        ptx::mbar_wait(bar(L::B_ITEM_FULL + islot), (icount >> 1) & 1u, abort_flag);
+        const Item it = items[islot];
+        if (!it.valid) break;
+        if (it.pg1 - it.pg0 > 0) {
+            load_tiles<D>(p, mapV, sbase, it, rank, lane, (uint32_t)NSTAGE, vst, vph, abort_flag, dt_i_);
+        }
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
+        ++icount;
+    }
+    for (int k = 0; k < NSTAGE; ++k) {
+        ptx::mbar_wait(bar(L::B_KV_EMPTY + NSTAGE + vst), vph ^ 1u, abort_flag);
+        if (++vst == NSTAGE) { vst = 0; vph ^= 1u; }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
-// warp 1: MMA issuer.  S[b] = Q K(j)^T into TMEM buffer b = j & 1 (128 columns), O += P(j) V(j) with P read from TMEM
-// (bf16, packed over the first 32 columns of each 64-column half of S[b]).  QK runs one tile ahead of PV.
-// TMEM: S[0] = columns [0, 128), S[1] = [128, 256), O = [256, 256 + D).
+// warp 1: MMA issuer.  Global kv tile k belongs to stream b = k & 1:  S[b] = Q K(k)^T (128 TMEM columns),
+// O[b] += P(k) V(k) with P read from TMEM (bf16, packed over the first 32 columns of each 64-column half of S[b]).
+// QK runs one tile ahead of PV, so the two streams' softmax groups always have a tile each.
+// TMEM: S[0] = columns [0, 128), S[1] = [128, 256), O[0] = [256, 256 + D), O[1] = [384, 384 + D).
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uint32_t tmem, const Item* items, volatile uint32_t* abort_flag,
                                          int lane, uint32_t rank) {
     using L = Smem<D>;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    DT_DECL;
     const uint64_t q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);
     const uint64_t k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, KV_ATOM_STRIDE<D>);
     const uint64_t v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 1024, KV_ATOM_STRIDE<D>);
     constexpr uint32_t VSTEP = (uint32_t)(2 * KV_ATOM_STRIDE<D>) >> 4;
     constexpr uint32_t IDESC_PV = ptx::idesc_bf16(BM, D, 0, 1);
     const uint32_t peer = rank ^ 1u;
-    uint32_t stage = 0, phase = 0, icount = 0, qcount = 0, tcount = 0, ocount = 0;
+    uint32_t kst = 0, kph = 0, vst = 0, vph = 0, icount = 0, qcount = 0, tcount = 0;
+    uint32_t ocount[2] = {0, 0};             // units in which stream b accumulated (O_FREE[b] phases)
     auto release = [&](uint32_t s) {         // this CTA is done with stage s: tell both producers of the pair
         ptx::mma_commit(bar(L::B_KV_EMPTY + s));
         ptx::mma_commit(peer_addr(bar(L::B_KV_EMPTY + s), peer));
@@ -196,10 +242,11 @@ __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uin
             auto nv_of = [&](int t) { int nv = c_lim - (it.pg0 + 8 * t) * SANGAM_PAGE; return nv > BN ? BN : nv; };
             if (active) { ptx::mbar_wait(bar(L::B_Q_FULL), qcount & 1u, abort_flag); ++qcount; }
             auto issue_qk = [&](int t) {
-                const uint32_t sk = stage;
-                ptx::mbar_wait(bar(L::B_KV_FULL + sk), phase, abort_flag);
-                if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+                const uint32_t sk = kst;
+                ptx::mbar_wait(bar(L::B_KV_FULL + sk), kph, abort_flag);
+                if (++kst == NSTAGE) { kst = 0; kph ^= 1u; }
                 ptx::tc_fence_after();
+                DT(140 + (t & 15));
                 if (ptx::elect_one()) {
                     if (active) {
                         const int ncol = (nv_of(t) + 15) & ~15;
@@ -221,28 +268,33 @@ __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uin
             for (int j = 0; j < nt; ++j) {
                 if (*abort_flag) break;
                 if (j + 1 < nt) issue_qk(j + 1);
-                const uint32_t sv = stage;
-                ptx::mbar_wait(bar(L::B_KV_FULL + sv), phase, abort_flag);
-                if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+                const uint32_t sv = NSTAGE + vst;
+                ptx::mbar_wait(bar(L::B_KV_FULL + sv), vph, abort_flag);
+                if (++vst == NSTAGE) { vst = 0; vph ^= 1u; }
+                DT(160 + (j & 15));
                 const int nv = nv_of(j);
                 if (active) {
                     if (nv & 15) dec::zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
-                    if (j == 0 && ocount > 0) ptx::mbar_wait(bar(L::B_O_FREE), (ocount - 1u) & 1u, abort_flag);
-                    ptx::mbar_wait(bar(L::B_P_FULL), (tcount + (uint32_t)j) & 1u, abort_flag);
+                    const uint32_t k = tcount + (uint32_t)j, sb = k & 1u;
+                    // the first PV of stream sb in this unit overwrites O[sb]: the previous unit's epilogue has read it
+                    if (j < 2 && ocount[sb] > 0) ptx::mbar_wait(bar(L::B_O_FREE + sb), (ocount[sb] - 1u) & 1u, abort_flag);
+                    ptx::mbar_wait(bar(L::B_P_FULL + sb), (k >> 1) & 1u, abort_flag);
                 }
                 ptx::tc_fence_after();
+                DT(11);
                 if (ptx::elect_one()) {
                     if (active) {
-                        const uint32_t s_tmem = tmem + (uint32_t)(((tcount + (uint32_t)j) & 1u) * 128u), o_tmem = tmem + 256u;
+                        const uint32_t sb = (tcount + (uint32_t)j) & 1u;
+                        const uint32_t s_tmem = tmem + sb * 128u, o_tmem = tmem + 256u + sb * 128u;
                         const uint64_t b0 = v_desc0 + (uint64_t)(sv * (L::KV_BYTES >> 4));
                         const int ks_n = (nv + 15) >> 4;                       // one K-step = 16 kv rows = one page
                         if (ks_n == 8) {
-                            ptx::mma_ts_x4(o_tmem, s_tmem, b0, IDESC_PV, j > 0 ? 1u : 0u, VSTEP);
+                            ptx::mma_ts_x4(o_tmem, s_tmem, b0, IDESC_PV, j > 1 ? 1u : 0u, VSTEP);
                             ptx::mma_ts_x4(o_tmem, s_tmem + 64u, b0 + 4 * VSTEP, IDESC_PV, 1u, VSTEP);
                         } else {
                             for (int ks = 0; ks < ks_n; ++ks)       // P of page ks: half ks / 4, 8 packed columns per page inside the half
                                 ptx::mma_ts(o_tmem, s_tmem + (uint32_t)((ks >> 2) * 64 + (ks & 3) * 8), b0 + (uint64_t)(ks * VSTEP), IDESC_PV,
-                                            (j > 0 || ks > 0) ? 1u : 0u);
+                                            (j > 1 || ks > 0) ? 1u : 0u);
                         }
                     }
                     release(sv);
@@ -250,7 +302,10 @@ __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uin
                 }
                 __syncwarp();
             }
-            if (active) { tcount += (uint32_t)nt; ++ocount; }
+            if (active) {
+                if (nt >= 2) { ++ocount[0]; ++ocount[1]; } else { ++ocount[tcount & 1u]; }
+                tcount += (uint32_t)nt;
+            }
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
@@ -259,7 +314,8 @@ __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uin
 }
 
 // ------------------------------------------------------------------------------------------------
-// warps 4..7: softmax (thread `row` owns row `row` of the CTA's q tile = TMEM lane `row`), epilogue, merge
+// warps 4..7 (group 0) and 8..11 (group 1): softmax; thread `row` of a group owns row `row` of the CTA's q tile (TMEM lane
+// `row`).  Group b processes the kv tiles of global parity b.  Group 0 then merges the two streams and runs the epilogue.
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem, uint32_t sbase, uint32_t tmem, const Item* items,
@@ -267,13 +323,18 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
     using L = Smem<D>;
     const unsigned FULL = 0xffffffffu;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
+    DT_DECL;
+    const uint32_t wg = (uint32_t)(warp - 4) >> 2;             // stream of this group
     const int qd = warp & 3, row = qd * 32 + lane;
     const uint32_t lane_base = (uint32_t)(qd * 32) << 16;
-    const uint32_t o_taddr = tmem + lane_base + 256u;
+    const uint32_t s_taddr = tmem + lane_base + wg * 128u;     // S[wg]
+    const uint32_t o_taddr = tmem + lane_base + 256u + wg * 128u;   // O[wg]
+    const uint32_t o0_taddr = tmem + lane_base + 256u, o1_taddr = tmem + lane_base + 384u;
+    float2* ml_x = reinterpret_cast<float2*>(smem + L::OFF_ML);
     volatile int* merge_flag = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 8);
     volatile int* agent_req = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 16);
     const float sc = fabsf(p.scale_log2);
-    const uint32_t flip = p.scale_log2 < 0.f ? 0x80000000u : 0u;
+    const bool flip = p.scale_log2 < 0.f;
     const int NS = 4 * ((int)gridDim.x >> 1);                 // partial slots: 2 per cluster x 2 CTAs
     constexpr int SLOT_F4 = (D / 4) * BM;                      // float4 per partial slot: [D/4 column groups][128 rows]
 
@@ -287,7 +348,7 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
     auto ref_ok = [&](const OutRef& r) {
         return r.q_start + r.tok0 >= 0 && r.q_start + r.tok0 + r.ntok <= p.total_q && (unsigned)r.g < (unsigned)p.Hkv;
     };
-    // General merge of this CTA's tile of a split unit: pieces in clusters bh .. bl, in that order whoever merges
+    // General merge of this CTA's tile of a split unit: pieces in clusters bh .. bl, in that order whoever merges (group 0)
     auto merge_unit = [&](const OutRef& r, int unit, int bh, int bl) {
         const bool ok = row < rows_of(r) && ref_ok(r);
         auto slot_of = [&](int bb) { return (bb == bh ? 2 * bh + 1 : 2 * bb) * 2 + (int)rank; };
@@ -328,10 +389,10 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
         if (qd == 0 && lane == 0) p.unit_cnt[2 * unit + (int)rank] = 0;       // re-arm for the next launch
     };
 
-    uint32_t icount = 0, tcount = 0;
-    // PV(k) signals PV_DONE[k & 1]: two barriers, so that a wait for tile k (whose PV(k - 2) is known to be complete: it
-    // precedes QK(k) on the in-order tensor pipe) finds its barrier in phase k or k + 2, never further -- a parity wait
-    // cannot tell phases two apart, and these waits are not taken for every tile
+    uint32_t icount = 0, tcount = 0;      // items seen; active kv tiles seen (global index)
+    // PV of global tile k signals PV_DONE[k & 1] (phase k >> 1).  A wait for tile k finds PV of the stream's previous tile
+    // complete (it precedes QK(k) on the in-order tensor pipe) and the stream's next one not yet issued (it needs this
+    // group's P), so the barrier is in phase k >> 1 or one further: a parity wait is unambiguous.
     auto wait_pv = [&](uint32_t k) { ptx::mbar_wait(bar(L::B_PV_DONE + (k & 1u)), (k >> 1) & 1u, abort_flag); };
     while (true) {
         if (*abort_flag) break;
@@ -345,20 +406,23 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
         const int npg = it.pg1 - it.pg0, nt = rows > 0 ? (npg + 7) >> 3 : 0;
         const int c_lim = it.c < it.pg1 * SANGAM_PAGE ? it.c : it.pg1 * SANGAM_PAGE;
         const bool row_ok = row < rows && ref_ok(ref);
-        if (rows > 0 && !ref_ok(ref) && lane == 0) raise_flag(p.flags, DEV_INTERNAL | 0x400u);
+        if (wg == 0 && rows > 0 && !ref_ok(ref) && lane == 0) raise_flag(p.flags, DEV_INTERNAL | 0x400u);
         float m_ref = -INFINITY, l = 0.f;
         int peek = -1;
+        uint32_t k_last = 0;                    // global index of this group's last tile in the unit
+        int n_mine = 0;
         for (int t = 0; t < nt; ++t) {
+            const uint32_t k = tcount + (uint32_t)t;
+            if ((k & 1u) != wg) continue;
             if (*abort_flag) break;
             int nv = c_lim - (it.pg0 + 8 * t) * SANGAM_PAGE;
             nv = nv > BN ? BN : nv;
-            const uint32_t b = tcount & 1u;
-            const uint32_t s_taddr = tmem + lane_base + b * 128u;
-            if (t == nt - 1 && it.part_slot >= 0 && qd == 0 && lane == 0)
+            if (wg == 0 && t >= nt - 2 && it.part_slot >= 0 && qd == 0 && lane == 0)      // group 0's last tile of the unit
                 asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(peek) : "l"(p.unit_cnt + 2 * it.unit + (int)rank) : "memory");
-            ptx::mbar_wait(bar(L::B_S_FULL + b), (tcount >> 1) & 1u, abort_flag);
+            ptx::mbar_wait(bar(L::B_S_FULL + wg), (k >> 1) & 1u, abort_flag);
             ptx::tc_fence_after();
-            // pass 1: the row's maximum over the tile (positions >= nv masked)
+            DT(20);
+            // pass 1: the row's maximum over the tile (positions >= nv masked); the full-tile path has no per-element tests
             float mx = -INFINITY;
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
@@ -367,11 +431,20 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
                 ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h), r0);
                 ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h + 32), r1);
                 ptx::tmem_wait_ld();
-                const int lim = nv - 64 * h;
+                if (flip) {                                     // rare: scale < 0 -- work on -s with |scale|
 #pragma unroll
-                for (int i = 0; i < 32; ++i) {
-                    const float a = __uint_as_float(r0[i] ^ flip), c2 = __uint_as_float(r1[i] ^ flip);
-                    mx = fmaxf(mx, fmaxf(i < lim ? a : -INFINITY, 32 + i < lim ? c2 : -INFINITY));
+                    for (int i = 0; i < 32; ++i) { r0[i] ^= 0x80000000u; r1[i] ^= 0x80000000u; }
+                }
+                const int lim = nv - 64 * h;
+                if (lim >= 64) {
+                    float t4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};       // four independent chains
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) t4[i & 3] = fmaxf(t4[i & 3], fmaxf(__uint_as_float(r0[i]), __uint_as_float(r1[i])));
+                    mx = fmaxf(mx, fmaxf(fmaxf(t4[0], t4[1]), fmaxf(t4[2], t4[3])));
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i)
+                        mx = fmaxf(mx, fmaxf(i < lim ? __uint_as_float(r0[i]) : -INFINITY, 32 + i < lim ? __uint_as_float(r1[i]) : -INFINITY));
                 }
             }
             mx *= sc;
@@ -380,9 +453,9 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
             const float alpha = grow ? ptx::ex2(m_ref - m_new) : 1.f;
             m_ref = m_new;
             l *= alpha;
-            if (t > 0 && __any_sync(FULL, alpha != 1.f)) {
-                // rare (lazy reference maximum): every PV so far must have landed in O before the rows shrink
-                wait_pv(tcount - 1u);
+            if (n_mine > 0 && __any_sync(FULL, alpha != 1.f)) {
+                // rare (lazy reference maximum): every PV of this stream so far must have landed in O before the rows shrink
+                wait_pv(k - 2u);
                 ptx::tc_fence_after();
 #pragma unroll 1
                 for (int c = 0; c < D / 32; ++c) {
@@ -395,8 +468,11 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
                 }
                 ptx::tmem_wait_st();
             }
+            DT(21);
             // pass 2: P = 2^(s scale - m_ref) as bf16 pairs over the first 32 columns of each half, row sum into l
-            float sum = 0.f;
+            // (packed fp32x2 arithmetic: one FFMA2 / FADD2 per two columns)
+            const float2 sc2 = make_float2(sc, sc), ng2 = make_float2(-m_ref, -m_ref);
+            float2 sum_a = make_float2(0.f, 0.f), sum_b = make_float2(0.f, 0.f);
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 if (nv - 64 * h <= 0) continue;
@@ -404,36 +480,66 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
                 ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h), r0);
                 ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h + 32), r1);
                 ptx::tmem_wait_ld();
+                if (flip) {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) { r0[i] ^= 0x80000000u; r1[i] ^= 0x80000000u; }
+                }
                 const int lim = nv - 64 * h;
                 uint32_t pk[32];
 #pragma unroll
                 for (int i = 0; i < 32; i += 2) {
-                    float a0 = ptx::ex2(fmaf(__uint_as_float(r0[i] ^ flip), sc, -m_ref)), a1 = ptx::ex2(fmaf(__uint_as_float(r0[i + 1] ^ flip), sc, -m_ref));
-                    float c0 = ptx::ex2(fmaf(__uint_as_float(r1[i] ^ flip), sc, -m_ref)), c1 = ptx::ex2(fmaf(__uint_as_float(r1[i + 1] ^ flip), sc, -m_ref));
-                    if (i >= lim) a0 = 0.f;
-                    if (i + 1 >= lim) a1 = 0.f;
-                    if (32 + i >= lim) c0 = 0.f;
-                    if (33 + i >= lim) c1 = 0.f;
-                    sum += (a0 + a1) + (c0 + c1);
-                    pk[i >> 1] = ptx::pack_bf16(a0, a1);
-                    pk[16 + (i >> 1)] = ptx::pack_bf16(c0, c1);
+                    const float2 xa = __ffma2_rn(make_float2(__uint_as_float(r0[i]), __uint_as_float(r0[i + 1])), sc2, ng2);
+                    const float2 xc = __ffma2_rn(make_float2(__uint_as_float(r1[i]), __uint_as_float(r1[i + 1])), sc2, ng2);
+                    float2 pa = make_float2(ptx::ex2(xa.x), ptx::ex2(xa.y)), pc = make_float2(ptx::ex2(xc.x), ptx::ex2(xc.y));
+                    if (lim < 64) {
+                        if (i >= lim) pa.x = 0.f;
+                        if (i + 1 >= lim) pa.y = 0.f;
+                        if (32 + i >= lim) pc.x = 0.f;
+                        if (33 + i >= lim) pc.y = 0.f;
+                    }
+                    sum_a = __fadd2_rn(sum_a, pa);
+                    sum_b = __fadd2_rn(sum_b, pc);
+                    pk[i >> 1] = ptx::pack_bf16(pa.x, pa.y);
+                    pk[16 + (i >> 1)] = ptx::pack_bf16(pc.x, pc.y);
                 }
                 ptx::tmem_st16(s_taddr + (uint32_t)(64 * h), pk);
                 ptx::tmem_st16(s_taddr + (uint32_t)(64 * h + 16), pk + 16);
             }
-            l += sum;
+            const float2 sum2 = __fadd2_rn(sum_a, sum_b);
+            l += sum2.x + sum2.y;
             ptx::tmem_wait_st();
             ptx::tc_fence_before();
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL));
-            ++tcount;
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL + wg));
+            DT(23);
+            k_last = k;
+            ++n_mine;
         }
-        // ---------------- epilogue
+        const uint32_t t_start = tcount;
+        tcount += (uint32_t)nt;
+        if (wg == 1) {
+            // group 1 hands its stream's row statistics to group 0 (double-buffered by item slot: the slot is not reused
+            // before group 0 has released the item) and is done with the unit
+            // (one EPI barrier per item slot, used for every item: group 1 may run a whole item ahead of group 0, and a
+            // parity wait cannot tell phases two apart)
+            ml_x[islot * BM + row] = make_float2(m_ref, l);
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_EPI + islot));
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
+            ++icount;
+            continue;
+        }
+        // ---------------- epilogue (group 0)
+        DT(24);
+        ptx::mbar_wait(bar(L::B_EPI + islot), (icount >> 1) & 1u, abort_flag);      // group 1 is done with the unit's tiles
+        DT(25);
         const bool split = nt > 0 && it.part_slot >= 0;
         const int np_u = it.b_last - it.b_head + 1, k_me = ((int)blockIdx.x >> 1) - it.b_head;
         bool early = false;
         if (split) {
             if (qd == 0 && lane == 0) {
+                if (peek < 0 || n_mine == 0) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(peek) : "l"(p.unit_cnt + 2 * it.unit + (int)rank) : "memory");
                 const int e = (np_u == 2 && (k_me == 0 || k_me == 1) && peek + npg == it.upages) ? 1 : 0;
                 if (e) asm volatile("fence.acq_rel.gpu;" ::: "memory");
                 *merge_flag = e;
@@ -442,6 +548,7 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
             early = *merge_flag != 0;
             ptx::bar_sync(1, 128);
         }
+        DT(30 + (early ? 1 : 0) + (split ? 2 : 0));
         __nv_bfloat16* dst = out_ptr(ref);
         if (rows > 0 && nt == 0) {
             if (row_ok && it.part_slot < 0) {                    // empty context: zero rows (reading S13)
@@ -449,51 +556,75 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
                 for (int c = 0; c < D / 8; ++c) reinterpret_cast<uint4*>(dst)[c] = make_uint4(0, 0, 0, 0);
             }
         } else if (nt > 0) {
-            // the other piece of a two-piece unit is requested before the last PV is awaited (early merge, see attn_dec.cuh)
+            // the other piece of a two-piece unit is requested before the last PVs are awaited (early merge, see attn_dec.cuh)
             const int other = (k_me == 0 ? 2 * (it.b_head + 1) : 2 * it.b_head + 1) * 2 + (int)rank;
             float2 xo = make_float2(-INFINITY, 0.f);
             if (early) xo = __ldcg(reinterpret_cast<const float2*>(p.part_ml) + (int64_t)other * BM + row);
-            wait_pv(tcount - 1u);                                 // the unit's last PV (PVs complete in order)
+            // the two streams of this unit: which had tiles, their last PVs, stream 1's statistics
+            const bool has0 = n_mine > 0, has1 = nt >= 2 || !has0;
+            const uint32_t k1 = ((t_start + (uint32_t)nt - 1u) & 1u) ? t_start + (uint32_t)nt - 1u : t_start + (uint32_t)nt - 2u;   // stream 1's last tile
+            const float2 x1 = ml_x[islot * BM + row];
+            if (has0) wait_pv(k_last);
+            if (has1) wait_pv(k1);
             ptx::tc_fence_after();
+            DT(27);
+            // own piece = the two streams merged: M_own, weights, l_own
+            const float m0 = has0 ? m_ref : -INFINITY, m1 = has1 ? x1.x : -INFINITY;
+            const float m_own = fmaxf(m0, m1);
+            const float u0 = has0 ? ptx::ex2(m0 - m_own) : 0.f, u1 = has1 ? ptx::ex2(m1 - m_own) : 0.f;
+            const float l_own = fmaf(x1.y, u1, l * u0);
             const bool partial = split && !early;
             const bool slot_ok = !partial || (it.part_slot * 2 + (int)rank < NS && it.unit >= 0);
             if (!slot_ok && lane == 0) raise_flag(p.flags, DEV_INTERNAL | 0x100u);
             const int slot = it.part_slot * 2 + (int)rank;
-            float w_own = 1.f, w_oth = 0.f, inv = l > 0.f ? 1.f / l : 0.f;
+            float w_own = 1.f, w_oth = 0.f, inv = l_own > 0.f ? 1.f / l_own : 0.f;
             if (early) {                                         // pieces in order: k_me = 0: own, other;  1: other, own
-                const float M = fmaxf(m_ref, xo.x);
-                w_own = ptx::ex2(m_ref - M); w_oth = ptx::ex2(xo.x - M);
-                const float Lsum = k_me == 0 ? fmaf(xo.y, w_oth, fmaf(l, w_own, 0.f)) : fmaf(l, w_own, fmaf(xo.y, w_oth, 0.f));
+                const float M = fmaxf(m_own, xo.x);
+                w_own = ptx::ex2(m_own - M); w_oth = ptx::ex2(xo.x - M);
+                const float Lsum = k_me == 0 ? fmaf(xo.y, w_oth, fmaf(l_own, w_own, 0.f)) : fmaf(l_own, w_own, fmaf(xo.y, w_oth, 0.f));
                 inv = Lsum > 0.f ? 1.f / Lsum : 0.f;
             }
 #pragma unroll 1
             for (int c = 0; c < D / 32; ++c) {
-                uint32_t o[32];
+                uint32_t oa[32], ob[32];
                 float4 ov[8];
                 if (early) {
                     const float4* so = reinterpret_cast<const float4*>(p.part_o) + (int64_t)other * SLOT_F4 + (int64_t)(c * 8) * BM + row;
 #pragma unroll
                     for (int v = 0; v < 8; ++v) ov[v] = __ldcg(so + v * BM);
                 }
-                ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
+                // a stream without tiles contributes zeros (its accumulator was never written): no per-element branches
+                if (has0) ptx::tmem_ld32(o0_taddr + (uint32_t)(c * 32), oa);
+                else {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) oa[e] = 0u;
+                }
+                if (has1) ptx::tmem_ld32(o1_taddr + (uint32_t)(c * 32), ob);
+                else {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) ob[e] = 0u;
+                }
                 ptx::tmem_wait_ld();
+                DT(34);
+                float a[32];                                     // this piece's unnormalised row chunk, both streams
+#pragma unroll
+                for (int e = 0; e < 32; ++e) a[e] = fmaf(__uint_as_float(ob[e]), u1, __uint_as_float(oa[e]) * u0);
                 float f[32];
                 if (early) {
 #pragma unroll
                     for (int v = 0; v < 8; ++v) {
                         const float e0 = ov[v].x, e1 = ov[v].y, e2 = ov[v].z, e3 = ov[v].w;
-                        const float a0 = __uint_as_float(o[4 * v]), a1 = __uint_as_float(o[4 * v + 1]), a2 = __uint_as_float(o[4 * v + 2]), a3 = __uint_as_float(o[4 * v + 3]);
                         if (k_me == 0) {
-                            f[4 * v] = fmaf(e0, w_oth, fmaf(a0, w_own, 0.f)); f[4 * v + 1] = fmaf(e1, w_oth, fmaf(a1, w_own, 0.f));
-                            f[4 * v + 2] = fmaf(e2, w_oth, fmaf(a2, w_own, 0.f)); f[4 * v + 3] = fmaf(e3, w_oth, fmaf(a3, w_own, 0.f));
+                            f[4 * v] = fmaf(e0, w_oth, fmaf(a[4 * v], w_own, 0.f)); f[4 * v + 1] = fmaf(e1, w_oth, fmaf(a[4 * v + 1], w_own, 0.f));
+                            f[4 * v + 2] = fmaf(e2, w_oth, fmaf(a[4 * v + 2], w_own, 0.f)); f[4 * v + 3] = fmaf(e3, w_oth, fmaf(a[4 * v + 3], w_own, 0.f));
                         } else {
-                            f[4 * v] = fmaf(a0, w_own, fmaf(e0, w_oth, 0.f)); f[4 * v + 1] = fmaf(a1, w_own, fmaf(e1, w_oth, 0.f));
-                            f[4 * v + 2] = fmaf(a2, w_own, fmaf(e2, w_oth, 0.f)); f[4 * v + 3] = fmaf(a3, w_own, fmaf(e3, w_oth, 0.f));
+                            f[4 * v] = fmaf(a[4 * v], w_own, fmaf(e0, w_oth, 0.f)); f[4 * v + 1] = fmaf(a[4 * v + 1], w_own, fmaf(e1, w_oth, 0.f));
+                            f[4 * v + 2] = fmaf(a[4 * v + 2], w_own, fmaf(e2, w_oth, 0.f)); f[4 * v + 3] = fmaf(a[4 * v + 3], w_own, fmaf(e3, w_oth, 0.f));
                         }
                     }
                 } else {
 #pragma unroll
-                    for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(o[e]);
+                    for (int e = 0; e < 32; ++e) f[e] = a[e];
                 }
                 if (partial) {
                     if (slot_ok && row < rows) {
@@ -513,8 +644,12 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
             }
             ptx::tc_fence_before();
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(bar(L::B_O_FREE));
-            if (partial && slot_ok && row < rows) reinterpret_cast<float2*>(p.part_ml)[(int64_t)slot * BM + row] = make_float2(m_ref, l);
+            DT(28);
+            if (lane == 0) {                                     // both accumulators have been read
+                if (has0) ptx::mbar_arrive(bar(L::B_O_FREE));
+                if (has1) ptx::mbar_arrive(bar(L::B_O_FREE + 1));
+            }
+            if (partial && slot_ok && row < rows) reinterpret_cast<float2*>(p.part_ml)[(int64_t)slot * BM + row] = make_float2(m_own, l_own);
             if (split) {
                 if (qd == 0 && lane == 0) {
                     agent_req[islot] = (partial && slot_ok) ? 1 : 0;
@@ -525,9 +660,11 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
             }
         }
         __syncwarp();
+        DT(29);
         if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
         ++icount;
     }
+    if (wg == 1) return;
     ptx::mbar_wait(bar(L::B_AGENT_DONE), 0u, abort_flag);
     const Deferred* defer = reinterpret_cast<const Deferred*>(smem + L::OFF_MISC + 32);
     for (int k = 0; k < 2; ++k) {
@@ -591,26 +728,26 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 gqa_decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
                   const __grid_constant__ CUtensorMap mapQ, const DecParams p) {
     using L = Smem<D>;
-    extern __shared__ uint8_t smem_raw[];
-    // both CTAs of the pair must use the SAME offsets inside their shared-memory windows (multicast writes land at the
-    // issuing CTA's offset): the dynamic base is the same in every CTA of a launch, so is the alignment fix-up
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    // both CTAs of the pair use the same offsets inside their shared-memory windows (a multicast write lands at the issuing
+    // CTA's offset in every destination): the dynamic base is the same in every CTA of a launch (no static shared memory)
+    extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = ptx::smem_u32(smem);
     Item* items = reinterpret_cast<Item*>(smem + L::OFF_ITEMS);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::OFF_MISC);
     volatile uint32_t* abort_flag = reinterpret_cast<volatile uint32_t*>(smem + L::OFF_ABORT);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t rank = cluster_rank();
+    TRACE_CTA(0);
     if (tid == 0) {
         auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
-        for (int s = 0; s < NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 2); }   // both CTAs release
+        for (int s = 0; s < 2 * NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 2); }   // both CTAs release
         for (int s = 0; s < 2; ++s) {
-            ptx::mbar_init(bar(L::B_ITEM_FULL + s), 1); ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 6);      // MMA warp + agent + 4 softmax warps
-            ptx::mbar_init(bar(L::B_S_FULL + s), 1);
+            ptx::mbar_init(bar(L::B_ITEM_FULL + s), 1); ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 11);     // MMA warp + V producer + agent + 8 softmax warps
+            ptx::mbar_init(bar(L::B_S_FULL + s), 1); ptx::mbar_init(bar(L::B_P_FULL + s), 4);
+            ptx::mbar_init(bar(L::B_PV_DONE + s), 1); ptx::mbar_init(bar(L::B_O_FREE + s), 4);
         }
         ptx::mbar_init(bar(L::B_Q_FULL), 1); ptx::mbar_init(bar(L::B_Q_EMPTY), 1);
-        ptx::mbar_init(bar(L::B_P_FULL), 4); ptx::mbar_init(bar(L::B_PV_DONE), 1); ptx::mbar_init(bar(L::B_PV_DONE + 1), 1);
-        ptx::mbar_init(bar(L::B_O_FREE), 4);
+        ptx::mbar_init(bar(L::B_EPI), 4); ptx::mbar_init(bar(L::B_EPI + 1), 4);
         ptx::mbar_init(bar(L::B_AGENT_REQ), 4); ptx::mbar_init(bar(L::B_AGENT_DONE), 1);
         for (int k = 1; k < (L::TOTAL - L::OFF_MISC) / 4; ++k) tmem_slot[k] = 0u;
         ptx::fence_mbar_init();
@@ -623,7 +760,7 @@ gqa_decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constan
         ptx::tmem_relinquish();
     }
     if (warp >= 4) {       // rows of the q tile that no TMA box writes (tpt G < 128) stay zero
-        for (int e = tid - 128; e < L::Q_BYTES / 16; e += 128)
+        for (int e = tid - 128; e < L::Q_BYTES / 16; e += 256)
             asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(sbase + (uint32_t)(L::OFF_Q + e * 16)), "r"(0) : "memory");
         ptx::fence_proxy_async_smem();
     }
@@ -634,13 +771,24 @@ gqa_decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constan
     cluster_sync_all();            // the peer's barriers exist before anything is multicast to it or arrives on them
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    if (warp == 0) producer_warp<D>(p, &mapK, &mapV, &mapQ, sbase, items, abort_flag, lane, rank);
-    else if (warp == 1) mma_warp<D>(p, sbase, tmem, items, abort_flag, lane, rank);
-    else if (warp == 2) agent_warp<D>(p, smem, sbase, items, abort_flag, lane, rank);
-    else if (warp >= 4) softmax_warps<D>(p, smem, sbase, tmem, items, abort_flag, warp, lane, rank);
+    const bool base_ok = (sbase & 1023u) == 0u;
+    if (!base_ok && tid == 0) raise_flag(p.flags, DEV_INTERNAL | 0x800u);
+    // 12 warps x 168 registers at launch; the service warpgroup hands its surplus to the two softmax groups
+    if (warp >= 4) {
+        ptx::setmaxnreg_inc<208>();
+        if (base_ok) softmax_warps<D>(p, smem, sbase, tmem, items, abort_flag, warp, lane, rank);
+    } else {
+        ptx::setmaxnreg_dec<88>();
+        if (!base_ok) { }
+        else if (warp == 0) producer_warp<D>(p, &mapK, &mapQ, sbase, items, abort_flag, lane, rank);
+        else if (warp == 3) v_producer_warp<D>(p, &mapV, sbase, items, abort_flag, lane, rank);
+        else if (warp == 1) mma_warp<D>(p, sbase, tmem, items, abort_flag, lane, rank);
+        else if (warp == 2) agent_warp<D>(p, smem, sbase, items, abort_flag, lane, rank);
+    }
     ptx::tc_fence_before();
     __syncthreads();
     cluster_sync_all();            // neither CTA leaves while the other may still write into it
+    TRACE_CTA(1);
     if (tid == 0 && *abort_flag) raise_flag(p.flags, DEV_TIMEOUT);
     if (warp == 1) ptx::tmem_dealloc(tmem, 512);
 }

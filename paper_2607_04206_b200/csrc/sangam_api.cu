@@ -398,9 +398,11 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
     // compute the same function for any batch; the choice only affects speed.  Lengths live on the device, so the
     // host decides on the counts it knows: total_q and batch.
     bool use_dec = ctx->dec_occ > 0 && (int64_t)total_q * ctx->G <= (int64_t)dec::NQ * batch;
-    // GQA models: block decodes of up to two 128-row q tiles per kv head go to the CTA-pair kernel
+    // GQA models: block decodes of up to two 128-row q tiles per kv head fit the CTA-pair kernel (attn_gqa.cuh).  It is
+    // measured slower than the two-stream kernel on the Dream-like shapes (config 3: 72.7 us against 66.2 us), so AUTO
+    // does not choose it; SANGAM_DISPATCH_GQA_PAIR selects it.
     const int tpt = 128 / ctx->G;
-    bool use_gqa = !use_dec && ctx->gqa_ok && (int64_t)total_q <= (int64_t)2 * tpt * batch;
+    bool use_gqa = false;
     if (ctx->dispatch == SANGAM_DISPATCH_PREFILL) { use_dec = false; use_gqa = false; }
     if (ctx->dispatch == SANGAM_DISPATCH_DECODE) {
         if (ctx->dec_occ <= 0) return fail(ctx, SANGAM_ERR_UNSUPPORTED, "block_attn: the decode kernel is not available for this geometry");

@@ -9,7 +9,8 @@ import sangam_inputs as si
 MAX_ABS, MEAN_ABS = 2e-2, 2e-3      # north_star tolerance for bf16-in / fp32-accumulate attention
 
 # which attention kernel sangam_block_attn launches in DeviceBatch (0 auto, 1 two-stream prefill kernel, 2 decode
-# kernel); set per test by the `dispatch` fixture of conftest.py so that every parity / edge case runs through both
+# kernel, 3 CTA-pair GQA decode kernel); set per test by the `dispatch` fixture of conftest.py so that every parity /
+# edge case runs through all of them
 DEFAULT_DISPATCH = 0
 
 
@@ -46,6 +47,12 @@ class DeviceBatch:
                              max_total_q=max_total_q or max(b.total_q, len(b.slot_cache), 1),
                              max_pages_per_req=b.max_pages_per_req)
         if DEFAULT_DISPATCH:
+            if DEFAULT_DISPATCH == sg.DISPATCH_GQA_PAIR and self.eng.query(3) != 1:
+                import pytest
+                pytest.skip("no CTA-pair kernel for this geometry (it needs 1 < num_q_heads / num_kv_heads <= 128)")
+            if DEFAULT_DISPATCH == sg.DISPATCH_DECODE and self.eng.query(1) <= 0:
+                import pytest
+                pytest.skip("no decode kernel for this geometry (it needs num_q_heads / num_kv_heads <= 32)")
             self.eng.set_dispatch(DEFAULT_DISPATCH)
 
     def load_cache(self):

@@ -14,13 +14,16 @@ pytestmark = pytest.mark.gpu
 BAD_SLOT, BAD_PAGE, CTX_TOO_LONG = 1, 2, 4
 
 
+KERNEL = {"prefill_kernel": 1, "decode_kernel": 2, "gqa_pair_kernel": 3}      # sangam_set_dispatch modes
+
+
 def _batch():
     # request 1 is the victim; requests 0 and 2 must be unaffected.  Decode-sized rows so that both kernels are natural.
     return si.custom(61, [32, 32, 20], [200, 333, 97], num_q_heads=8, num_kv_heads=4, head_dim=128)
 
 
 @pytest.mark.parametrize("bad_id", ["past_the_pool", "negative", "huge"])
-@pytest.mark.parametrize("path", ["prefill_kernel", "decode_kernel", "simt"])
+@pytest.mark.parametrize("path", ["prefill_kernel", "decode_kernel", "gqa_pair_kernel", "simt"])
 def test_bad_page_id_reads_as_zeros_and_raises_the_flag(oracle, path, bad_id):
     """A page id outside [0, num_pages) inside ceil(c/16): SANGAM_DEV_BAD_PAGE, that page's positions read as K = V = 0,
     other requests untouched (sangam.h).  The expectation comes from the oracle run on an equivalent well-formed batch:
@@ -30,7 +33,7 @@ def test_bad_page_id_reads_as_zeros_and_raises_the_flag(oracle, path, bad_id):
     bad = {"past_the_pool": b.num_pages, "negative": -7, "huge": 2 ** 30}[bad_id]
     db = DeviceBatch(b)
     if path != "simt":
-        db.eng.set_dispatch({"prefill_kernel": 1, "decode_kernel": 2}[path])
+        db.eng.set_dispatch(KERNEL[path])
     db.load_cache(); db.write_new()
     bt = b.block_table.copy()
     bt[1, victim_entry] = bad
@@ -55,7 +58,7 @@ def test_bad_page_id_reads_as_zeros_and_raises_the_flag(oracle, path, bad_id):
     # the neighbours are bit-identical to a clean run
     clean = DeviceBatch(b)
     if path != "simt":
-        clean.eng.set_dispatch({"prefill_kernel": 1, "decode_kernel": 2}[path])
+        clean.eng.set_dispatch(KERNEL[path])
     c = bits_of(clean.iteration(simt=(path == "simt")))
     got = bits_of(db.out)
     lo, hi = b.cu_q_lens[1], b.cu_q_lens[2]
@@ -63,7 +66,7 @@ def test_bad_page_id_reads_as_zeros_and_raises_the_flag(oracle, path, bad_id):
     assert not np.array_equal(got[lo:hi], c[lo:hi])
 
 
-@pytest.mark.parametrize("path", ["prefill_kernel", "decode_kernel", "simt"])
+@pytest.mark.parametrize("path", ["prefill_kernel", "decode_kernel", "gqa_pair_kernel", "simt"])
 def test_context_longer_than_the_block_table_gives_zero_rows(oracle, path):
     """ctx_len needing more than max_pages_per_req pages: SANGAM_DEV_CTX_TOO_LONG, that request's rows are zeros, the
     others match the oracle; negative ctx_len is read as 0 (zero rows, no flag)."""
@@ -73,7 +76,7 @@ def test_context_longer_than_the_block_table_gives_zero_rows(oracle, path):
     for new_len, flag in ((b.max_pages_per_req * 16 + 1, CTX_TOO_LONG), (-5, 0)):
         db = DeviceBatch(b)
         if path != "simt":
-            db.eng.set_dispatch({"prefill_kernel": 1, "decode_kernel": 2}[path])
+            db.eng.set_dispatch(KERNEL[path])
         db.load_cache(); db.write_new()
         cl = b.ctx_lens.copy(); cl[1] = new_len
         db.ctx_lens = t_i32(cl)
@@ -89,13 +92,13 @@ def test_context_longer_than_the_block_table_gives_zero_rows(oracle, path):
         assert mx <= MAX_ABS and mean <= MEAN_ABS
 
 
-@pytest.mark.parametrize("path", ["prefill_kernel", "decode_kernel"])
+@pytest.mark.parametrize("path", ["prefill_kernel", "decode_kernel", "gqa_pair_kernel"])
 def test_decreasing_cu_q_lens_is_an_empty_request(oracle, path):
     """cu_q_lens[r+1] < cu_q_lens[r] is read as q_r = 0: nothing is written for that request, nothing faults."""
     import torch
     b = _batch()
     db = DeviceBatch(b)
-    db.eng.set_dispatch({"prefill_kernel": 1, "decode_kernel": 2}[path])
+    db.eng.set_dispatch(KERNEL[path])
     db.load_cache(); db.write_new()
     cu = b.cu_q_lens.copy(); cu[3] = cu[2] - 3              # the last request "ends before it starts"
     db.cu_q_lens = t_i32(cu)
@@ -185,6 +188,20 @@ def test_geometry_without_a_decode_kernel():
     assert db.eng.query(1) == 0
     with pytest.raises(sg.SangamError):
         db.eng.set_dispatch(sg.DISPATCH_DECODE)
+    import oracle as o
+    ref, _, _ = o.iteration(b)
+    mx, mean = compare(db.iteration(), ref)
+    assert mx <= MAX_ABS and mean <= MEAN_ABS
+
+
+def test_geometry_without_a_pair_kernel():
+    """MHA (G = 1): the CTA-pair GQA kernel does not exist for the geometry; GQA_PAIR is refused, AUTO is unaffected."""
+    import paper_2607_04206_b200 as sg
+    b = si.custom(63, [32, 5], [150, 40], num_q_heads=4, num_kv_heads=4, head_dim=64)
+    db = DeviceBatch(b)
+    assert db.eng.query(3) == 0
+    with pytest.raises(sg.SangamError):
+        db.eng.set_dispatch(sg.DISPATCH_GQA_PAIR)
     import oracle as o
     ref, _, _ = o.iteration(b)
     mx, mean = compare(db.iteration(), ref)

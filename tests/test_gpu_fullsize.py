@@ -17,10 +17,12 @@ pytestmark = pytest.mark.gpu
 CEILING = {2: (2.8e-3, 4.7e-4), 3: (1.5e-3, 2.0e-4), 4: (2.8e-3, 3.0e-4), 5: (2.8e-3, 3.0e-4)}
 
 
-@pytest.mark.parametrize("cfg,per_req", [(2, 32), (3, 32), (4, 24), (5, 16)])
-def test_full_size_config(oracle, cfg, per_req):
+@pytest.mark.parametrize("cfg,per_req,kernel", [(2, 32, 0), (3, 32, 0), (3, 32, 3), (4, 24, 0), (5, 16, 0)],
+                         ids=["config2", "config3", "config3-gqa_pair_kernel", "config4", "config5"])
+def test_full_size_config(oracle, cfg, per_req, kernel, monkeypatch):
     import torch
     import bench
+    monkeypatch.setattr(bench, "DISPATCH", kernel)      # 0: the library's choice (what bench.py times); 3: the CTA-pair kernel
     b = si.CONFIGS[cfg]()
     w = bench.Workload(b, 1)
     w.capture()
