@@ -35,6 +35,7 @@ struct DecParams {
     const int32_t* cu_q_lens;      // [batch+1]
     const int32_t* ctx_lens;       // [batch]
     __nv_bfloat16* out;            // [total_q][Hq][D]
+    const __nv_bfloat16* q;        // [total_q][Hq][D] (the GQA pair kernel reads q rows directly; the decode kernel through its tensor map)
     int32_t batch, total_q;
     int32_t Hq, Hkv, G, W, P;
     int32_t tq;                    // query tokens per unit: 32 / G (decode kernel), 2 tpt (GQA pair kernel)

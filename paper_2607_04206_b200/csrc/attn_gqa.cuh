@@ -37,10 +37,10 @@ using dec::dtrace;
 
 constexpr int BM = 128;          // rows of a q tile (UMMA M)
 constexpr int BN = 128;          // kv positions per tile (8 pages)
-constexpr int NSTAGE = 3;        // stages of the K ring and of the V ring (separate rings: a V tile waits for its
-                                 // softmax much longer than a K tile for its QK, and must not hold up the K loads)
+constexpr int NK = 3;            // stages of the K ring
+constexpr int NV = 3;            // stages of the V ring (separate rings with an issuing warp each: a V tile is held until its
+                                 // softmax has been multiplied in, much longer than a K tile)
 constexpr int NTHREADS = 384;
-constexpr int SLAB = 128 * 128;  // bytes of one 64-wide swizzled slab of the q tile
 constexpr float LAZY_T = 8.f;
 #ifndef SANGAM_GQA_OV
 #define SANGAM_GQA_OV 16
@@ -48,22 +48,23 @@ constexpr float LAZY_T = 8.f;
 constexpr int OV = SANGAM_GQA_OV;   // fixed cost of starting / finishing a unit, in pages (stream-K weight)
 constexpr int MIN_W = 64;           // smallest share of the weighted unit list given to a cluster
 template <int D> constexpr int KV_ATOM_STRIDE = 1024 * (D / 64);
+// TMEM columns: Q (bf16 pairs, D / 2 columns) at 0, S[j] at 64 + 128 j (j = 0, 1), O at 320
+constexpr uint32_t TM_Q = 0u, TM_S = 64u, TM_O = 320u;
 
 template <int D>
 struct Smem {
     static constexpr int KV_BYTES = BN * D * 2;
-    static constexpr int Q_BYTES = BM * D * 2;
-    static constexpr int OFF_KV = 0;                     // stages 0 .. NSTAGE-1: K ring, NSTAGE .. 2 NSTAGE-1: V ring
-    static constexpr int OFF_Q = 2 * NSTAGE * KV_BYTES;
-    static constexpr int OFF_BAR = OFF_Q + Q_BYTES;
-    static constexpr int B_KV_FULL = 0, B_KV_EMPTY = 2 * NSTAGE, B_ITEM_FULL = 4 * NSTAGE, B_ITEM_EMPTY = B_ITEM_FULL + 2,
-                         B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 1, B_S_FULL = B_Q_EMPTY + 1 /* [stream] */,
-                         B_P_FULL = B_S_FULL + 2 /* [stream] */, B_PV_DONE = B_P_FULL + 2 /* [stream] */, B_O_FREE = B_PV_DONE + 2 /* [stream] */,
-                         B_EPI = B_O_FREE + 2 /* [item slot] */, B_AGENT_REQ = B_EPI + 2, B_AGENT_DONE = B_AGENT_REQ + 1, NBAR = B_AGENT_DONE + 1;
+    static constexpr int OFF_KV = 0;                     // stages 0 .. NK-1: K ring, NK .. NK+NV-1: V ring
+    static constexpr int OFF_BAR = (NK + NV) * KV_BYTES;
+    static constexpr int B_KV_FULL = 0, B_KV_EMPTY = NK + NV, B_ITEM_FULL = 2 * (NK + NV), B_ITEM_EMPTY = B_ITEM_FULL + 2,
+                         B_Q_FULL = B_ITEM_EMPTY + 2, B_Q_EMPTY = B_Q_FULL + 1, B_S_FULL = B_Q_EMPTY + 1 /* [tile parity] */,
+                         B_P_FULL = B_S_FULL + 2 /* [tile parity] */, B_PV_DONE = B_P_FULL + 2 /* [tile parity] */, B_O_FREE = B_PV_DONE + 2,
+                         B_EPI = B_O_FREE + 1 /* [item slot] */, B_AGENT_REQ = B_EPI + 2, B_AGENT_DONE = B_AGENT_REQ + 1, NBAR = B_AGENT_DONE + 1;
     static constexpr int OFF_ITEMS = OFF_BAR + ((NBAR * 8 + 15) / 16) * 16;
-    static constexpr int OFF_ML = OFF_ITEMS + 2 * (int)sizeof(Item);     // [2 item slots][128 rows] (m, l) of stream 1
+    static constexpr int OFF_ML = OFF_ITEMS + 2 * (int)sizeof(Item);     // [2 item slots][128 rows] row sum of group 1's half
+    static constexpr int OFF_MX = OFF_ML + 2 * BM * 4;                   // [2 tile parities][2 groups][128 rows] half-tile row maxima
     // misc block: +0 tmem slot, +8 merge flag, +16 agent_req[2], +32 Deferred[2], +96 abort word (+ wait table in debug builds)
-    static constexpr int OFF_MISC = OFF_ML + 2 * BM * 8;
+    static constexpr int OFF_MISC = OFF_MX + 4 * BM * 4;
     static constexpr int OFF_ABORT = OFF_MISC + 96;
     static constexpr int TOTAL = OFF_ABORT + 80;
     static constexpr int ALLOC = TOTAL;                  // no alignment slack: the dynamic base is 1024-byte aligned (checked at run time)
@@ -100,7 +101,8 @@ __device__ __forceinline__ void tma_load_4d_mc(uint32_t dst_smem, const CUtensor
 // the current one is entered, eight tiles before it is needed: no load waits on a block-table read except the unit's first.
 template <int D>
 __device__ __forceinline__ void load_tiles(const DecParams& p, const CUtensorMap* map, uint32_t sbase, const Item& it, uint32_t rank, int lane,
-                                           uint32_t ring0, uint32_t& st, uint32_t& ph, volatile uint32_t* abort_flag, [[maybe_unused]] unsigned& dt_i_) {
+                                           uint32_t ring0, uint32_t nstage, uint32_t& st, uint32_t& ph, volatile uint32_t* abort_flag,
+                                           [[maybe_unused]] unsigned& dt_i_) {
     using L = Smem<D>;
     const unsigned FULL = 0xffffffffu;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
@@ -126,15 +128,15 @@ __device__ __forceinline__ void load_tiles(const DecParams& p, const CUtensorMap
         if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_KV_FULL + stage), (uint32_t)(np * SANGAM_PAGE * D * 2));
         __syncwarp();
         if (mine) tma_load_4d_mc(dst0 + stage * L::KV_BYTES, map, bar(L::B_KV_FULL + stage), (page * p.Hkv + it.g) * 2, (uint16_t)3);
-        if (++st == NSTAGE) { st = 0; ph ^= 1u; }
+        if (++st == nstage) { st = 0; ph ^= 1u; }
         DT((ring0 ? 120 : 100) + (t & 15));
         if (*abort_flag) break;
     }
 }
 
-// warp 0: device-side plan (a3), Q loads, the K ring
+// warp 0: device-side plan (a3), the K ring
 template <int D>
-__device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensorMap* mapK, const CUtensorMap* mapQ, uint32_t sbase, Item* items,
+__device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensorMap* mapK, uint32_t sbase, Item* items,
                                               volatile uint32_t* abort_flag, int lane, uint32_t rank) {
     using L = Smem<D>;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
@@ -143,7 +145,7 @@ __device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensor
     Planner plan;
     plan.init(p, lane, (int)gridDim.x >> 1, (int)blockIdx.x >> 1);
     DT(2);
-    uint32_t kst = 0, kph = 0, icount = 0, qcount = 0;
+    uint32_t kst = 0, kph = 0, icount = 0;
     while (true) {
         if (*abort_flag) break;
         Item it;
@@ -158,23 +160,12 @@ __device__ __forceinline__ void producer_warp(const DecParams& p, const CUtensor
         ++icount;
         if (!it.valid) break;
         if (it.pg1 - it.pg0 <= 0) continue;
-        const int ntok_c = it.ntok - (int)rank * p.tpt;                       // tokens of this CTA's q tile
-        if (ntok_c > 0) {
-            ptx::mbar_wait(bar(L::B_Q_EMPTY), (qcount & 1u) ^ 1u, abort_flag);
-            if (lane == 0) ptx::mbar_arrive_expect_tx(bar(L::B_Q_FULL), (uint32_t)(p.tpt * p.G * D * 2));
-            __syncwarp();
-            if (lane < D / 64)
-                ptx::tma_load_3d(sbase + (uint32_t)(L::OFF_Q + lane * SLAB), mapQ, bar(L::B_Q_FULL), lane * 64, it.g * p.G,
-                                 it.q_start + it.tok0 + (int)rank * p.tpt);
-            ++qcount;
-        }
-        load_tiles<D>(p, mapK, sbase, it, rank, lane, 0u, kst, kph, abort_flag, dt_i_);
+        load_tiles<D>(p, mapK, sbase, it, rank, lane, 0u, (uint32_t)NK, kst, kph, abort_flag, dt_i_);
     }
-    for (int k = 0; k < NSTAGE; ++k) {      // every commit aimed at this CTA's barriers has landed before it may exit
+    for (int k = 0; k < NK; ++k) {          // every commit aimed at this CTA's barriers has landed before it may exit
         ptx::mbar_wait(bar(L::B_KV_EMPTY + kst), kph ^ 1u, abort_flag);
-        if (++kst == NSTAGE) { kst = 0; kph ^= 1u; }
+        if (++kst == NK) { kst = 0; kph ^= 1u; }
     }
-    ptx::mbar_wait(bar(L::B_Q_EMPTY), (qcount & 1u) ^ 1u, abort_flag);
 }
 
 // warp 3: the V ring (a ring and an issuing warp of its own: a V tile is needed a whole softmax later than its K tile, and one
@@ -193,23 +184,26 @@ __device__ __forceinline__ void v_producer_warp(const DecParams& p, const CUtens
         const Item it = items[islot];
         if (!it.valid) break;
         if (it.pg1 - it.pg0 > 0) {
-            load_tiles<D>(p, mapV, sbase, it, rank, lane, (uint32_t)NSTAGE, vst, vph, abort_flag, dt_i_);
+            load_tiles<D>(p, mapV, sbase, it, rank, lane, (uint32_t)NK, (uint32_t)NV, vst, vph, abort_flag, dt_i_);
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
         ++icount;
     }
-    for (int k = 0; k < NSTAGE; ++k) {
-        ptx::mbar_wait(bar(L::B_KV_EMPTY + NSTAGE + vst), vph ^ 1u, abort_flag);
-        if (++vst == NSTAGE) { vst = 0; vph ^= 1u; }
+    for (int k = 0; k < NV; ++k) {
+        ptx::mbar_wait(bar(L::B_KV_EMPTY + NK + vst), vph ^ 1u, abort_flag);
+        if (++vst == NV) { vst = 0; vph ^= 1u; }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// warp 1: MMA issuer.  Global kv tile k belongs to stream b = k & 1:  S[b] = Q K(k)^T (128 TMEM columns),
-// O[b] += P(k) V(k) with P read from TMEM (bf16, packed over the first 32 columns of each 64-column half of S[b]).
-// QK runs one tile ahead of PV, so the two streams' softmax groups always have a tile each.
-// TMEM: S[0] = columns [0, 128), S[1] = [128, 256), O[0] = [256, 256 + D), O[1] = [384, 384 + D).
+// warp 1: MMA issuer.  Per kv tile k (global count, score buffer j = k & 1):
+//     S[j] = Q K(k)^T    A = Q from TMEM (bf16; the q tile is stored there once per unit by softmax group 1, so a QK reads only
+//                        the K tile from shared memory), 128 fp32 columns,
+//     O   += P(k) V(k)   A = P from TMEM: bf16, packed over the first 32 columns of each 64-column half of S[j].
+// QK(k + 1) is issued before PV(k) is waited for, QK(k + 2) right behind PV(k) (it overwrites the buffer PV(k) reads: the
+// tensor pipe executes in order): the scores of the next tile are complete long before the softmax of the current one is.
+// TMEM: Q = columns [0, 64), S[0] = [64, 192), S[1] = [192, 320), O = [320, 320 + D).
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uint32_t tmem, const Item* items, volatile uint32_t* abort_flag,
@@ -217,14 +211,12 @@ __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uin
     using L = Smem<D>;
     auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
     DT_DECL;
-    const uint64_t q_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_Q, 16, 1024);
     const uint64_t k_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 16, KV_ATOM_STRIDE<D>);
     const uint64_t v_desc0 = ptx::smem_desc_sw128(sbase + L::OFF_KV, 1024, KV_ATOM_STRIDE<D>);
-    constexpr uint32_t VSTEP = (uint32_t)(2 * KV_ATOM_STRIDE<D>) >> 4;
+    constexpr uint32_t VSTEP = (uint32_t)(2 * KV_ATOM_STRIDE<D>) >> 4;       // one page = 16 kv rows, in descriptor units
     constexpr uint32_t IDESC_PV = ptx::idesc_bf16(BM, D, 0, 1);
     const uint32_t peer = rank ^ 1u;
-    uint32_t kst = 0, kph = 0, vst = 0, vph = 0, icount = 0, qcount = 0, tcount = 0;
-    uint32_t ocount[2] = {0, 0};             // units in which stream b accumulated (O_FREE[b] phases)
+    uint32_t kst = 0, kph = 0, vst = 0, vph = 0, icount = 0, qcount = 0, tcount = 0, ocount = 0;
     auto release = [&](uint32_t s) {         // this CTA is done with stage s: tell both producers of the pair
         ptx::mma_commit(bar(L::B_KV_EMPTY + s));
         ptx::mma_commit(peer_addr(bar(L::B_KV_EMPTY + s), peer));
@@ -244,17 +236,18 @@ __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uin
             auto issue_qk = [&](int t) {
                 const uint32_t sk = kst;
                 ptx::mbar_wait(bar(L::B_KV_FULL + sk), kph, abort_flag);
-                if (++kst == NSTAGE) { kst = 0; kph ^= 1u; }
+                if (++kst == NK) { kst = 0; kph ^= 1u; }
                 ptx::tc_fence_after();
                 DT(140 + (t & 15));
                 if (ptx::elect_one()) {
                     if (active) {
+                        const uint32_t j = (tcount + (uint32_t)t) & 1u;
                         const int ncol = (nv_of(t) + 15) & ~15;
-                        const uint32_t s_tmem = tmem + (uint32_t)(((tcount + (uint32_t)t) & 1u) * 128u);
+                        const uint32_t s_tmem = tmem + TM_S + j * 128u;
                         const uint64_t b_desc = k_desc0 + (uint64_t)(sk * (L::KV_BYTES >> 4));
                         const uint32_t idesc = ptx::idesc_bf16(BM, (uint32_t)ncol, 0, 0);
-                        ptx::mma_ss_x4(s_tmem, q_desc0, b_desc, idesc, 0u, 2u);
-                        if (D == 128) ptx::mma_ss_x4(s_tmem, q_desc0 + (SLAB >> 4), b_desc + (1024 >> 4), idesc, 1u, 2u);
+                        ptx::mma_ts_x4(s_tmem, tmem + TM_Q, b_desc, idesc, 0u, 2u);
+                        if (D == 128) ptx::mma_ts_x4(s_tmem, tmem + TM_Q + 32u, b_desc + (1024 >> 4), idesc, 1u, 2u);
                     }
                     release(sk);
                     if (active) {
@@ -265,47 +258,44 @@ __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uin
                 __syncwarp();
             };
             issue_qk(0);
-            for (int j = 0; j < nt; ++j) {
+            if (nt > 1) issue_qk(1);
+            for (int t = 0; t < nt; ++t) {
                 if (*abort_flag) break;
-                if (j + 1 < nt) issue_qk(j + 1);
-                const uint32_t sv = NSTAGE + vst;
+                const uint32_t sv = NK + vst;
                 ptx::mbar_wait(bar(L::B_KV_FULL + sv), vph, abort_flag);
-                if (++vst == NSTAGE) { vst = 0; vph ^= 1u; }
-                DT(160 + (j & 15));
-                const int nv = nv_of(j);
+                if (++vst == NV) { vst = 0; vph ^= 1u; }
+                DT(160 + (t & 15));
+                const int nv = nv_of(t);
+                const uint32_t k = tcount + (uint32_t)t, j = k & 1u;
                 if (active) {
                     if (nv & 15) dec::zero_v_tail<D>(sbase + (uint32_t)(L::OFF_KV + sv * L::KV_BYTES), nv, (nv + 15) & ~15, lane);
-                    const uint32_t k = tcount + (uint32_t)j, sb = k & 1u;
-                    // the first PV of stream sb in this unit overwrites O[sb]: the previous unit's epilogue has read it
-                    if (j < 2 && ocount[sb] > 0) ptx::mbar_wait(bar(L::B_O_FREE + sb), (ocount[sb] - 1u) & 1u, abort_flag);
-                    ptx::mbar_wait(bar(L::B_P_FULL + sb), (k >> 1) & 1u, abort_flag);
+                    // the first PV of a unit overwrites O: the previous unit's epilogue has read it
+                    if (t == 0 && ocount > 0) ptx::mbar_wait(bar(L::B_O_FREE), (ocount - 1u) & 1u, abort_flag);
+                    ptx::mbar_wait(bar(L::B_P_FULL + j), (k >> 1) & 1u, abort_flag);
                 }
                 ptx::tc_fence_after();
                 DT(11);
                 if (ptx::elect_one()) {
                     if (active) {
-                        const uint32_t sb = (tcount + (uint32_t)j) & 1u;
-                        const uint32_t s_tmem = tmem + sb * 128u, o_tmem = tmem + 256u + sb * 128u;
+                        const uint32_t s_tmem = tmem + TM_S + j * 128u, o_tmem = tmem + TM_O;
                         const uint64_t b0 = v_desc0 + (uint64_t)(sv * (L::KV_BYTES >> 4));
                         const int ks_n = (nv + 15) >> 4;                       // one K-step = 16 kv rows = one page
                         if (ks_n == 8) {
-                            ptx::mma_ts_x4(o_tmem, s_tmem, b0, IDESC_PV, j > 1 ? 1u : 0u, VSTEP);
+                            ptx::mma_ts_x4(o_tmem, s_tmem, b0, IDESC_PV, t > 0 ? 1u : 0u, VSTEP);
                             ptx::mma_ts_x4(o_tmem, s_tmem + 64u, b0 + 4 * VSTEP, IDESC_PV, 1u, VSTEP);
                         } else {
                             for (int ks = 0; ks < ks_n; ++ks)       // P of page ks: half ks / 4, 8 packed columns per page inside the half
                                 ptx::mma_ts(o_tmem, s_tmem + (uint32_t)((ks >> 2) * 64 + (ks & 3) * 8), b0 + (uint64_t)(ks * VSTEP), IDESC_PV,
-                                            (j > 1 || ks > 0) ? 1u : 0u);
+                                            (t > 0 || ks > 0) ? 1u : 0u);
                         }
                     }
                     release(sv);
-                    if (active) ptx::mma_commit(bar(L::B_PV_DONE + ((tcount + (uint32_t)j) & 1u)));
+                    if (active) ptx::mma_commit(bar(L::B_PV_DONE + j));
                 }
                 __syncwarp();
+                if (t + 2 < nt) issue_qk(t + 2);
             }
-            if (active) {
-                if (nt >= 2) { ++ocount[0]; ++ocount[1]; } else { ++ocount[tcount & 1u]; }
-                tcount += (uint32_t)nt;
-            }
+            if (active) { ++ocount; tcount += (uint32_t)nt; }
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
@@ -315,7 +305,8 @@ __device__ __forceinline__ void mma_warp(const DecParams& p, uint32_t sbase, uin
 
 // ------------------------------------------------------------------------------------------------
 // warps 4..7 (group 0) and 8..11 (group 1): softmax; thread `row` of a group owns row `row` of the CTA's q tile (TMEM lane
-// `row`).  Group b processes the kv tiles of global parity b.  Group 0 then merges the two streams and runs the epilogue.
+// `row`).  Group h processes kv positions [64 h, 64 h + 64) of every tile (stream h).  Group 0 then merges the two streams and
+// runs the epilogue.
 // ------------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem, uint32_t sbase, uint32_t tmem, const Item* items,
@@ -327,10 +318,10 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
     const uint32_t wg = (uint32_t)(warp - 4) >> 2;             // stream of this group
     const int qd = warp & 3, row = qd * 32 + lane;
     const uint32_t lane_base = (uint32_t)(qd * 32) << 16;
-    const uint32_t s_taddr = tmem + lane_base + wg * 128u;     // S[wg]
-    const uint32_t o_taddr = tmem + lane_base + 256u + wg * 128u;   // O[wg]
-    const uint32_t o0_taddr = tmem + lane_base + 256u, o1_taddr = tmem + lane_base + 384u;
-    float2* ml_x = reinterpret_cast<float2*>(smem + L::OFF_ML);
+    const uint32_t s_taddr = tmem + lane_base + TM_S + wg * 64u;    // this group's half of S[0]; S[1] is 128 columns further
+    const uint32_t o_taddr = tmem + lane_base + TM_O;               // O
+    float* l_x = reinterpret_cast<float*>(smem + L::OFF_ML);        // [item slot][row]: group 1's half of the row sum
+    float* mx_x = reinterpret_cast<float*>(smem + L::OFF_MX);       // [tile parity][group][row]: half-tile row maxima
     volatile int* merge_flag = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 8);
     volatile int* agent_req = reinterpret_cast<volatile int*>(smem + L::OFF_MISC + 16);
     const float sc = fabsf(p.scale_log2);
@@ -390,9 +381,9 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
     };
 
     uint32_t icount = 0, tcount = 0;      // items seen; active kv tiles seen (global index)
-    // PV of global tile k signals PV_DONE[k & 1] (phase k >> 1).  A wait for tile k finds PV of the stream's previous tile
-    // complete (it precedes QK(k) on the in-order tensor pipe) and the stream's next one not yet issued (it needs this
-    // group's P), so the barrier is in phase k >> 1 or one further: a parity wait is unambiguous.
+    uint32_t qcount = 0;                   // units whose Q was stored (group 1)
+    // PV of global tile k signals PV_DONE[k & 1] (phase k >> 1); its commit covers every MMA issued before it.  A wait for tile
+    // k finds the barrier in phase k >> 1 or one before: the next PV that signals it needs the P of tile k + 2.
     auto wait_pv = [&](uint32_t k) { ptx::mbar_wait(bar(L::B_PV_DONE + (k & 1u)), (k >> 1) & 1u, abort_flag); };
     while (true) {
         if (*abort_flag) break;
@@ -409,120 +400,140 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
         if (wg == 0 && rows > 0 && !ref_ok(ref) && lane == 0) raise_flag(p.flags, DEV_INTERNAL | 0x400u);
         float m_ref = -INFINITY, l = 0.f;
         int peek = -1;
-        uint32_t k_last = 0;                    // global index of this group's last tile in the unit
-        int n_mine = 0;
-        for (int t = 0; t < nt; ++t) {
-            const uint32_t k = tcount + (uint32_t)t;
-            if ((k & 1u) != wg) continue;
-            if (*abort_flag) break;
-            int nv = c_lim - (it.pg0 + 8 * t) * SANGAM_PAGE;
-            nv = nv > BN ? BN : nv;
-            if (wg == 0 && t >= nt - 2 && it.part_slot >= 0 && qd == 0 && lane == 0)      // group 0's last tile of the unit
-                asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(peek) : "l"(p.unit_cnt + 2 * it.unit + (int)rank) : "memory");
-            ptx::mbar_wait(bar(L::B_S_FULL + wg), (k >> 1) & 1u, abort_flag);
+        uint32_t k_last = 0;                    // global index of the unit's last tile
+        if (wg == 1 && nt > 0) {
+            // group 1 (it has no epilogue, so it reaches the next unit first) stores the q tile into TMEM as the A operand of
+            // QK: row `row` = lane `row`, element pairs in consecutive columns.  Rows past the tile's tokens are zeros.
+            const __nv_bfloat16* qrow;
+            {
+                const int tl = p.G == 1 ? row : (int)__umulhi((uint32_t)row, p.g_magic), hh = row - tl * p.G;
+                const int tok = ref.q_start + ref.tok0 + (int)rank * p.tpt + tl;
+                qrow = p.q + ((int64_t)tok * p.Hq + (int64_t)ref.g * p.G + hh) * D;
+            }
+            uint4 qv[D / 8];
+#pragma unroll
+            for (int c = 0; c < D / 8; ++c) qv[c] = row_ok ? __ldg(reinterpret_cast<const uint4*>(qrow) + c) : make_uint4(0, 0, 0, 0);
+            ptx::mbar_wait(bar(L::B_Q_EMPTY), (qcount & 1u) ^ 1u, abort_flag);       // the previous unit's QKs have read theirs
             ptx::tc_fence_after();
-            DT(20);
-            // pass 1: the row's maximum over the tile (positions >= nv masked); the full-tile path has no per-element tests
-            float mx = -INFINITY;
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                if (nv - 64 * h <= 0) continue;
-                uint32_t r0[32], r1[32];
-                ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h), r0);
-                ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h + 32), r1);
-                ptx::tmem_wait_ld();
-                if (flip) {                                     // rare: scale < 0 -- work on -s with |scale|
+            for (int c = 0; c < D / 32; ++c) {
+                uint32_t w[16];
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) { r0[i] ^= 0x80000000u; r1[i] ^= 0x80000000u; }
-                }
-                const int lim = nv - 64 * h;
-                if (lim >= 64) {
-                    float t4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};       // four independent chains
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) t4[i & 3] = fmaxf(t4[i & 3], fmaxf(__uint_as_float(r0[i]), __uint_as_float(r1[i])));
-                    mx = fmaxf(mx, fmaxf(fmaxf(t4[0], t4[1]), fmaxf(t4[2], t4[3])));
-                } else {
-#pragma unroll
-                    for (int i = 0; i < 32; ++i)
-                        mx = fmaxf(mx, fmaxf(i < lim ? __uint_as_float(r0[i]) : -INFINITY, 32 + i < lim ? __uint_as_float(r1[i]) : -INFINITY));
-                }
+                for (int e = 0; e < 4; ++e) { w[4 * e] = qv[4 * c + e].x; w[4 * e + 1] = qv[4 * c + e].y; w[4 * e + 2] = qv[4 * c + e].z; w[4 * e + 3] = qv[4 * c + e].w; }
+                ptx::tmem_st16(tmem + lane_base + TM_Q + (uint32_t)(16 * c), w);
             }
-            mx *= sc;
-            const bool grow = mx > m_ref + LAZY_T;
-            const float m_new = grow ? mx : m_ref;
-            const float alpha = grow ? ptx::ex2(m_ref - m_new) : 1.f;
-            m_ref = m_new;
-            l *= alpha;
-            if (n_mine > 0 && __any_sync(FULL, alpha != 1.f)) {
-                // rare (lazy reference maximum): every PV of this stream so far must have landed in O before the rows shrink
-                wait_pv(k - 2u);
-                ptx::tc_fence_after();
-#pragma unroll 1
-                for (int c = 0; c < D / 32; ++c) {
-                    uint32_t o[32];
-                    ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
-                    ptx::tmem_wait_ld();
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
-                    ptx::tmem_st32(o_taddr + (uint32_t)(c * 32), o);
-                }
-                ptx::tmem_wait_st();
-            }
-            DT(21);
-            // pass 2: P = 2^(s scale - m_ref) as bf16 pairs over the first 32 columns of each half, row sum into l
-            // (packed fp32x2 arithmetic: one FFMA2 / FADD2 per two columns)
-            const float2 sc2 = make_float2(sc, sc), ng2 = make_float2(-m_ref, -m_ref);
-            float2 sum_a = make_float2(0.f, 0.f), sum_b = make_float2(0.f, 0.f);
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                if (nv - 64 * h <= 0) continue;
-                uint32_t r0[32], r1[32];
-                ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h), r0);
-                ptx::tmem_ld32(s_taddr + (uint32_t)(64 * h + 32), r1);
-                ptx::tmem_wait_ld();
-                if (flip) {
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) { r0[i] ^= 0x80000000u; r1[i] ^= 0x80000000u; }
-                }
-                const int lim = nv - 64 * h;
-                uint32_t pk[32];
-#pragma unroll
-                for (int i = 0; i < 32; i += 2) {
-                    const float2 xa = __ffma2_rn(make_float2(__uint_as_float(r0[i]), __uint_as_float(r0[i + 1])), sc2, ng2);
-                    const float2 xc = __ffma2_rn(make_float2(__uint_as_float(r1[i]), __uint_as_float(r1[i + 1])), sc2, ng2);
-                    float2 pa = make_float2(ptx::ex2(xa.x), ptx::ex2(xa.y)), pc = make_float2(ptx::ex2(xc.x), ptx::ex2(xc.y));
-                    if (lim < 64) {
-                        if (i >= lim) pa.x = 0.f;
-                        if (i + 1 >= lim) pa.y = 0.f;
-                        if (32 + i >= lim) pc.x = 0.f;
-                        if (33 + i >= lim) pc.y = 0.f;
-                    }
-                    sum_a = __fadd2_rn(sum_a, pa);
-                    sum_b = __fadd2_rn(sum_b, pc);
-                    pk[i >> 1] = ptx::pack_bf16(pa.x, pa.y);
-                    pk[16 + (i >> 1)] = ptx::pack_bf16(pc.x, pc.y);
-                }
-                ptx::tmem_st16(s_taddr + (uint32_t)(64 * h), pk);
-                ptx::tmem_st16(s_taddr + (uint32_t)(64 * h + 16), pk + 16);
-            }
-            const float2 sum2 = __fadd2_rn(sum_a, sum_b);
-            l += sum2.x + sum2.y;
             ptx::tmem_wait_st();
             ptx::tc_fence_before();
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL + wg));
-            DT(23);
-            k_last = k;
-            ++n_mine;
+            if (lane == 0) ptx::mbar_arrive(bar(L::B_Q_FULL));
+            ++qcount;
         }
-        const uint32_t t_start = tcount;
+        for (int t = 0; t < nt; ++t) {
+            const uint32_t k = tcount + (uint32_t)t;      // (no early exit on abort: the two groups meet at a barrier per tile)
+            int nv = c_lim - (it.pg0 + 8 * t) * SANGAM_PAGE;
+            nv = nv > BN ? BN : nv;
+            if (wg == 0 && t == nt - 1 && it.part_slot >= 0 && qd == 0 && lane == 0)      // the last tile of the unit
+                asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(peek) : "l"(p.unit_cnt + 2 * it.unit + (int)rank) : "memory");
+            {                                        // this group's half of the tile: kv positions [64 wg, 64 wg + 64) of S[k & 1]
+                const uint32_t j = k & 1u;
+                const uint32_t sh_taddr = s_taddr + j * 128u;
+                const int lim = nv - 64 * (int)wg;   // valid positions of the half (<= 0: the unit's ragged end)
+                ptx::mbar_wait(bar(L::B_S_FULL + j), (k >> 1) & 1u, abort_flag);
+                ptx::tc_fence_after();
+                DT(20);
+                uint32_t r0[32], r1[32];
+                float mx = -INFINITY;
+                if (lim > 0) {
+                    ptx::tmem_ld32(sh_taddr, r0);
+                    ptx::tmem_ld32(sh_taddr + 32u, r1);
+                    ptx::tmem_wait_ld();
+                    if (flip) {                                     // rare: scale < 0 -- work on -s with |scale|
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) { r0[i] ^= 0x80000000u; r1[i] ^= 0x80000000u; }
+                    }
+                    // the row's maximum over the half (positions >= lim masked); the full path has no per-element tests
+                    if (lim >= 64) {
+                        float t4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};       // four independent chains
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) t4[i & 3] = fmaxf(t4[i & 3], fmaxf(__uint_as_float(r0[i]), __uint_as_float(r1[i])));
+                        mx = fmaxf(fmaxf(t4[0], t4[1]), fmaxf(t4[2], t4[3]));
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i)
+                            mx = fmaxf(mx, fmaxf(i < lim ? __uint_as_float(r0[i]) : -INFINITY, 32 + i < lim ? __uint_as_float(r1[i]) : -INFINITY));
+                    }
+                    mx *= sc;
+                }
+                // the two threads of a row (one per group) exchange their halves' maxima: one reference maximum, one accumulator
+                // per row.  The exchange buffer alternates with the tile parity: a thread writes tile k + 2's maximum only after
+                // the barrier of tile k + 1, which its partner passes after reading tile k's.
+                mx_x[(j * 2u + wg) * BM + row] = mx;
+                ptx::bar_sync(2, 256);
+                mx = fmaxf(mx, mx_x[(j * 2u + (wg ^ 1u)) * BM + row]);
+                const bool grow = mx > m_ref + LAZY_T;
+                const float m_new = grow ? mx : m_ref;
+                const float alpha = grow ? ptx::ex2(m_ref - m_new) : 1.f;
+                m_ref = m_new;
+                l *= alpha;
+                if (wg == 0 && t > 0 && __any_sync(FULL, alpha != 1.f)) {
+                    // rare (lazy reference maximum): every PV so far must have landed in O before the rows shrink; group 0 does
+                    // it, and the PV of this tile is not issued before group 0 has handed its P
+                    wait_pv(k - 1u);
+                    ptx::tc_fence_after();
+#pragma unroll 1
+                    for (int c = 0; c < D / 32; ++c) {
+                        uint32_t o[32];
+                        ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), o);
+                        ptx::tmem_wait_ld();
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
+                        ptx::tmem_st32(o_taddr + (uint32_t)(c * 32), o);
+                    }
+                    ptx::tmem_wait_st();
+                }
+                DT(21);
+                if (lim > 0) {
+                    // P = 2^(s scale - m_ref) as bf16 pairs over the first 32 columns of the half, row sum into l
+                    // (packed fp32x2 arithmetic: one FFMA2 / FADD2 per two columns)
+                    const float2 sc2 = make_float2(sc, sc), ng2 = make_float2(-m_ref, -m_ref);
+                    float2 sum_a = make_float2(0.f, 0.f), sum_b = make_float2(0.f, 0.f);
+                    uint32_t pk[32];
+#pragma unroll
+                    for (int i = 0; i < 32; i += 2) {
+                        const float2 xa = __ffma2_rn(make_float2(__uint_as_float(r0[i]), __uint_as_float(r0[i + 1])), sc2, ng2);
+                        const float2 xc = __ffma2_rn(make_float2(__uint_as_float(r1[i]), __uint_as_float(r1[i + 1])), sc2, ng2);
+                        float2 pa = make_float2(ptx::ex2(xa.x), ptx::ex2(xa.y)), pc = make_float2(ptx::ex2(xc.x), ptx::ex2(xc.y));
+                        if (lim < 64) {
+                            if (i >= lim) pa.x = 0.f;
+                            if (i + 1 >= lim) pa.y = 0.f;
+                            if (32 + i >= lim) pc.x = 0.f;
+                            if (33 + i >= lim) pc.y = 0.f;
+                        }
+                        sum_a = __fadd2_rn(sum_a, pa);
+                        sum_b = __fadd2_rn(sum_b, pc);
+                        pk[i >> 1] = ptx::pack_bf16(pa.x, pa.y);
+                        pk[16 + (i >> 1)] = ptx::pack_bf16(pc.x, pc.y);
+                    }
+                    ptx::tmem_st16(sh_taddr, pk);
+                    ptx::tmem_st16(sh_taddr + 16u, pk + 16);
+                    const float2 sum2 = __fadd2_rn(sum_a, sum_b);
+                    l += sum2.x + sum2.y;
+                    ptx::tmem_wait_st();
+                }
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(bar(L::B_P_FULL + j));
+                DT(23);
+            }
+            k_last = k;
+        }
         tcount += (uint32_t)nt;
         if (wg == 1) {
-            // group 1 hands its stream's row statistics to group 0 (double-buffered by item slot: the slot is not reused
+            // group 1 hands its half of the row sums to group 0 (double-buffered by item slot: the slot is not reused
             // before group 0 has released the item) and is done with the unit
             // (one EPI barrier per item slot, used for every item: group 1 may run a whole item ahead of group 0, and a
             // parity wait cannot tell phases two apart)
-            ml_x[islot * BM + row] = make_float2(m_ref, l);
+            l_x[islot * BM + row] = l;
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(bar(L::B_EPI + islot));
             __syncwarp();
@@ -539,7 +550,7 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
         bool early = false;
         if (split) {
             if (qd == 0 && lane == 0) {
-                if (peek < 0 || n_mine == 0) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(peek) : "l"(p.unit_cnt + 2 * it.unit + (int)rank) : "memory");
+                if (peek < 0) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(peek) : "l"(p.unit_cnt + 2 * it.unit + (int)rank) : "memory");
                 const int e = (np_u == 2 && (k_me == 0 || k_me == 1) && peek + npg == it.upages) ? 1 : 0;
                 if (e) asm volatile("fence.acq_rel.gpu;" ::: "memory");
                 *merge_flag = e;
@@ -560,19 +571,12 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
             const int other = (k_me == 0 ? 2 * (it.b_head + 1) : 2 * it.b_head + 1) * 2 + (int)rank;
             float2 xo = make_float2(-INFINITY, 0.f);
             if (early) xo = __ldcg(reinterpret_cast<const float2*>(p.part_ml) + (int64_t)other * BM + row);
-            // the two streams of this unit: which had tiles, their last PVs, stream 1's statistics
-            const bool has0 = n_mine > 0, has1 = nt >= 2 || !has0;
-            const uint32_t k1 = ((t_start + (uint32_t)nt - 1u) & 1u) ? t_start + (uint32_t)nt - 1u : t_start + (uint32_t)nt - 2u;   // stream 1's last tile
-            const float2 x1 = ml_x[islot * BM + row];
-            if (has0) wait_pv(k_last);
-            if (has1) wait_pv(k1);
+            wait_pv(k_last);                                     // the unit's last PV (its commit covers all before it)
             ptx::tc_fence_after();
             DT(27);
-            // own piece = the two streams merged: M_own, weights, l_own
-            const float m0 = has0 ? m_ref : -INFINITY, m1 = has1 ? x1.x : -INFINITY;
-            const float m_own = fmaxf(m0, m1);
-            const float u0 = has0 ? ptx::ex2(m0 - m_own) : 0.f, u1 = has1 ? ptx::ex2(m1 - m_own) : 0.f;
-            const float l_own = fmaf(x1.y, u1, l * u0);
+            // own piece: the row's reference maximum is common to the two groups, the row sum is the sum of their halves
+            const float m_own = m_ref;
+            const float l_own = l + l_x[islot * BM + row];
             const bool partial = split && !early;
             const bool slot_ok = !partial || (it.part_slot * 2 + (int)rank < NS && it.unit >= 0);
             if (!slot_ok && lane == 0) raise_flag(p.flags, DEV_INTERNAL | 0x100u);
@@ -586,29 +590,19 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
             }
 #pragma unroll 1
             for (int c = 0; c < D / 32; ++c) {
-                uint32_t oa[32], ob[32];
                 float4 ov[8];
                 if (early) {
                     const float4* so = reinterpret_cast<const float4*>(p.part_o) + (int64_t)other * SLOT_F4 + (int64_t)(c * 8) * BM + row;
 #pragma unroll
                     for (int v = 0; v < 8; ++v) ov[v] = __ldcg(so + v * BM);
                 }
-                // a stream without tiles contributes zeros (its accumulator was never written): no per-element branches
-                if (has0) ptx::tmem_ld32(o0_taddr + (uint32_t)(c * 32), oa);
-                else {
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) oa[e] = 0u;
-                }
-                if (has1) ptx::tmem_ld32(o1_taddr + (uint32_t)(c * 32), ob);
-                else {
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) ob[e] = 0u;
-                }
+                uint32_t oa[32];
+                ptx::tmem_ld32(o_taddr + (uint32_t)(c * 32), oa);
                 ptx::tmem_wait_ld();
                 DT(34);
-                float a[32];                                     // this piece's unnormalised row chunk, both streams
+                float a[32];                                     // this piece's unnormalised row chunk
 #pragma unroll
-                for (int e = 0; e < 32; ++e) a[e] = fmaf(__uint_as_float(ob[e]), u1, __uint_as_float(oa[e]) * u0);
+                for (int e = 0; e < 32; ++e) a[e] = __uint_as_float(oa[e]);
                 float f[32];
                 if (early) {
 #pragma unroll
@@ -646,8 +640,7 @@ __device__ __forceinline__ void softmax_warps(const DecParams& p, uint8_t* smem,
             __syncwarp();
             DT(28);
             if (lane == 0) {                                     // both accumulators have been read
-                if (has0) ptx::mbar_arrive(bar(L::B_O_FREE));
-                if (has1) ptx::mbar_arrive(bar(L::B_O_FREE + 1));
+                ptx::mbar_arrive(bar(L::B_O_FREE));
             }
             if (partial && slot_ok && row < rows) reinterpret_cast<float2*>(p.part_ml)[(int64_t)slot * BM + row] = make_float2(m_own, l_own);
             if (split) {
@@ -726,7 +719,7 @@ __device__ __forceinline__ void agent_warp(const DecParams& p, uint8_t* smem, ui
 template <int D>
 __global__ void __launch_bounds__(NTHREADS, 1)
 gqa_decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
-                  const __grid_constant__ CUtensorMap mapQ, const DecParams p) {
+                  const __grid_constant__ CUtensorMap /* q map: unused, q rows are read directly */, const DecParams p) {
     using L = Smem<D>;
     // both CTAs of the pair use the same offsets inside their shared-memory windows (a multicast write lands at the issuing
     // CTA's offset in every destination): the dynamic base is the same in every CTA of a launch (no static shared memory)
@@ -740,29 +733,24 @@ gqa_decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constan
     TRACE_CTA(0);
     if (tid == 0) {
         auto bar = [&](int i) { return sbase + (uint32_t)(L::OFF_BAR + i * 8); };
-        for (int s = 0; s < 2 * NSTAGE; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 2); }   // both CTAs release
+        for (int s = 0; s < NK + NV; ++s) { ptx::mbar_init(bar(L::B_KV_FULL + s), 1); ptx::mbar_init(bar(L::B_KV_EMPTY + s), 2); }   // both CTAs release
         for (int s = 0; s < 2; ++s) {
             ptx::mbar_init(bar(L::B_ITEM_FULL + s), 1); ptx::mbar_init(bar(L::B_ITEM_EMPTY + s), 11);     // MMA warp + V producer + agent + 8 softmax warps
-            ptx::mbar_init(bar(L::B_S_FULL + s), 1); ptx::mbar_init(bar(L::B_P_FULL + s), 4);
-            ptx::mbar_init(bar(L::B_PV_DONE + s), 1); ptx::mbar_init(bar(L::B_O_FREE + s), 4);
+            ptx::mbar_init(bar(L::B_S_FULL + s), 1); ptx::mbar_init(bar(L::B_P_FULL + s), 8);             // both groups hand their half of P
+            ptx::mbar_init(bar(L::B_PV_DONE + s), 1);
         }
-        ptx::mbar_init(bar(L::B_Q_FULL), 1); ptx::mbar_init(bar(L::B_Q_EMPTY), 1);
+        ptx::mbar_init(bar(L::B_O_FREE), 4);
+        ptx::mbar_init(bar(L::B_Q_FULL), 4); ptx::mbar_init(bar(L::B_Q_EMPTY), 1);      // group 1's warps store the q tile
         ptx::mbar_init(bar(L::B_EPI), 4); ptx::mbar_init(bar(L::B_EPI + 1), 4);
         ptx::mbar_init(bar(L::B_AGENT_REQ), 4); ptx::mbar_init(bar(L::B_AGENT_DONE), 1);
         for (int k = 1; k < (L::TOTAL - L::OFF_MISC) / 4; ++k) tmem_slot[k] = 0u;
         ptx::fence_mbar_init();
         ptx::prefetch_tensormap(&mapK);
         ptx::prefetch_tensormap(&mapV);
-        ptx::prefetch_tensormap(&mapQ);
     }
     if (warp == 1) {
         ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
         ptx::tmem_relinquish();
-    }
-    if (warp >= 4) {       // rows of the q tile that no TMA box writes (tpt G < 128) stay zero
-        for (int e = tid - 128; e < L::Q_BYTES / 16; e += 256)
-            asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(sbase + (uint32_t)(L::OFF_Q + e * 16)), "r"(0) : "memory");
-        ptx::fence_proxy_async_smem();
     }
     ptx::pdl_wait();
     ptx::pdl_trigger();
@@ -780,7 +768,7 @@ gqa_decode_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constan
     } else {
         ptx::setmaxnreg_dec<88>();
         if (!base_ok) { }
-        else if (warp == 0) producer_warp<D>(p, &mapK, &mapQ, sbase, items, abort_flag, lane, rank);
+        else if (warp == 0) producer_warp<D>(p, &mapK, sbase, items, abort_flag, lane, rank);
         else if (warp == 3) v_producer_warp<D>(p, &mapV, sbase, items, abort_flag, lane, rank);
         else if (warp == 1) mma_warp<D>(p, sbase, tmem, items, abort_flag, lane, rank);
         else if (warp == 2) agent_warp<D>(p, smem, sbase, items, abort_flag, lane, rank);

@@ -416,6 +416,7 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
         DecParams d = {};
         d.block_table = block_table; d.cu_q_lens = cu_q_lens; d.ctx_lens = ctx_lens;
         d.out = (__nv_bfloat16*)out;
+        d.q = (const __nv_bfloat16*)q;
         d.batch = batch; d.total_q = total_q;
         d.Hq = c.num_q_heads; d.Hkv = c.num_kv_heads; d.G = ctx->G; d.W = c.max_pages_per_req; d.P = c.num_pages;
         d.tpt = tpt;
