@@ -62,13 +62,8 @@ def nsets_for(b):
 
 
 def sources_hash():
-    """sha256 over the CUDA sources: profiles/traffic.json records the hash of the build its ncu numbers came from."""
-    import hashlib
-    h = hashlib.sha256()
-    d = os.path.join(ROOT, "paper_2607_04206_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        h.update(open(os.path.join(d, f), "rb").read())
-    return h.hexdigest()[:16]
+    from paper_2607_04206_b200.build import sources_hash as h
+    return h()
 
 
 def load_peaks():
@@ -507,8 +502,9 @@ def main():
         ach = b.flops() / (attn_ms * 1e-3) / 1e12
         roof = {"bound": "tensor", "achieved": round(ach, 1), "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                 "frac": round(ach / peaks["bf16_tflops"], 4)}
-    kernel_name = ("dec::decode_kernel (device-side plan, swapped-operand attention, fused split-KV merge)" if kernels_per_step == 2
-                   else "tc::attn_kernel (device-side plan inside) + tc::combine_kernel")
+    kernel_name = {1: "tc::attn_kernel (two-stream kernel, device-side plan inside) + tc::combine_kernel",
+                   2: "dec::decode_kernel (device-side plan, swapped-operand attention, fused split-KV merge)",
+                   3: "gqa::gqa_decode_kernel (CTA pairs, K/V tiles multicast, fused split-KV merge)"}.get(w.eng.query(4), "?")
     roof.update({"traffic": traffic, "traffic_sources_hash": tj.get("sources_hash"), "traffic_matches_this_build": tj.get("sources_hash") == sources_hash(),
                  "kernel": kernel_name + ", timed alone over the same rotation",
                  "kernel_us": round(attn_ms * 1e3, 3), "peak_source": peaks["source"] + " (burst)",

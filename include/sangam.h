@@ -171,6 +171,8 @@ int sangam_set_dispatch(sangam_ctx* ctx, int32_t mode);
 #define SANGAM_QUERY_DECODE_CTAS_PER_SM  1   /* resident CTAs per SM of the decode kernel (0: kernel unavailable) */
 #define SANGAM_QUERY_DISPATCH            2   /* current SANGAM_DISPATCH_* mode */
 #define SANGAM_QUERY_GQA_PAIR_KERNEL     3   /* 1 if the CTA-pair decode kernel exists for the geometry */
+#define SANGAM_QUERY_LAST_KERNEL         4   /* SANGAM_DISPATCH_PREFILL / DECODE / GQA_PAIR: the kernel the last sangam_block_attn
+                                               launched (what AUTO chose); 0 before the first call */
 int32_t sangam_query(const sangam_ctx* ctx, int32_t what);
 
 /*

@@ -197,7 +197,8 @@ class Sangam:
         self._check(self.lib.sangam_set_dispatch(self.ctx, int(mode)))
 
     def query(self, what: int) -> int:
-        """0: SM count, 1: decode-kernel CTAs per SM, 2: dispatch mode."""
+        """0: SM count, 1: decode-kernel CTAs per SM, 2: dispatch mode, 3: 1 if the CTA-pair GQA kernel exists for the
+        geometry, 4: the kernel the last block_attn launched (DISPATCH_PREFILL / DECODE / GQA_PAIR, 0 before the first)."""
         return int(self.lib.sangam_query(self.ctx, int(what)))
 
     def device_status(self) -> int:

@@ -19,6 +19,18 @@ def _newest_source() -> float:
     return t
 
 
+def sources_hash() -> str:
+    """sha256 (first 16 hex digits) over csrc/: profiles/traffic.json records the hash of the build its ncu numbers came from,
+    bench.py compares it with the sources it runs."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(HERE, "csrc")
+    for f in sorted(os.listdir(d)):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source():
         return LIB

@@ -57,26 +57,6 @@ struct DecParams {
 
 namespace dec {
 
-#ifdef SANGAM_TRACE
-// debug builds: per-warp event trace of one CTA; the event index lives in a register of the role function (DT_DECL), so an
-// event costs one clock read and one store
-__device__ __forceinline__ void dtrace(const DecParams& p, unsigned ev, unsigned& i) {
-    if ((int)blockIdx.x == p.trace_cta && (threadIdx.x & 31) == 0) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %%clock64;" : "=l"(t));
-        const unsigned w = threadIdx.x >> 5;
-        if (i < SANGAM_TRACE_CAP) g_trace[w * SANGAM_TRACE_CAP + i] = (t << 16) | ((unsigned long long)w << 8) | ev;
-        ++i;
-        g_trace_n[w] = i;
-    }
-}
-#define DT_DECL unsigned dt_i_ = 0
-#define DT(ev) dtrace(p, ev, dt_i_)
-#else
-#define DT_DECL [[maybe_unused]] unsigned dt_i_ = 0
-#define DT(ev) ((void)0)
-#endif
-
 constexpr int BN = 128;          // kv positions per tile (UMMA M; 8 pages)
 constexpr int NQ = 32;           // packed query rows per unit (UMMA N)
 constexpr int NSTAGE = 3;        // ring of K / V tiles

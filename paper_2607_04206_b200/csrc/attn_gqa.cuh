@@ -31,9 +31,6 @@ using dec::Deferred;
 using dec::Item;
 using dec::OutRef;
 using dec::Planner;
-#ifdef SANGAM_TRACE
-using dec::dtrace;
-#endif
 
 constexpr int BM = 128;          // rows of a q tile (UMMA M)
 constexpr int BN = 128;          // kv positions per tile (8 pages)

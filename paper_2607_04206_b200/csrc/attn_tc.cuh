@@ -52,9 +52,6 @@ constexpr int DYN_UNITS_PER_CTA = SANGAM_DYN_UNITS;   // >= this many units per 
 #endif
 constexpr int UNIT_OV = SANGAM_UNIT_OV;  // static partition: fixed cost of starting/finishing a unit, in kv-tile equivalents
 constexpr float LAZY_T = 8.f;    // the reference maximum moves only when a tile exceeds it by 2^8
-#ifndef SANGAM_POLY_EXP
-#define SANGAM_POLY_EXP 0        // of every 8 exponentials, this many run on the FMA pipe instead of MUFU
-#endif
 
 struct Item {          // one piece of work, published through shared memory (64 bytes)
     int valid;         // 0 = no more work
@@ -705,18 +702,6 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
 // warps 0-7: softmax warpgroups (a6) + epilogue (a8) + fused split-KV merge (a9).
 // Thread `row` of stream s owns TMEM lane `row` of S_s / O_s.
 // ------------------------------------------------------------------------------------------------
-// 2^x on the FMA pipe (Cody-Waite split + degree-3 minimax on [-0.5, 0.5], rel. error 7.6e-5 --
-// far below the bf16 rounding of P); relieves the 16/clk/SM MUFU unit, the co-critical pipe of prefill.
-__device__ __forceinline__ float ex2_poly(float x) {
-    x = fmaxf(x, -125.f);
-    const float t = x + 12582912.f;            // 1.5 * 2^23: round(x) sits in the low mantissa bits
-    const float f = x - (t - 12582912.f);
-    float y = fmaf(f, 0.05520550534129143f, 0.24261397123336792f);
-    y = fmaf(y, f, 0.6932547688484192f);
-    y = fmaf(y, f, 0.9999276995658875f);
-    return __int_as_float(__float_as_int(y) + (__float_as_int(t) << 23));
-}
-
 // One 64-column half tile of one row: returns alpha (the factor by which O and l shrink; 1 if the
 // reference maximum m_ref stays).  m_ref is in log2 units and is only raised when the half's maximum
 // exceeds it by more than LAZY_T, so p = 2^(x - m_ref) <= 2^LAZY_T: exact in range for bf16 / fp32.
@@ -764,8 +749,8 @@ __device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float sc
         for (int i = 0; i < 16; ++i) {
             const float2 x = __ffma2_rn(make_float2(__uint_as_float(r[c][2 * i]), __uint_as_float(r[c][2 * i + 1])), sc2, ng2);
             float2 pp;
-            pp.x = ((2 * i) & 7) < SANGAM_POLY_EXP ? ex2_poly(x.x) : ptx::ex2(x.x);
-            pp.y = ((2 * i + 1) & 7) < SANGAM_POLY_EXP ? ex2_poly(x.y) : ptx::ex2(x.y);
+            pp.x = ptx::ex2(x.x);
+            pp.y = ptx::ex2(x.y);
             if (MASK) {
                 if (c * 32 + 2 * i >= nv) pp.x = 0.f;
                 if (c * 32 + 2 * i + 1 >= nv) pp.y = 0.f;

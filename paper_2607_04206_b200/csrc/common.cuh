@@ -58,48 +58,4 @@ static inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, unsigned
     return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
-// Optional event trace of CTA 0 (debug builds with -DSANGAM_TRACE only; compiled out otherwise).
-#ifdef SANGAM_TRACE
-#define SANGAM_TRACE_CAP 8192            // events per warp
-__device__ unsigned long long g_trace[16 * SANGAM_TRACE_CAP];
-__device__ unsigned int g_trace_n[16];
-__device__ unsigned long long g_cta_times[2 * 512];   // per CTA: %globaltimer at entry / exit
-__device__ unsigned int g_trace_cta;     // which CTA records (sangam_trace_set_cta)
-__device__ __forceinline__ unsigned int* trace_cnt() {
-    __shared__ unsigned int cnt[17];      // [16] = 1 if this CTA records (g_trace_cta read once: a global read per event costs an L2 trip)
-    return cnt;
-}
-__device__ __forceinline__ void trace_ev(unsigned ev) {
-    unsigned int* cnt = trace_cnt();
-    if (cnt[16] && (threadIdx.x & 31) == 0) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %%clock64;" : "=l"(t));
-        const unsigned w = threadIdx.x >> 5, i = cnt[w];
-        cnt[w] = i + 1;
-        if (i < SANGAM_TRACE_CAP) g_trace[w * SANGAM_TRACE_CAP + i] = (t << 16) | ((unsigned long long)w << 8) | ev;
-        g_trace_n[w] = i + 1;
-    }
-}
-// same record, but the time stamp is %globaltimer (ns): start/end pair gives the effective SM clock
-__device__ __forceinline__ void trace_ns(unsigned ev) {
-    unsigned int* cnt = trace_cnt();
-    if (cnt[16] && (threadIdx.x & 31) == 0) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-        const unsigned w = threadIdx.x >> 5, i = cnt[w];
-        cnt[w] = i + 1;
-        if (i < SANGAM_TRACE_CAP) g_trace[w * SANGAM_TRACE_CAP + i] = (t << 16) | ((unsigned long long)w << 8) | ev;
-        g_trace_n[w] = i + 1;
-    }
-}
-#define TRACE_EV(ev) trace_ev(ev)
-#define TRACE_NS(ev) trace_ns(ev)
-// bits 63..54 of the entry stamp carry %smid (the timer's high bits are constant over a launch: the host masks them off)
-#define TRACE_CTA(which) do { if (threadIdx.x == 0 && blockIdx.x < 512) { unsigned long long t_; unsigned sm_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm_)); g_cta_times[2 * blockIdx.x + (which)] = (which) ? t_ : ((t_ & 0x003fffffffffffffull) | ((unsigned long long)sm_ << 54)); } } while (0)
-#define TRACE_INIT() do { if (threadIdx.x < 16) trace_cnt()[threadIdx.x] = 0; if (threadIdx.x == 16) trace_cnt()[16] = blockIdx.x == g_trace_cta; __syncthreads(); } while (0)
-#else
-#define TRACE_EV(ev) ((void)0)
-#define TRACE_NS(ev) ((void)0)
-#define TRACE_CTA(which) ((void)0)
-#define TRACE_INIT() ((void)0)
-#endif
+#include "trace.cuh"     // debug event trace: every macro is empty unless built with -DSANGAM_TRACE

@@ -39,6 +39,7 @@ struct sangam_ctx {
     int dec_occ;
     int gqa_ok;                   // GQA pair kernel (attn_gqa.cuh) available for this geometry
     int dispatch;                 // SANGAM_DISPATCH_*
+    int last_kernel;              // SANGAM_DISPATCH_PREFILL / DECODE / GQA_PAIR: what the last sangam_block_attn launched (0: nothing yet)
     float* d_dec_part_o;
     float* d_dec_part_ml;
     int32_t* d_dec_cnt;
@@ -438,9 +439,11 @@ extern "C" int sangam_block_attn(sangam_ctx* ctx, const void* q, const void* k_p
                                 : dec_launch(d, kv->mk, kv->mv, qm->dec, c.head_dim, ctx->dec_occ * ctx->sm_count, (cudaStream_t)stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, use_gqa ? "block_attn launch (GQA pair kernel)" : "block_attn launch (decode kernel)");
         ctx->launches += 1;
+        ctx->last_kernel = use_gqa ? SANGAM_DISPATCH_GQA_PAIR : SANGAM_DISPATCH_DECODE;
         return SANGAM_OK;
     }
     AttnParams p = make_params(ctx, q, k_pages, v_pages, block_table, cu_q_lens, ctx_lens, batch, total_q, scale, out);
+    ctx->last_kernel = SANGAM_DISPATCH_PREFILL;
     int launched = 0;
     cudaError_t e = tc_launch(p, kv->mk, kv->mv, qm->main, c.head_dim, ctx->sm_count, (cudaStream_t)stream, &launched);
     ctx->launches += launched;
@@ -455,6 +458,7 @@ extern "C" int32_t sangam_query(const sangam_ctx* ctx, int32_t what) {
         case SANGAM_QUERY_DECODE_CTAS_PER_SM: return ctx->dec_occ;
         case SANGAM_QUERY_DISPATCH: return ctx->dispatch;
         case SANGAM_QUERY_GQA_PAIR_KERNEL: return ctx->gqa_ok;
+        case SANGAM_QUERY_LAST_KERNEL: return ctx->last_kernel;
         default: return -1;
     }
 }
@@ -588,29 +592,3 @@ extern "C" int sangam_debug_timeout_info(unsigned int* out20) {
 }
 #endif
 
-#ifdef SANGAM_TRACE
-extern "C" int sangam_trace_cta_times(unsigned long long* host_buf) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(host_buf, g_cta_times, sizeof(unsigned long long) * 1024);
-    return 0;
-}
-extern "C" int sangam_trace_set_cta(int cta) {
-    unsigned int v = (unsigned int)cta, z[16] = {0};
-    cudaDeviceSynchronize();
-    cudaMemcpyToSymbol(g_trace_cta, &v, sizeof v);
-    cudaMemcpyToSymbol(g_trace_n, z, sizeof z);
-    return 0;
-}
-// debug builds only: copy the event trace of the recording CTA (per-warp rings, concatenated) to the host
-extern "C" int sangam_trace_read(unsigned long long* host_buf, int cap) {
-    unsigned int n[16];
-    static unsigned long long tmp[16 * SANGAM_TRACE_CAP];
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(n, g_trace_n, sizeof n);
-    cudaMemcpyFromSymbol(tmp, g_trace, sizeof tmp);
-    int k = 0;
-    for (int w = 0; w < 16; ++w)
-        for (unsigned i = 0; i < n[w] && i < SANGAM_TRACE_CAP && k < cap; ++i) host_buf[k++] = tmp[w * SANGAM_TRACE_CAP + i];
-    return k;
-}
-#endif
