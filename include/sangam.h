@@ -137,6 +137,26 @@ int sangam_confidence_sample(sangam_ctx* ctx, const void* logits, int32_t vocab,
                              int32_t* unmask, void* stream);
 
 /*
+ * The same sampler for callers that must not allocate (code under CUDA-graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): no ctx, and the call performs no cudaMalloc / cudaFree and no allocating library routine.
+ * sangam_confidence_sample allocates its scratch lazily on first use; here the per-(row, vocabulary slice) partials live
+ * in a file-scope device array inside the library, SANGAM_STATIC_SAMPLER_MAX_PARTIALS entries of 16 bytes = 1 MiB,
+ * which every GPU that loads the library holds until the process exits.  Same arguments, same results (bit-identical
+ * when the slicing coincides, else within fp32 rounding of conf) as sangam_confidence_sample, on the caller's CURRENT
+ * device.  Limit: num_rows <= SANGAM_STATIC_SAMPLER_MAX_ROWS, else SANGAM_ERR_WORKSPACE and nothing is launched (use
+ * sangam_confidence_sample for larger batches).  Every call on a device shares the one array; nothing in it has to be
+ * cleared between calls (each call writes every entry it later reads), but two calls whose kernels overlap on the GPU
+ * (different streams without an event between them, concurrently launched graphs) race on it: serialise them.
+ * Errors: return code as above; the message of the calling thread's last failure from sangam_static_last_error().
+ */
+#define SANGAM_STATIC_SAMPLER_MAX_PARTIALS 65536
+#define SANGAM_STATIC_SAMPLER_MAX_ROWS     4096
+int sangam_confidence_sample_static(const void* logits, int32_t vocab, const int32_t* masked, const int32_t* cu_rows,
+                                    int32_t num_requests, int32_t num_rows, float threshold, int32_t* token, float* conf,
+                                    int32_t* unmask, void* stream);
+const char* sangam_static_last_error(void);
+
+/*
  * Block attention (steps a3-a9): for request r < batch, row t in [cu_q_lens[r], cu_q_lens[r+1]),
  * q head h, kv head g = h / G, context length c = ctx_lens[r]:
  *   s_j = scale * <q[t][h], K_r[j][g]>, j < c;   out[t][h] = sum_j softmax_j(s) V_r[j][g]

@@ -5,4 +5,5 @@ of the path runs in the CUDA kernels of csrc/.  There is no CPU fallback -- if l
 missing or a CUDA device is absent the calls raise.
 """
 from .binding import (SangamError, Sangam, Scheduler, rope_table, load_library, exported_symbols, DECLARED_SYMBOLS,  # noqa: F401
-                      DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE, DISPATCH_GQA_PAIR)
+                      DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE, DISPATCH_GQA_PAIR,
+                      confidence_sample_static, STATIC_SAMPLER_MAX_ROWS, STATIC_SAMPLER_MAX_PARTIALS)

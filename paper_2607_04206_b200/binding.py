@@ -15,6 +15,7 @@ DECLARED_SYMBOLS = [
     "sangam_sched_create", "sangam_sched_destroy", "sangam_sched_submit", "sangam_sched_next", "sangam_sched_complete",
     "sangam_sched_query", "sangam_packed_layout", "sangam_iteration_packed",
     "sangam_kv_write_rope", "sangam_confidence_sample", "sangam_kv_gather", "sangam_kv_scatter",
+    "sangam_confidence_sample_static", "sangam_static_last_error",
 ]
 
 DISPATCH_AUTO, DISPATCH_PREFILL, DISPATCH_DECODE, DISPATCH_GQA_PAIR = 0, 1, 2, 3
@@ -77,6 +78,8 @@ def load_library(build_if_missing: bool = False):
     lib.sangam_iteration_packed.argtypes = [vp, vp, i32, vp, vp, i32, i32, f32, vp, vp]
     lib.sangam_kv_write_rope.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, vp, vp, vp]
     lib.sangam_confidence_sample.argtypes = [vp, vp, i32, vp, vp, i32, i32, f32, vp, vp, vp, vp]
+    lib.sangam_confidence_sample_static.argtypes = [vp, i32, vp, vp, i32, i32, f32, vp, vp, vp, vp]
+    lib.sangam_static_last_error.restype = ctypes.c_char_p
     lib.sangam_kv_gather.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp]
     lib.sangam_kv_scatter.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp]
     lib.sangam_sched_create.argtypes = [ctypes.POINTER(_SchedConfig), ctypes.POINTER(vp)]
@@ -103,6 +106,20 @@ def _stream(stream):
     import torch
     s = stream if stream is not None else torch.cuda.current_stream()
     return ctypes.c_void_p(s.cuda_stream)
+
+
+STATIC_SAMPLER_MAX_ROWS, STATIC_SAMPLER_MAX_PARTIALS = 4096, 65536      # include/sangam.h
+
+
+def confidence_sample_static(logits, masked, cu_rows, threshold, token, conf, unmask, stream=None):
+    """sangam_confidence_sample_static: the sampler without a ctx and without any allocation (its scratch is a 1 MiB
+    static device array inside the library); same arguments and results as Sangam.confidence_sample, on the current
+    device, rows <= STATIC_SAMPLER_MAX_ROWS.  Calls that overlap on the GPU race on the shared scratch."""
+    lib = load_library()
+    rc = lib.sangam_confidence_sample_static(_ptr(logits), int(logits.shape[1]), _ptr(masked), _ptr(cu_rows), int(cu_rows.numel()) - 1,
+                                             int(logits.shape[0]), float(threshold), _ptr(token), _ptr(conf), _ptr(unmask), _stream(stream))
+    if rc != 0:
+        raise SangamError(f"sangam error {rc}: {lib.sangam_static_last_error().decode()}")
 
 
 def rope_table(max_pos: int, head_dim: int, base: float = 10000.0):

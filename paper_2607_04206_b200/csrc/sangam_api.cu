@@ -8,6 +8,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 
 #include "attn_dec.cuh"
@@ -592,3 +593,89 @@ extern "C" int sangam_debug_timeout_info(unsigned int* out20) {
 }
 #endif
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// sangam_confidence_sample_static: the confidence sampler for callers that must not allocate (CUDA-graph capture,
+// tight serving loops, harnesses that forbid cudaMalloc).  No ctx, no cudaMalloc / cudaFree, no allocating library
+// call: the per-(row, vocabulary slice) partials of pass 1 live in the file-scope device array below, which every
+// GPU that loads the library holds until the process exits (SANGAM_STATIC_SAMPLER_MAX_PARTIALS * 16 B = 1 MiB).
+// In host code `g_static_conf_part` is only a host-side stand-in for the symbol, NOT a device address: the device
+// address is taken once per device, with that device current, by cudaGetSymbolAddress, and that pointer is what the
+// kernels receive.
+// Every call on a device shares the one array and finds the previous call's contents in it.  Nothing has to start
+// at zero: pass 1 writes every (row, slice) entry that pass 2 of the same call reads, and no entry outside
+// [0, num_rows * slices) is read.  Two calls whose kernels overlap on the GPU (different streams, or graphs
+// launched concurrently) race on the array: callers serialise them (same stream, or an event between them).
+// ---------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) ConfPartial g_static_conf_part[SANGAM_STATIC_SAMPLER_MAX_PARTIALS];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticSamplerDev {
+    ConfPartial* part;       // device address of g_static_conf_part on this device
+    int sm_count;
+    bool ready;
+};
+StaticSamplerDev g_static_dev[STATIC_MAX_DEVICES];
+std::mutex g_static_mu;
+thread_local char g_static_err[256] = "";
+
+int static_fail(int code, const char* msg, const char* detail = "") {
+    snprintf(g_static_err, sizeof g_static_err, "%s%s", msg, detail);
+    return code;
+}
+}  // namespace
+
+extern "C" const char* sangam_static_last_error(void) { return g_static_err; }
+
+extern "C" int sangam_confidence_sample_static(const void* logits, int32_t vocab, const int32_t* masked, const int32_t* cu_rows,
+                                               int32_t num_requests, int32_t num_rows, float threshold, int32_t* token, float* conf,
+                                               int32_t* unmask, void* stream) {
+    if (vocab <= 0 || num_requests < 0 || num_rows < 0) return static_fail(SANGAM_ERR_INVALID_ARG, "confidence_sample_static: bad count");
+    if (num_rows > SANGAM_STATIC_SAMPLER_MAX_ROWS)
+        return static_fail(SANGAM_ERR_WORKSPACE, "confidence_sample_static: num_rows above SANGAM_STATIC_SAMPLER_MAX_ROWS (the static scratch "
+                                                 "array holds no more; use sangam_confidence_sample)");
+    if (num_requests == 0 || num_rows == 0) return SANGAM_OK;
+    if (!logits || !masked || !cu_rows || !token || !conf || !unmask) return static_fail(SANGAM_ERR_INVALID_ARG, "confidence_sample_static: null pointer");
+    if (reinterpret_cast<uintptr_t>(logits) & 1u) return static_fail(SANGAM_ERR_INVALID_ARG, "confidence_sample_static: logits not 2-byte aligned");
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return static_fail(SANGAM_ERR_CUDA, "confidence_sample_static: cudaGetDevice: ", cudaGetErrorString(e));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return static_fail(SANGAM_ERR_UNSUPPORTED, "confidence_sample_static: device ordinal above 63");
+    StaticSamplerDev d;
+    {
+        // set-up, once per device, with that device current (it is: the call runs on the caller's current device)
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        if (!g_static_dev[dev].ready) {
+            void* p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_static_conf_part);
+            if (e != cudaSuccess || !p) return static_fail(SANGAM_ERR_CUDA, "confidence_sample_static: cudaGetSymbolAddress: ", cudaGetErrorString(e));
+            int sms = 0;
+            e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e != cudaSuccess || sms <= 0) return static_fail(SANGAM_ERR_CUDA, "confidence_sample_static: cudaDeviceGetAttribute: ", cudaGetErrorString(e));
+            g_static_dev[dev].part = static_cast<ConfPartial*>(p);
+            g_static_dev[dev].sm_count = sms;
+            g_static_dev[dev].ready = true;
+        }
+        d = g_static_dev[dev];
+    }
+    // same slicing rule as sangam_confidence_sample, capped by the array: num_rows * slices <= MAX_PARTIALS
+    int slices = (8 * d.sm_count + num_rows - 1) / num_rows;
+    const int cap = SANGAM_STATIC_SAMPLER_MAX_PARTIALS / num_rows;
+    slices = slices > cap ? cap : slices;
+    slices = slices < 1 ? 1 : (slices > 64 ? 64 : slices);
+    const int slice_len = ((vocab + slices - 1) / slices + 7) & ~7;
+    slices = (vocab + slice_len - 1) / slice_len;
+    if ((int64_t)num_rows * slices > SANGAM_STATIC_SAMPLER_MAX_PARTIALS)
+        return static_fail(SANGAM_ERR_WORKSPACE, "confidence_sample_static: partials exceed the static scratch array");
+    e = launch_pdl(confidence_pass1_kernel, dim3((unsigned)slices, (unsigned)num_rows), (unsigned)CONF_THREADS, 0, (cudaStream_t)stream,
+                   (const __nv_bfloat16*)logits, vocab, (int32_t)slice_len, d.part);
+    if (e != cudaSuccess) return static_fail(SANGAM_ERR_CUDA, "confidence_sample_static: launch of pass 1: ", cudaGetErrorString(e));
+    e = launch_pdl(confidence_pass2_kernel, dim3((unsigned)((num_requests + 3) / 4)), 128u, 0, (cudaStream_t)stream,
+                   (const ConfPartial*)d.part, (int32_t)slices, masked, cu_rows, num_requests, threshold, token, conf, unmask);
+    if (e != cudaSuccess) return static_fail(SANGAM_ERR_CUDA, "confidence_sample_static: launch of pass 2: ", cudaGetErrorString(e));
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return static_fail(SANGAM_ERR_CUDA, "confidence_sample_static: ", cudaGetErrorString(e));
+    g_static_err[0] = 0;
+    return SANGAM_OK;
+}
