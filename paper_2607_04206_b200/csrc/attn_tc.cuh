@@ -91,7 +91,11 @@ struct Smem {
     static constexpr int OFF_MISC = OFF_ML + BM * 8;
     static constexpr int OFF_SEQ = OFF_MISC + 16 + 64;   // tmem slot, abort word, pad; per-warp wait table (diagnostics)
     static constexpr int TOTAL = OFF_SEQ + 32;           // kv_seq[NSTAGE]
+#ifdef SANGAM_TRACE
+    static constexpr int ALLOC = TOTAL;          // debug trace builds: their static shared memory takes the slack (2 KB static: the base stays aligned)
+#else
     static constexpr int ALLOC = TOTAL + 1024;   // slack to align the base to 1024 B (128B swizzle atoms)
+#endif
 };
 static_assert(sizeof(Item) == 64, "Item is 64 bytes");
 static_assert(Smem<128>::ALLOC <= 232448, "shared memory budget (227 KB)");
@@ -558,12 +562,14 @@ template <int D>
 __device__ __forceinline__ void half_step(MmaState<D>& st, int s, int h, int pv_cols, bool first_pv, uint32_t stage_v, int rel_v,
                                           int qk_cols, uint32_t stage_k, uint32_t qs, int rel_k, int q_rel) {
     using L = Smem<D>;
+    TRACE_EV(60 + s);
     if (pv_cols > 0) {
         uint32_t& par = h ? st.p_par1 : st.p_par0;
         ptx::mbar_wait(st.bar(L::B_P_FULL + 2 * s + h), par, st.abort_flag);
         par ^= 1u;
     }
     ptx::tc_fence_after();
+    TRACE_EV(62 + s);
     if (ptx::elect_one()) {
         const uint32_t sh_tmem = st.tmem + (uint32_t)(s * 128 + h * 64);          // S_s,h / P_s,h
         if (pv_cols > 0) {
@@ -595,6 +601,7 @@ __device__ __forceinline__ void half_step(MmaState<D>& st, int s, int h, int pv_
         }
     }
     __syncwarp();
+    TRACE_EV(64 + s);
 }
 
 // all steps of stream s on kv tile `tile` (PV) and `next` (QK; next < 0: none).  rel = 1 (SHARED) or 2 (SPLIT);
@@ -706,8 +713,13 @@ __device__ __forceinline__ void mma_warp(const AttnParams& p, uint32_t sbase, ui
 // reference maximum m_ref stays).  m_ref is in log2 units and is only raised when the half's maximum
 // exceeds it by more than LAZY_T, so p = 2^(x - m_ref) <= 2^LAZY_T: exact in range for bf16 / fp32.
 // P (bf16 pairs) overwrites the first 32 columns of the half's S buffer.
+// `turn`: 0 = none; else the named barrier this warp waits on before its exponentials (the partner warp of the other
+// stream on the same sub-partition arrives on it after its own), `turn ^ 1` the one it arrives on after: the two warps
+// that share a sub-partition's MUFU alternate instead of contending for it, and each one's loads, maximum, stores and
+// hand-over run in the shadow of the other's exponentials (config 4: 1 970 -> 1 810 us; unsynchronised they fall into lock
+// step, both in the exponentials, then both outside them).
 template <bool MASK>
-__device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float scale_log2, float& m_ref, float& l) {
+__device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float scale_log2, float& m_ref, float& l, uint32_t turn = 0) {
     uint32_t r[2][32];
 #pragma unroll
     for (int c = 0; c < 2; ++c) ptx::tmem_ld32(s_taddr + (uint32_t)(c * 32), r[c]);
@@ -742,6 +754,7 @@ __device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float sc
     // packed fp32x2 arithmetic (FFMA2 / FADD2): one instruction per two columns
     const float2 sc2 = make_float2(scale_log2, scale_log2), ng2 = make_float2(-m_new, -m_new);
     float2 sum_a = make_float2(0.f, 0.f), sum_b = make_float2(0.f, 0.f);
+    if (turn) asm volatile("bar.sync %0, 64;" ::"r"(turn) : "memory");
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
         uint32_t pk[16];
@@ -760,6 +773,7 @@ __device__ __forceinline__ float softmax_half(uint32_t s_taddr, int nv, float sc
         }
         ptx::tmem_st16(s_taddr + (uint32_t)(c * 16), pk);
     }
+    if (turn) asm volatile("bar.arrive %0, 64;" ::"r"(turn ^ 1u) : "memory");
     const float2 sum2 = __fadd2_rn(sum_a, sum_b);
     const float sum0 = sum2.x, sum1 = sum2.y;
     l = l * alpha + (sum0 + sum1);
@@ -818,7 +832,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
     const uint32_t o_taddr = tmem + lane_base + 256u + (uint32_t)s * 128u;     // own accumulator
     const uint32_t o_other = tmem + lane_base + 256u + (uint32_t)(s ^ 1) * 128u;
     float2* ml_x = reinterpret_cast<float2*>(smem + L::OFF_ML);
-    uint32_t icount = 0, hcount0 = 0, hcount1 = 0, pv0 = 0, pv1 = 0, ecount = 0;
+    uint32_t icount = 0, hpar = 0, pv0 = 0, pv1 = 0, ecount = 0;      // hpar: bit h = parity of the next S_FULL wait of half h
     TRACE_NS(40);
     TRACE_EV(36);
     while (true) {
@@ -835,8 +849,15 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         const bool warp_active = wg_warp * 32 < rows_valid;
         float m = -INFINITY, l = 0.f;
         uint32_t steps = 0;                                    // half tiles of this item handed to the issuer
+        // SHARED items: warp w of stream 0 and warp w of stream 1 (same sub-partition) take
+        // turns at the exponentials; barrier 2 + 2 w = "stream 0 may", 3 + 2 w = "stream 1 may".  Stream 1 primes stream 0's.
+        const bool ping = shared && wg_warp * 32 < it.rows0 && wg_warp * 32 < it.rows1;      // both warps of the pair compute
+        const uint32_t turn = ping ? (uint32_t)(2 + 2 * wg_warp + s) : 0u;
+        if (ping && s == 1) asm volatile("bar.arrive %0, 64;" ::"r"(turn ^ 1u) : "memory");
         for (int i = 0; i < ns; ++i) {
-            if (*abort_flag) break;
+            // (after a watchdog abort every wait returns at once; a warp that takes turns with a partner must still run all
+            // of its half steps, or the partner would block for ever on the named barrier)
+            if (!ping) { if (*abort_flag) break; }
             const int tile = shared ? it.kv0 + i : it.kv0 + 2 * i + s;
             int nvt = it.c - tile * BN;
             nvt = nvt > BN ? BN : nvt;
@@ -844,17 +865,16 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
             for (int h = 0; h < 2; ++h) {                     // not unrolled: one copy of the softmax code (instruction cache)
                 const int nv = nvt - h * 64 > 64 ? 64 : nvt - h * 64;
                 if (nv <= 0) continue;                       // the context's last tile may lack half B
-                uint32_t& hcnt = h ? hcount1 : hcount0;
                 TRACE_EV(20 + s);
-                ptx::mbar_wait(bar(L::B_S_FULL + 2 * s + h), hcnt & 1u, abort_flag);
+                ptx::mbar_wait(bar(L::B_S_FULL + 2 * s + h), (hpar >> h) & 1u, abort_flag);
                 TRACE_EV(22 + s);
                 ptx::tc_fence_after();
-                ++hcnt;
+                hpar ^= 1u << h;
                 if (warp_active) {
                     const uint32_t sh = s_taddr + (uint32_t)(h * 64);
                     float alpha;
-                    if (nv == 64) alpha = softmax_half<false>(sh, nv, p.scale_log2, m, l);
-                    else alpha = softmax_half<true>(sh, nv, p.scale_log2, m, l);
+                    if (nv == 64) alpha = softmax_half<false>(sh, nv, p.scale_log2, m, l, turn);
+                    else alpha = softmax_half<true>(sh, nv, p.scale_log2, m, l, turn);
                     if (steps > 0 && __any_sync(FULL, alpha != 1.f)) {
                         // rare (lazy reference maximum): every PV handed over so far must have landed in O first.
                         // Per half at most the latest one is still in flight (the S_FULL just seen was committed
@@ -882,6 +902,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
                 if (h) ++pv1; else ++pv0;
             }
         }
+        if (ping && s == 0) asm volatile("bar.sync %0, 64;" ::"r"(turn) : "memory");      // consume stream 1's last hand-over
         if (steps > 0) {
             ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s), (pv0 - 1u) & 1u, abort_flag);
             ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s + 1), (pv1 - 1u) & 1u, abort_flag);

@@ -88,7 +88,7 @@ __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, volatil
     uint32_t spins = 0;
     bool ok = true;
     while (!mbar_try_wait_hint(bar, parity, SANGAM_WAIT_HINT_NS)) {
-        if ((++spins & 0xFu) == 0 && (*abort_flag || spins > SANGAM_WAIT_MAX_SPINS)) {
+        if (*abort_flag || ++spins > SANGAM_WAIT_MAX_SPINS) {      // (one check per expired 20-us suspension: free)
 #ifdef SANGAM_WAIT_TABLE
             if (!*abort_flag && atomicCAS(&g_timeout_info[0], 0u, bar | 0x80000000u) == 0u) {
                 g_timeout_info[1] = threadIdx.x >> 5; g_timeout_info[2] = blockIdx.x; g_timeout_info[3] = parity;
