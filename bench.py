@@ -189,9 +189,46 @@ class Workload:
         self.eng.kv_write(s["kn"], s["vn"], self.slot_new, s["kp"], s["vp"], stream=stream)
         self.run_attn(s, stream)
 
-    def run_attn(self, s, stream):
-        self.eng.block_attn(s["q"], s["kp"], s["vp"], self.block_table, self.cu_q_lens, self.ctx_lens,
+    def run_attn(self, s, stream, ctx_lens=None):
+        self.eng.block_attn(s["q"], s["kp"], s["vp"], self.block_table, self.cu_q_lens, self.ctx_lens if ctx_lens is None else ctx_lens,
                             float(self.b.scale), s["out"], stream=stream)
+
+    def capture_chain(self, fn):
+        """ONE graph holding a step on every pool set back to back, as the layers of a model sit in one captured iteration:
+        kernel-to-kernel launch latency inside a graph (programmatic dependent launch) instead of graph-to-graph."""
+        import torch
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(self.stream):
+            with torch.cuda.graph(g, stream=self.stream):
+                for s in self.sets:
+                    fn(s, self.stream)
+        torch.cuda.synchronize()
+        return g
+
+    def capture_plan_miss(self):
+        """Attention graphs whose consecutive replays alternate between two metadata sets that differ by one context position
+        (the longest request, one token shorter): the two-stream kernel's per-CTA plan cache, keyed by the lengths, misses on
+        every launch -- what the first layer of a serving iteration pays.  None when there is nothing to vary."""
+        import torch
+        c = self.b.ctx_lens.copy()
+        r = int(np.argmax(c))
+        if c[r] < 2:
+            return None
+        c[r] -= 1
+        alt = _i32(c, self.device)
+        graphs = []
+        with torch.cuda.stream(self.stream):
+            for k in range(2 * self.nsets):
+                s, cl = self.sets[k % self.nsets], (alt if k % 2 else self.ctx_lens)
+                self.run_attn(s, self.stream, cl)
+                self.stream.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=self.stream):
+                    self.run_attn(s, self.stream, cl)
+                graphs.append(g)
+        torch.cuda.synchronize()
+        self._alt_ctx = alt
+        return graphs
 
     def capture(self):
         import torch
@@ -256,6 +293,22 @@ def measure_batch(b: si.Batch, name: str, nsets: int, steps: int, warmup: int, p
                 "device_flags": int(w.eng.device_status())})
     if "kv_write" in parts:
         res["kv_write_gbs"] = round(b.write_bytes() / max(res["kv_write_us"], 1e-9) / 1e3, 1)
+    if w.nsets > 1:      # the same steps with the pool sets' launches chained inside one graph (launch gaps of a layer loop)
+        for key, fn in (("attn", w.run_attn), ("iteration", w.run_iteration)):
+            if key in parts:
+                g = w.capture_chain(fn)
+                k = max(1, steps // w.nsets)
+                per = [w.time_graphs([g], k, max(1, warmup // w.nsets)) / (k * w.nsets) * 1e3 for _ in range(reps)]
+                res[key + "_us_chained"] = round(statistics.median(per), 3)
+        res["chained"] = f"{w.nsets} consecutive steps (one per pool set) captured in ONE graph and replayed; *_us: one step per graph"
+    # The timed replays above repeat one set of lengths, so the two-stream kernel's plan cache (batches of <= 32 requests) hits
+    # on every launch; the miss path is timed beside it.  (The decode kernel plans on every launch: no second figure.)
+    if w.eng.query(4) == 1 and b.batch <= 32:
+        miss = w.capture_plan_miss()
+        if miss is not None:
+            per = [w.time_graphs(miss, steps, warmup) / steps * 1e3 for _ in range(reps)]
+            res["attn_us_plan_miss"] = round(statistics.median(per), 3)
+            res["plan_cache"] = "attn_us: every launch hits the per-CTA plan cache; attn_us_plan_miss: every launch misses (lengths alternate)"
     return res, w
 
 
