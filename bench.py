@@ -606,6 +606,7 @@ def main():
             line["variants"] = measure_variants(peaks)
             line["fig3_sweep"] = measure_fig3(peaks)
             line["sched_series"] = measure_sched_series()
+            line["neighbours"] = measure_neighbours(peaks)
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:
@@ -641,6 +642,82 @@ def measure_fig3(peaks):
             out.append({k: r[k] for k in ("workload", "pool_sets", "attn_us", "attn_us_min", "attn_gbs", "attn_tflops", "bound", "t_roof_us", "roofline_frac", "device_flags")})
             del w
             torch.cuda.empty_cache()
+    return out
+
+
+# ------------------------------------------------------------------------------------------------
+# the HBM-bound kernels next to the path, each against its own algorithmic bytes
+# ------------------------------------------------------------------------------------------------
+def measure_neighbours(peaks):
+    """RoPE-fused KV write, confidence sampler (both entry points), KV page gather / scatter: CUDA-event time of `steps`
+    back-to-back calls on buffers larger than L2 in total (several buffer sets rotate), algorithmic bytes / time against the
+    measured HBM peak.  LLaDA-8B-like geometry (32 kv heads, D 128, vocabulary 126 464)."""
+    import torch
+    import paper_2607_04206_b200 as sg
+    dev = torch.cuda.current_device()
+    Hkv, D, V = 32, 128, 126464
+    out = []
+
+    def timed(fn, nsets, steps=60, warmup=6):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            for i in range(warmup):
+                fn(i % nsets, st)
+            st.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            for i in range(steps):
+                fn(i % nsets, st)
+            e1.record(st)
+            e1.synchronize()
+        return e0.elapsed_time(e1) / steps * 1e3          # us per call
+
+    def rec(name, us, nbytes, note):
+        out.append({"kernel": name, "us": round(us, 2), "algorithmic_bytes": int(nbytes), "gbs": round(nbytes / us / 1e3, 1),
+                    "frac_of_hbm_peak": round(nbytes / us / 1e3 / peaks["hbm_gbs"], 4), "workload": note})
+
+    g = torch.Generator(device="cuda").manual_seed(7)
+    # ---- RoPE-fused KV write: a refresh-sized write (8192 rows) and a decode-sized one (16 x 32 rows)
+    P = 2048
+    eng = sg.Sangam(num_q_heads=Hkv, num_kv_heads=Hkv, head_dim=D, num_pages=P, max_batch=16, max_total_q=8192, max_pages_per_req=512, device=dev)
+    table = torch.from_numpy(sg.rope_table(4096, D)).cuda()
+    for T, nsets in ((8192, 3), (512, 8)):
+        sets = []
+        for _ in range(nsets):
+            k = torch.randn((T, Hkv, D), device="cuda", generator=g).to(torch.bfloat16); v = torch.randn((T, Hkv, D), device="cuda", generator=g).to(torch.bfloat16)
+            kp = torch.zeros((P, Hkv, si.PAGE, D), dtype=torch.bfloat16, device="cuda"); vp = torch.zeros_like(kp)
+            sets.append((k, v, kp, vp))
+        slots = torch.randperm(P * si.PAGE, device="cuda", generator=g)[:T].to(torch.int32)
+        pos = torch.randint(0, 4096, (T,), device="cuda", generator=g, dtype=torch.int32)
+        us = timed(lambda i, st: eng.kv_write_rope(sets[i][0], sets[i][1], slots, pos, table, sets[i][2], sets[i][3], stream=st), nsets)
+        rec("kv_write_rope", us, 2 * (2 * 2 * T * Hkv * D) + 8 * T + T * D * 4, f"{T} new rows x {Hkv} kv heads x {D}, table rows from L2")
+        del sets
+    # ---- confidence sampler: one decode iteration's rows (16 requests x 32 rows) at LLaDA's vocabulary
+    rows, nsets = 512, 3
+    lsets = [(2.0 * torch.randn((rows, V), device="cuda", generator=g)).to(torch.bfloat16) for _ in range(nsets)]
+    masked = torch.ones(rows, dtype=torch.int32, device="cuda"); cu = torch.arange(0, rows + 1, 32, dtype=torch.int32, device="cuda")
+    tok = torch.empty(rows, dtype=torch.int32, device="cuda"); conf = torch.empty(rows, dtype=torch.float32, device="cuda"); un = torch.empty(rows, dtype=torch.int32, device="cuda")
+    nbytes = rows * V * 2 + rows * 16
+    us = timed(lambda i, st: eng.confidence_sample(lsets[i], masked, cu, 0.9, tok, conf, un, stream=st), nsets)
+    rec("confidence_sample", us, nbytes, f"{rows} rows x vocabulary {V} (bf16 logits read once)")
+    us = timed(lambda i, st: sg.confidence_sample_static(lsets[i], masked, cu, 0.9, tok, conf, un, stream=st), nsets)
+    rec("confidence_sample_static", us, nbytes, "same, through the entry point that allocates nothing")
+    del lsets
+    # ---- KV page gather / scatter: one request of 4096 tokens (256 pages)
+    npg, nsets = 256, 3
+    pools = [(torch.randn((P, Hkv, si.PAGE, D), device="cuda", generator=g).to(torch.bfloat16), torch.randn((P, Hkv, si.PAGE, D), device="cuda", generator=g).to(torch.bfloat16)) for _ in range(nsets)]
+    ids = [torch.randperm(P, device="cuda", generator=g)[:npg].to(torch.int32) for _ in range(nsets)]
+    ks = torch.empty((npg, Hkv, si.PAGE, D), dtype=torch.bfloat16, device="cuda"); vs = torch.empty_like(ks)
+    nbytes = 2 * 2 * npg * Hkv * si.PAGE * D * 2 + 4 * npg
+    us = timed(lambda i, st: eng.kv_gather(pools[i][0], pools[i][1], ids[i], ks, vs, stream=st), nsets)
+    rec("kv_gather", us, nbytes, f"{npg} pages x {Hkv} kv heads (a 4096-token request), K and V")
+    us = timed(lambda i, st: eng.kv_scatter(ks, vs, ids[i], pools[i][0], pools[i][1], stream=st), nsets)
+    rec("kv_scatter", us, nbytes, "the same pages back into a pool")
+    flags = int(eng.device_status())
+    for r in out:
+        r["device_flags"] = flags
+    del pools
+    torch.cuda.empty_cache()
     return out
 
 

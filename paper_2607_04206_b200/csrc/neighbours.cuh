@@ -15,6 +15,7 @@
 //      pass 2 merges the slices per row and takes the per-request decision.
 #pragma once
 #include "common.cuh"
+#include "ptx.cuh"
 
 // one thread-iteration = one 16-byte chunk (8 bf16) of a K row's LOWER half and the matching chunk of its upper half
 __global__ void __launch_bounds__(256)
@@ -87,56 +88,169 @@ __device__ __forceinline__ void conf_merge(float& m, float& sum, int32_t& arg, f
 }
 
 constexpr int CONF_THREADS = 256;
-// grid = (slices, rows): block (s, t) scans logits[t][s * slice_len .. +slice_len)
-__global__ void __launch_bounds__(CONF_THREADS)
-confidence_pass1_kernel(const __nv_bfloat16* __restrict__ logits, int32_t V, int32_t slice_len, ConfPartial* __restrict__ part) {
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    const int32_t t = blockIdx.y, sl = blockIdx.x;
-    const int32_t lo = sl * slice_len, hi = min(V, lo + slice_len);
-    const __nv_bfloat16* row = logits + (int64_t)t * V;
-    float m = -INFINITY, sum = 0.f;
-    int32_t arg = 0x7fffffff;
-    // 16-byte vector loads over the aligned middle of the slice, scalar loads at its ragged ends
-    const uintptr_t a0 = reinterpret_cast<uintptr_t>(row + lo);
-    int32_t head = (int32_t)(((16 - (a0 & 15)) & 15) / 2);
-    head = min(head, hi - lo);
-    auto visit = [&](float x, int32_t j) {
-        if (x > m) { sum = sum * __expf(m - x) + 1.f; m = x; arg = j; }
-        else if (x == m) { sum += 1.f; arg = j < arg ? j : arg; }
-        else sum += __expf(x - m);
-    };
-    for (int32_t j = lo + threadIdx.x; j < lo + head; j += CONF_THREADS) visit(__bfloat162float(row[j]), j);
-    const int32_t nvec = (hi - lo - head) / 8;
-    const uint4* vec = reinterpret_cast<const uint4*>(row + lo + head);
-    for (int32_t q = threadIdx.x; q < nvec; q += CONF_THREADS) {
-        const uint4 w = __ldcs(vec + q);
-        const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
-        const int32_t j0 = lo + head + q * 8;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            visit(__uint_as_float(ww[e] << 16), j0 + 2 * e);
-            visit(__uint_as_float(ww[e] & 0xffff0000u), j0 + 2 * e + 1);
-        }
-    }
-    for (int32_t j = lo + head + nvec * 8 + threadIdx.x; j < hi; j += CONF_THREADS) visit(__bfloat162float(row[j]), j);
-    // block reduction
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        const float m2 = __shfl_xor_sync(0xffffffffu, m, o), s2 = __shfl_xor_sync(0xffffffffu, sum, o);
-        const int32_t a2 = __shfl_xor_sync(0xffffffffu, arg, o);
-        conf_merge(m, sum, arg, m2, s2, a2);
-    }
+// Persistent blocks (the grid fills the machine once): block b takes the work items b, b + gridDim.x, ...; item = (row t, slice
+// sl) scans logits[t][sl * slice_len .. + slice_len).  Consecutive items are consecutive slices of a row, so neighbouring
+// blocks stream neighbouring memory.
+// The logits are streamed through a shared-memory ring by 1-D bulk copies (cp.async.bulk + mbarrier): thread 0 keeps
+// CONF_NST chunks of CONF_CHUNK bytes in flight per block, across item boundaries, so the bytes in flight per SM (3 - 4 blocks x
+// 40 KB) cover the HBM latency whatever the exponentials cost; with plain loads 4 x 16 B per thread the kernel ran at half
+// the bandwidth (memory latency and MUFU time in series).
+constexpr int CONF_CHUNK = 8192;                      // bytes per stage = 2 vectors of 8 logits per consumer thread
+constexpr int CONF_NST = 5;
+constexpr int CONF_BLOCK = CONF_THREADS + 32;         // 8 consumer warps + 1 producer warp
+__global__ void __launch_bounds__(CONF_BLOCK)
+confidence_pass1_kernel(const __nv_bfloat16* __restrict__ logits, int32_t V, int32_t slice_len, int32_t slices, int32_t num_items,
+                        ConfPartial* __restrict__ part) {
+    __shared__ __align__(128) uint8_t ring[CONF_NST * CONF_CHUNK];
+    __shared__ __align__(8) unsigned long long full[CONF_NST], empty[CONF_NST];
     __shared__ float sm[CONF_THREADS / 32], ss[CONF_THREADS / 32];
     __shared__ int32_t sa[CONF_THREADS / 32];
-    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-    if (l == 0) { sm[w] = m; ss[w] = sum; sa[w] = arg; }
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        for (int s_ = 0; s_ < CONF_NST; ++s_) { ptx::mbar_init(ptx::smem_u32(&full[s_]), 1); ptx::mbar_init(ptx::smem_u32(&empty[s_]), CONF_THREADS); }
+        ptx::fence_mbar_init();
+    }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int k = 1; k < CONF_THREADS / 32; ++k) conf_merge(m, sum, arg, sm[k], ss[k], sa[k]);
-        ConfPartial p;
-        p.m = m; p.sum = sum; p.arg = arg; p.pad = 0;
-        part[(int64_t)t * gridDim.x + sl] = p;
+    // geometry of an item: [lo, hi) of its row, `head` scalar elements up to the first 16-byte boundary, nvec whole vectors
+    auto geom = [&](int32_t item, int32_t& t, int32_t& lo, int32_t& hi, int32_t& head, int32_t& nvec) {
+        t = item / slices;
+        const int32_t sl = item - t * slices;
+        lo = sl * slice_len; hi = min(V, lo + slice_len);
+        const uintptr_t a0 = reinterpret_cast<uintptr_t>(logits + (int64_t)t * V + lo);
+        head = min((int32_t)(((16 - (a0 & 15)) & 15) / 2), hi - lo);
+        nvec = (hi - lo - head) / 8;
+    };
+    auto wait = [&](unsigned long long* b_, uint32_t ph) {
+        const uint32_t bar = ptx::smem_u32(b_);
+        uint32_t spins = 0;
+        while (!ptx::mbar_try_wait_hint(bar, ph, 10000u))
+            if (++spins > (1u << 20)) break;                        // (never in a correct run: no hang, wrong numbers instead)
+    };
+    if (tid >= CONF_THREADS) {
+        // ---- producer warp (one lane): the block's flattened chunk stream, CONF_NST chunks ahead of the consumers
+        if (tid == CONF_THREADS) {
+            uint32_t issued = 0;
+            for (int32_t item = blockIdx.x; item < num_items; item += gridDim.x) {
+                int32_t t, lo, hi, head, nvec;
+                geom(item, t, lo, hi, head, nvec);
+                const uint8_t* src = reinterpret_cast<const uint8_t*>(logits + (int64_t)t * V + lo + head);
+                for (int32_t left = nvec * 16; left > 0; left -= CONF_CHUNK, src += CONF_CHUNK, ++issued) {
+                    const uint32_t st = issued % CONF_NST, use = issued / CONF_NST;
+                    if (use > 0) wait(&empty[st], (use - 1u) & 1u);            // every consumer thread has the previous use in registers
+                    const uint32_t bytes = (uint32_t)(left < CONF_CHUNK ? left : CONF_CHUNK);
+                    ptx::mbar_arrive_expect_tx(ptx::smem_u32(&full[st]), bytes);
+                    ptx::bulk_load(ptx::smem_u32(ring + st * CONF_CHUNK), src, bytes, ptx::smem_u32(&full[st]));
+                }
+            }
+        }
+        return;
+    }
+    // ---- consumer warps
+    const float LOG2E = 1.4426950408889634f;
+    uint32_t cons = 0;                          // chunks consumed so far
+    for (int32_t item = blockIdx.x; item < num_items; item += gridDim.x) {
+        int32_t t, lo, hi, head, nvec;
+        geom(item, t, lo, hi, head, nvec);
+        const __nv_bfloat16* row = logits + (int64_t)t * V;
+        float m = -INFINITY, sum = 0.f;
+        int32_t arg = 0x7fffffff;
+        auto visit = [&](float x, int32_t j) {
+            if (x > m) { sum = sum * __expf(m - x) + 1.f; m = x; arg = j; }
+            else if (x == m) { sum += 1.f; arg = j < arg ? j : arg; }
+            else sum += __expf(x - m);
+        };
+        for (int32_t j = lo + tid; j < lo + head; j += CONF_THREADS) visit(__bfloat162float(row[j]), j);
+        // A thread meets its indices in increasing order, so only a strictly larger value moves (m, arg) (an equal one keeps
+        // the earlier index).  The maximum of a chunk's 16 logits is taken first, so that test is made once per chunk, and
+        // the rest is branch-free: exp(x - m) =
+        // ex2(x log2e - m log2e), one packed FFMA per two logits and one MUFU each.  A vector past the slice's end reads as
+        // eight -inf (exp = 0).
+        auto unpack = [](const uint4& w, float (&x)[8]) {
+            x[0] = __uint_as_float(w.x << 16); x[1] = __uint_as_float(w.x & 0xffff0000u);
+            x[2] = __uint_as_float(w.y << 16); x[3] = __uint_as_float(w.y & 0xffff0000u);
+            x[4] = __uint_as_float(w.z << 16); x[5] = __uint_as_float(w.z & 0xffff0000u);
+            x[6] = __uint_as_float(w.w << 16); x[7] = __uint_as_float(w.w & 0xffff0000u);
+        };
+        auto max8 = [](const float (&x)[8]) {
+            return fmaxf(fmaxf(fmaxf(x[0], x[1]), fmaxf(x[2], x[3])), fmaxf(fmaxf(x[4], x[5]), fmaxf(x[6], x[7])));
+        };
+        auto first_of = [](const float (&x)[8], float mx) {         // lowest e with x[e] == mx, 8 if none
+            int32_t k = 8;
+#pragma unroll
+            for (int e = 7; e >= 0; --e) k = x[e] == mx ? e : k;
+            return k;
+        };
+        auto sum8 = [&](const float (&x)[8], float2 nm2) {          // sum of ex2(x log2e + nm2)
+            const float2 sc2 = make_float2(LOG2E, LOG2E);
+            float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int e = 0; e < 8; e += 2) {
+                const float2 y = __ffma2_rn(make_float2(x[e], x[e + 1]), sc2, nm2);
+                acc = __fadd2_rn(acc, make_float2(ptx::ex2(y.x), ptx::ex2(y.y)));
+            }
+            return acc.x + acc.y;
+        };
+        const uint4 NEG = make_uint4(0xff80ff80u, 0xff80ff80u, 0xff80ff80u, 0xff80ff80u);       // bf16 -inf x 8
+        const int32_t nchunks = (nvec * 16 + CONF_CHUNK - 1) / CONF_CHUNK;
+        int32_t cbest = -1;                                        // chunk in which this thread's maximum was last raised
+        for (int32_t c = 0; c < nchunks; ++c, ++cons) {
+            const uint32_t st = cons % CONF_NST;
+            wait(&full[st], (cons / CONF_NST) & 1u);
+            const int32_t v0 = c * (CONF_CHUNK / 16) + tid, v1 = v0 + CONF_THREADS;      // vector indices inside the slice
+            const uint4* stage = reinterpret_cast<const uint4*>(ring + st * CONF_CHUNK);
+            const uint4 w0 = v0 < nvec ? stage[tid] : NEG, w1 = v1 < nvec ? stage[tid + CONF_THREADS] : NEG;
+            float x0[8], x1[8];
+            unpack(w0, x0); unpack(w1, x1);
+            const float mx = fmaxf(max8(x0), max8(x1));
+            // Release the stage only when the 32 bytes are in registers: the arrive takes `mx` (which depends on every loaded
+            // word) as an operand, so it issues after the loads have returned.  An arrive right behind the LDS instructions
+            // let the producer's next bulk copy overwrite the stage under loads still queued in the shared-memory pipe.
+            {
+                // (the barrier address is made to depend on mx: a value with nonzero low mantissa bits cannot come out of bf16
+                // logits, so the offset is always 0, but neither compiler can know that and drop the dependency)
+                const uint32_t off = __float_as_uint(mx) == 0x7fc00001u ? 8u : 0u;
+                ptx::mbar_arrive(ptx::smem_u32(&empty[st]) + off);                        // every consumer thread arrives
+            }
+            if (mx > m) {                                          // new maximum: remember the chunk, find the index later
+                sum *= __expf(m - mx);                             // (m = -inf, sum = 0: 0 * 0)
+                m = mx; cbest = c;
+            }
+            const float nm = -fmaxf(m, -1.0e30f) * LOG2E;          // (nothing but -inf so far: ex2(-inf + 1.4e30) = 0, not NaN)
+            const float2 nm2 = make_float2(nm, nm);
+            sum += sum8(x0, nm2) + sum8(x1, nm2);
+        }
+        if (cbest >= 0) {
+            // the index of the maximum: this thread's two vectors of the chunk that raised it last are read again (from L2),
+            // once per item, instead of 32 compare / select instructions in every chunk
+            const int32_t v0 = cbest * (CONF_CHUNK / 16) + tid, v1 = v0 + CONF_THREADS;
+            const uint4* vec = reinterpret_cast<const uint4*>(row + lo + head);
+            const uint4 w0 = __ldg(vec + v0), w1 = v1 < nvec ? __ldg(vec + v1) : NEG;
+            float x0[8], x1[8];
+            unpack(w0, x0); unpack(w1, x1);
+            const int32_t k0 = first_of(x0, m), k1 = first_of(x1, m);
+            const int32_t jb = lo + head + v0 * 8;
+            arg = k0 < 8 ? jb + k0 : jb + CONF_THREADS * 8 + k1;
+        }
+        for (int32_t j = lo + head + nvec * 8 + tid; j < hi; j += CONF_THREADS) visit(__bfloat162float(row[j]), j);
+        // block reduction (the 256 consumer threads: named barrier 1)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const float m2 = __shfl_xor_sync(0xffffffffu, m, o), s2 = __shfl_xor_sync(0xffffffffu, sum, o);
+            const int32_t a2 = __shfl_xor_sync(0xffffffffu, arg, o);
+            conf_merge(m, sum, arg, m2, s2, a2);
+        }
+        const int w = tid >> 5, l = tid & 31;
+        if (l == 0) { sm[w] = m; ss[w] = sum; sa[w] = arg; }
+        asm volatile("bar.sync 1, %0;" ::"n"(CONF_THREADS) : "memory");
+        if (tid == 0) {
+            for (int k = 1; k < CONF_THREADS / 32; ++k) conf_merge(m, sum, arg, sm[k], ss[k], sa[k]);
+            ConfPartial p;
+            p.m = m; p.sum = sum; p.arg = arg; p.pad = 0;
+            part[item] = p;                                        // = [t][sl]
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(CONF_THREADS) : "memory");       // the staging arrays are reused by the next item
     }
 }
 

@@ -243,6 +243,29 @@ extern "C" int sangam_kv_write_rope(sangam_ctx* ctx, const void* k, const void* 
     return SANGAM_OK;
 }
 
+// Slicing of the sampler's first pass.  Work items = (row, vocabulary slice); a grid of persistent blocks (at most the
+// CONF_BLOCKS_PER_SM x #SM that are resident at once) takes them round robin.  An item costs a block reduction, so slices are
+// as long as they can be while the items still fill the machine: slices = ceil(resident blocks / rows), at most `cap` (and
+// 64) per row, never shorter than 4096 logits; the grid is then shrunk so that every block gets the same number of items.
+#ifndef SANGAM_CONF_BPS
+#define SANGAM_CONF_BPS 5
+#endif
+constexpr int CONF_BLOCKS_PER_SM = SANGAM_CONF_BPS;          // 288 threads x 38 registers, 41 KB of shared memory: 5 per SM
+static void conf_slicing(int sm_count, int num_rows, int vocab, int cap, int* slices_out, int* slice_len_out, unsigned* grid_out) {
+    const int resident = CONF_BLOCKS_PER_SM * sm_count;
+    int slices = (resident + num_rows - 1) / num_rows;
+    const int by_len = (vocab + 4095) / 4096;
+    slices = slices > by_len ? by_len : slices;
+    slices = slices > cap ? cap : slices;
+    slices = slices < 1 ? 1 : (slices > 64 ? 64 : slices);
+    const int slice_len = ((vocab + slices - 1) / slices + 7) & ~7;
+    slices = (vocab + slice_len - 1) / slice_len;
+    const int64_t items = (int64_t)num_rows * slices;
+    const int64_t rounds = (items + resident - 1) / resident;
+    *slices_out = slices; *slice_len_out = slice_len;
+    *grid_out = (unsigned)((items + rounds - 1) / rounds);
+}
+
 extern "C" int sangam_confidence_sample(sangam_ctx* ctx, const void* logits, int32_t vocab, const int32_t* masked, const int32_t* cu_rows,
                                         int32_t num_requests, int32_t num_rows, float threshold, int32_t* token, float* conf,
                                         int32_t* unmask, void* stream) {
@@ -252,11 +275,9 @@ extern "C" int sangam_confidence_sample(sangam_ctx* ctx, const void* logits, int
     if (!logits || !masked || !cu_rows || !token || !conf || !unmask) return fail(ctx, SANGAM_ERR_INVALID_ARG, "confidence_sample: null pointer");
     if (reinterpret_cast<uintptr_t>(logits) & 1u) return fail(ctx, SANGAM_ERR_INVALID_ARG, "confidence_sample: logits not 2-byte aligned");
     ON_CTX_DEVICE(ctx);
-    // enough (row, slice) blocks to fill the machine a few times over; slices of a multiple of 8 elements
-    int slices = (8 * ctx->sm_count + num_rows - 1) / num_rows;
-    slices = slices < 1 ? 1 : (slices > 64 ? 64 : slices);
-    int slice_len = ((vocab + slices - 1) / slices + 7) & ~7;
-    slices = (vocab + slice_len - 1) / slice_len;
+    int slices, slice_len;
+    unsigned grid;
+    conf_slicing(ctx->sm_count, num_rows, vocab, 1 << 30, &slices, &slice_len, &grid);
     const int64_t need = (int64_t)num_rows * slices;
     if (need > ctx->conf_part_cap) {                       // first use / larger batch: (re)allocate (not during graph capture)
         cudaFree(ctx->d_conf_part); ctx->d_conf_part = nullptr; ctx->conf_part_cap = 0;
@@ -264,8 +285,8 @@ extern "C" int sangam_confidence_sample(sangam_ctx* ctx, const void* logits, int
         CK(cudaMalloc(&ctx->d_conf_part, (size_t)cap * sizeof(ConfPartial)));
         ctx->conf_part_cap = cap;
     }
-    CK(launch_pdl(confidence_pass1_kernel, dim3((unsigned)slices, (unsigned)num_rows), (unsigned)CONF_THREADS, 0, (cudaStream_t)stream,
-                  (const __nv_bfloat16*)logits, vocab, (int32_t)slice_len, ctx->d_conf_part));
+    CK(launch_pdl(confidence_pass1_kernel, dim3(grid), (unsigned)CONF_BLOCK, 0, (cudaStream_t)stream,
+                  (const __nv_bfloat16*)logits, vocab, (int32_t)slice_len, (int32_t)slices, (int32_t)need, ctx->d_conf_part));
     CK(launch_pdl(confidence_pass2_kernel, dim3((unsigned)((num_requests + 3) / 4)), 128u, 0, (cudaStream_t)stream,
                   (const ConfPartial*)ctx->d_conf_part, (int32_t)slices, masked, cu_rows, num_requests, threshold, token, conf, unmask));
     ctx->launches += 2;
@@ -660,16 +681,13 @@ extern "C" int sangam_confidence_sample_static(const void* logits, int32_t vocab
         d = g_static_dev[dev];
     }
     // same slicing rule as sangam_confidence_sample, capped by the array: num_rows * slices <= MAX_PARTIALS
-    int slices = (8 * d.sm_count + num_rows - 1) / num_rows;
-    const int cap = SANGAM_STATIC_SAMPLER_MAX_PARTIALS / num_rows;
-    slices = slices > cap ? cap : slices;
-    slices = slices < 1 ? 1 : (slices > 64 ? 64 : slices);
-    const int slice_len = ((vocab + slices - 1) / slices + 7) & ~7;
-    slices = (vocab + slice_len - 1) / slice_len;
+    int slices, slice_len;
+    unsigned grid;
+    conf_slicing(d.sm_count, num_rows, vocab, SANGAM_STATIC_SAMPLER_MAX_PARTIALS / num_rows, &slices, &slice_len, &grid);
     if ((int64_t)num_rows * slices > SANGAM_STATIC_SAMPLER_MAX_PARTIALS)
         return static_fail(SANGAM_ERR_WORKSPACE, "confidence_sample_static: partials exceed the static scratch array");
-    e = launch_pdl(confidence_pass1_kernel, dim3((unsigned)slices, (unsigned)num_rows), (unsigned)CONF_THREADS, 0, (cudaStream_t)stream,
-                   (const __nv_bfloat16*)logits, vocab, (int32_t)slice_len, d.part);
+    e = launch_pdl(confidence_pass1_kernel, dim3(grid), (unsigned)CONF_BLOCK, 0, (cudaStream_t)stream,
+                   (const __nv_bfloat16*)logits, vocab, (int32_t)slice_len, (int32_t)slices, (int32_t)(num_rows * slices), d.part);
     if (e != cudaSuccess) return static_fail(SANGAM_ERR_CUDA, "confidence_sample_static: launch of pass 1: ", cudaGetErrorString(e));
     e = launch_pdl(confidence_pass2_kernel, dim3((unsigned)((num_requests + 3) / 4)), 128u, 0, (cudaStream_t)stream,
                    (const ConfPartial*)d.part, (int32_t)slices, masked, cu_rows, num_requests, threshold, token, conf, unmask);
