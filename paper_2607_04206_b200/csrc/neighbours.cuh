@@ -195,6 +195,7 @@ confidence_pass1_kernel(const __nv_bfloat16* __restrict__ logits, int32_t V, int
         const uint4 NEG = make_uint4(0xff80ff80u, 0xff80ff80u, 0xff80ff80u, 0xff80ff80u);       // bf16 -inf x 8
         const int32_t nchunks = (nvec * 16 + CONF_CHUNK - 1) / CONF_CHUNK;
         int32_t cbest = -1;                                        // chunk in which this thread's maximum was last raised
+        uint4 wb0 = NEG, wb1 = NEG;                                // ... and the thread's two vectors of that chunk
         for (int32_t c = 0; c < nchunks; ++c, ++cons) {
             const uint32_t st = cons % CONF_NST;
             wait(&full[st], (cons / CONF_NST) & 1u);
@@ -213,24 +214,21 @@ confidence_pass1_kernel(const __nv_bfloat16* __restrict__ logits, int32_t V, int
                 const uint32_t off = __float_as_uint(mx) == 0x7fc00001u ? 8u : 0u;
                 ptx::mbar_arrive(ptx::smem_u32(&empty[st]) + off);                        // every consumer thread arrives
             }
-            if (mx > m) {                                          // new maximum: remember the chunk, find the index later
+            if (mx > m) {                                          // new maximum: keep the chunk's vectors, find the index later
                 sum *= __expf(m - mx);                             // (m = -inf, sum = 0: 0 * 0)
-                m = mx; cbest = c;
+                m = mx; cbest = c; wb0 = w0; wb1 = w1;
             }
             const float nm = -fmaxf(m, -1.0e30f) * LOG2E;          // (nothing but -inf so far: ex2(-inf + 1.4e30) = 0, not NaN)
             const float2 nm2 = make_float2(nm, nm);
             sum += sum8(x0, nm2) + sum8(x1, nm2);
         }
         if (cbest >= 0) {
-            // the index of the maximum: this thread's two vectors of the chunk that raised it last are read again (from L2),
-            // once per item, instead of 32 compare / select instructions in every chunk
-            const int32_t v0 = cbest * (CONF_CHUNK / 16) + tid, v1 = v0 + CONF_THREADS;
-            const uint4* vec = reinterpret_cast<const uint4*>(row + lo + head);
-            const uint4 w0 = __ldg(vec + v0), w1 = v1 < nvec ? __ldg(vec + v1) : NEG;
+            // the index of the maximum, once per item, from the kept copy of the two vectors that raised it last (8 registers)
+            // instead of 32 compare / select instructions in every chunk
             float x0[8], x1[8];
-            unpack(w0, x0); unpack(w1, x1);
+            unpack(wb0, x0); unpack(wb1, x1);
             const int32_t k0 = first_of(x0, m), k1 = first_of(x1, m);
-            const int32_t jb = lo + head + v0 * 8;
+            const int32_t jb = lo + head + (cbest * (CONF_CHUNK / 16) + tid) * 8;
             arg = k0 < 8 ? jb + k0 : jb + CONF_THREADS * 8 + k1;
         }
         for (int32_t j = lo + head + nvec * 8 + tid; j < hi; j += CONF_THREADS) visit(__bfloat162float(row[j]), j);
