@@ -833,6 +833,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
     const uint32_t o_other = tmem + lane_base + 256u + (uint32_t)(s ^ 1) * 128u;
     float2* ml_x = reinterpret_cast<float2*>(smem + L::OFF_ML);
     uint32_t icount = 0, hpar = 0, pv0 = 0, pv1 = 0, ecount = 0;      // hpar: bit h = parity of the next S_FULL wait of half h
+    bool owed = false;               // stream 1: the boundary barrier of its last turn-taking item is still to be waited on
     TRACE_NS(40);
     TRACE_EV(36);
     while (true) {
@@ -853,7 +854,10 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         // turns at the exponentials; barrier 2 + 2 w = "stream 0 may", 3 + 2 w = "stream 1 may".  Stream 1 primes stream 0's.
         const bool ping = shared && wg_warp * 32 < it.rows0 && wg_warp * 32 < it.rows1;      // both warps of the pair compute
         const uint32_t turn = ping ? (uint32_t)(2 + 2 * wg_warp + s) : 0u;
-        if (ping && s == 1) asm volatile("bar.arrive %0, 64;" ::"r"(turn ^ 1u) : "memory");
+        if (ping && s == 1) {
+            if (owed) { asm volatile("bar.sync %0, 64;" ::"r"(10u + (uint32_t)wg_warp) : "memory"); owed = false; }
+            asm volatile("bar.arrive %0, 64;" ::"r"(turn ^ 1u) : "memory");
+        }
         for (int i = 0; i < ns; ++i) {
             // (after a watchdog abort every wait returns at once; a warp that takes turns with a partner must still run all
             // of its half steps, or the partner would block for ever on the named barrier)
@@ -902,7 +906,17 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
                 if (h) ++pv1; else ++pv0;
             }
         }
-        if (ping && s == 0) asm volatile("bar.sync %0, 64;" ::"r"(turn) : "memory");      // consume stream 1's last hand-over
+        if (ping) {
+            if (s == 0) {
+                asm volatile("bar.sync %0, 64;" ::"r"(turn) : "memory");                  // consume stream 1's last hand-over
+                // ... and only then may stream 1 prime its next turn-taking item (it does so after its epilogue; should stream
+                // 0 be held up meanwhile -- a late O rescale -- the prime would land in the generation that is still open).
+                // Barrier 10 + w: stream 0 arrives here, stream 1 waits on it just before its next prime (`owed`).
+                asm volatile("bar.arrive %0, 64;" ::"r"(10u + (uint32_t)wg_warp) : "memory");
+            } else {
+                owed = true;
+            }
+        }
         if (steps > 0) {
             ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s), (pv0 - 1u) & 1u, abort_flag);
             ptx::mbar_wait(bar(L::B_PV_DONE + 2 * s + 1), (pv1 - 1u) & 1u, abort_flag);
@@ -980,6 +994,7 @@ __device__ __forceinline__ void softmax_wg(const AttnParams& p, uint8_t* smem, u
         if (lane == 0) ptx::mbar_arrive(bar(L::B_ITEM_EMPTY + islot));
         ++icount;
     }
+    if (owed) asm volatile("bar.sync %0, 64;" ::"r"(10u + (uint32_t)wg_warp) : "memory");     // balance stream 0's last arrive
     TRACE_EV(35);
     TRACE_NS(41);
 }
